@@ -1,0 +1,196 @@
+/*
+ * hcms.h -- C ABI of libhcms: the HCMS (Head-Chunked Multi-Stream) attention hot path,
+ * emulated on ONE NVIDIA B200 (sm_100a).
+ *
+ * Source of the method: arxiv/paper_2607_01817 (PAPER.md; "L<n>" = PAPER.md line).
+ *   - Ulysses all-to-all sequence parallelism: the input all-to-all turns "sequence-sharded,
+ *     heads-complete" activations into "sequence-complete, heads-sharded" ones, attention runs,
+ *     the output all-to-all inverts the layout (L45, L59).
+ *   - HCMS splits the heads of every rank into C chunks (Eq. 3; Table 8),
+ *     runs all all-to-alls on a communication stream and all attention calls on a compute
+ *     stream, ordered by CUDA events (section 3.4-3.5; Algorithm 1).
+ *
+ * Emulation: the P ranks are logical.  The concatenation, in rank order, of the P ranks'
+ * shards [S/P, H, D] is the global tensor [S, H, D]; rank p owns global heads
+ * [p*Hl, (p+1)*Hl), Hl = H/P; chunk c is local heads [o_c, o_c+h_c) on every rank with
+ * h_c = floor(Hl/C) + 1[c < Hl mod C], o_c = sum_{c'<c} h_c'.  The all-to-all is a device
+ * layout kernel writing the head-sharded chunk buffer
+ *
+ *        X'_c [P][S][h_c][D]   with   X'_c[p][s][j][d] = X[s][p*Hl + o_c + j][d]
+ *
+ * (row-major, densely packed); this layout is part of the contract.
+ *
+ * Conventions
+ *   - every function is extern "C", returns an int status (HCMS_OK == 0, errors < 0) unless it
+ *     returns a size or a string, never throws, never exits, never synchronises the host
+ *     unless stated;
+ *   - "device pointer" = CUDA device memory owned by the caller; "host pointer" = ordinary host
+ *     memory owned by the caller; the library never frees caller memory;
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream);
+ *   - there is NO CPU fallback: without a compute-capability-10.x device every call that needs
+ *     the GPU returns HCMS_ERR_UNSUPPORTED_DEVICE or HCMS_ERR_CUDA.
+ */
+#ifndef HCMS_H_
+#define HCMS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define HCMS_VERSION 100 /* major*10000 + minor*100 + patch */
+
+/* ---- status codes ------------------------------------------------------------------- */
+enum {
+  HCMS_OK = 0,
+  HCMS_ERR_INVALID_ARG = -1,         /* NULL pointer, non-positive size, non-finite or negative scale */
+  HCMS_ERR_UNSUPPORTED_SHAPE = -2,   /* S%P, H%P, C>H/P, D not in {64,128}, D*es%16 */
+  HCMS_ERR_UNSUPPORTED_DTYPE = -3,   /* attention needs bf16; layout kernels take 2- or 4-byte elements */
+  HCMS_ERR_UNSUPPORTED_DEVICE = -4,  /* no CUDA device of compute capability 10.x */
+  HCMS_ERR_MISALIGNED = -5,          /* a device pointer is not 16-byte aligned */
+  HCMS_ERR_ALIAS = -6,               /* `out` overlaps q, k or v */
+  HCMS_ERR_PLAN_MISMATCH = -7,       /* S,H,D,P,C differ from the plan's, or chunk index out of range */
+  HCMS_ERR_WORKSPACE_TOO_SMALL = -8,
+  HCMS_ERR_CUDA = -9                 /* a CUDA call failed; hcms_last_error() carries its text */
+};
+
+/* ---- element types ------------------------------------------------------------------ */
+enum {
+  HCMS_DTYPE_BF16 = 0, /* 2 bytes; the only type hcms_attention_* accepts */
+  HCMS_DTYPE_F32 = 1,  /* 4 bytes; layout kernels only (BASELINE.json config 1's permutation check) */
+  HCMS_DTYPE_F16 = 2   /* 2 bytes; layout kernels only */
+};
+
+/* ---- plan flags ----------------------------------------------------------------------- */
+#define HCMS_FLAG_SERIAL 0x1u          /* Ulysses baseline order (Eq. 1): all scatters, all
+                                          attention, all gathers, on the caller's stream, no overlap */
+#define HCMS_FLAG_LAYOUT_TMA 0x2u      /* layout kernels use the TMA bulk-tensor variant instead of the
+                                          128-bit ld/st variant (same bits out) */
+#define HCMS_FLAG_SPLIT_COMM 0x4u      /* separate streams for input and output all-to-all (Eq. 8
+                                          "all three in parallel"); default is Alg. 1's single S_comm */
+#define HCMS_FLAG_HOST_ROUTE_Q 0x10u   /* config 5: route this tensor's chunk buffer through pinned host */
+#define HCMS_FLAG_HOST_ROUTE_K 0x20u   /* memory (cudaMemcpyAsync D2H then H2D) after the scatter kernel */
+#define HCMS_FLAG_HOST_ROUTE_V 0x40u   /* (Q,K,V) or before the gather kernel (O) to raise the          */
+#define HCMS_FLAG_HOST_ROUTE_O 0x80u   /* communication ratio rho (section 3.7)                    */
+#define HCMS_FLAG_DEBUG_NO_COMM_WAIT 0x100u /* TEST ONLY: drop the compute stream's wait on E_c^comm
+                                          (Eq. 6) so a negative test can observe the race */
+
+typedef struct hcms_plan hcms_plan_t;
+
+/* ---- introspection (host only, no GPU needed) ---------------------------------------- */
+int hcms_version(void);
+const char* hcms_status_string(int status); /* static string, never NULL */
+const char* hcms_last_error(void);          /* thread-local text of the last failure ("" if none) */
+
+/*
+ * Chunk table, Eq. 3 (L83-84) applied to the per-rank head count (Table 8,
+ * "more-first-less-later" L221).  Host only.  o[c], h[c] for c < C; either array may be NULL.
+ * Errors: INVALID_ARG (heads_per_rank <= 0, C <= 0), UNSUPPORTED_SHAPE (C > heads_per_rank).
+ */
+int hcms_chunk_table_host(int heads_per_rank, int C, int* o, int* h);
+
+/*
+ * Time model of section 3.7 / Appendix A (host only, doubles in any one time unit).
+ *   hcms_model_t_hcms : Eq. 10  T_0 + T_comm/C + T_attn + C*beta
+ *   hcms_model_c_star : Theorem 1  sqrt(T_comm/beta)
+ *   hcms_model_speedup: Eq. 11  1/(1 - rho*(C-1)/C + C*beta/T_total)
+ *   hcms_model_s_max  : Theorem 2  1/(1-rho)
+ * Arguments out of domain (C<=0, beta<=0 for c_star, rho>=1) yield NaN.
+ */
+double hcms_model_t_hcms(int C, double t0, double t_comm, double t_attn, double beta);
+double hcms_model_c_star(double t_comm, double beta);
+double hcms_model_speedup(int C, double rho, double beta, double t_total);
+double hcms_model_s_max(double rho);
+
+/* ---- plan ------------------------------------------------------------------------------ */
+/*
+ * Create a plan for global tensors [S,H,D], P logical ranks, C head chunks (Alg. 1's
+ * `num_chunks`).  Validates the shape, builds the chunk table, creates the communication and
+ * compute streams (device-level stream caching, L221) and 2+2C timing-disabled events, and
+ * allocates the chunk workspace (4*S*H*D*es bytes + alignment) on the current device unless
+ * hcms_plan_set_workspace is used.  `*plan` is owned by the library; free it with
+ * hcms_plan_destroy.  May synchronise the host (allocation).
+ * Errors: INVALID_ARG, UNSUPPORTED_SHAPE, UNSUPPORTED_DTYPE, UNSUPPORTED_DEVICE, CUDA.
+ */
+int hcms_plan(hcms_plan_t** plan, int64_t S, int H, int D, int P, int C, int dtype, uint32_t flags);
+int hcms_plan_destroy(hcms_plan_t* plan); /* synchronises the plan's streams; NULL is a no-op */
+
+/* Bytes of device workspace the plan needs (0 for a NULL plan). */
+size_t hcms_plan_workspace_bytes(const hcms_plan_t* plan);
+/*
+ * Use caller memory (device pointer, 256-byte aligned, >= hcms_plan_workspace_bytes) as the
+ * workspace; the plan's own allocation, if any, is released.  The caller keeps ownership.
+ * Errors: INVALID_ARG, MISALIGNED, WORKSPACE_TOO_SMALL.
+ */
+int hcms_plan_set_workspace(hcms_plan_t* plan, void* dev, size_t bytes);
+
+/* Copy the plan's chunk table to o[C], h[C] (either may be NULL). */
+int hcms_chunk_table(const hcms_plan_t* plan, int* o, int* h);
+/*
+ * Layout of chunk c inside the workspace: `bytes` = size of one chunk tensor
+ * (P*S*h_c*D*es); q_off,k_off,v_off,o_off = byte offsets of Q'_c, K'_c, V'_c, O'_c from the
+ * workspace base.  Any output pointer may be NULL.  Errors: INVALID_ARG, PLAN_MISMATCH.
+ */
+int hcms_chunk_layout(const hcms_plan_t* plan, int c, size_t* bytes, size_t* q_off, size_t* k_off,
+                      size_t* v_off, size_t* o_off);
+/* Device address of the workspace (NULL if none); for tests (NaN poisoning, inspection). */
+void* hcms_plan_workspace(const hcms_plan_t* plan);
+
+/* ---- the hot path ----------------------------------------------------------------------- */
+/*
+ * Algorithm 1 lines 4-26 for one layer: for every chunk c, scatter Q,K,V (input all-to-all,
+ * line 8), attention O'_c = softmax(Q'_c K'_c^T * scale) V'_c per head, non-causal (line 15,
+ * Eq. 2), gather O'_c into `out` (output all-to-all + Concat, lines 21, 26).
+ *
+ * q,k,v,out: device pointers, bf16, contiguous [S,H,D] = the P ranks' shards [S/P,H,D] in rank
+ * order; 16-byte aligned; `out` must not overlap q,k,v.  S,H,D,P,C must equal the plan's
+ * (PLAN_MISMATCH otherwise).  scale: finite, >= 0 (the paper's workloads use 1/sqrt(D)).
+ *
+ * Asynchronous: work is ordered after everything already enqueued on `stream` (E_main, Alg. 1
+ * line 5) and `stream` is made to wait for the result (line 25); `out` is valid once the caller
+ * synchronises `stream`.  Unless HCMS_FLAG_SERIAL is set, scatters/gathers run on the plan's
+ * communication stream and attention on its compute stream, with Attn_c waiting on E_c^comm and
+ * the gather of chunk c on E_c^comp (Eq. 6-7).  Numerics: bf16 operands, fp32 scores,
+ * online softmax and accumulation in fp32, bf16 output (round to nearest even).  The result for
+ * a given (q,k,v,scale) is bitwise independent of P and C (Table 14).
+ * Errors: INVALID_ARG, PLAN_MISMATCH, MISALIGNED, ALIAS, UNSUPPORTED_DTYPE, CUDA.
+ */
+int hcms_attention_forward(hcms_plan_t* plan, const void* q, const void* k, const void* v, void* out,
+                           int64_t S, int H, int D, int P, int C, float scale, void* stream);
+
+/*
+ * Same computation with HOST buffers (q,k,v,out: host pointers, bf16 [S,H,D]; pinned memory
+ * makes the copies asynchronous): copies the inputs to plan-owned device staging, runs
+ * hcms_attention_forward, copies `out` back and SYNCHRONISES `stream` before returning.
+ * First use allocates 4*S*H*D*2 bytes of device staging inside the plan.
+ */
+int hcms_attention_forward_host(hcms_plan_t* plan, const void* q, const void* k, const void* v, void* out,
+                                int64_t S, int H, int D, int P, int C, float scale, void* stream);
+
+/* ---- single steps (tests time and compare each kernel on its own) ----------------------- */
+/*
+ * Input all-to-all of chunk c for up to three tensors in one launch (Alg. 1 line 8
+ * "AllToAll(Q_c,K_c,V_c)"): dst_i[p][s][j][d] = src_i[s][p*Hl+o_c+j][d] for i < n_tensors
+ * (1..3).  src_i: device [S,H,D]; dst_i: device [P][S][h_c][D]; any 2- or 4-byte element
+ * type as given to hcms_plan; all 16-byte aligned; bits are copied untouched.
+ */
+int hcms_a2a_scatter(hcms_plan_t* plan, int n_tensors, const void* const* src, void* const* dst, int c,
+                     void* stream);
+/* Output all-to-all of chunk c: dst[s][p*Hl+o_c+j][d] = src[p][s][j][d]; writes only chunk c's heads. */
+int hcms_a2a_gather(hcms_plan_t* plan, const void* src, void* dst, int c, void* stream);
+/*
+ * Attention of chunk c on head-sharded buffers qc,kc,vc -> oc, all device [P][S][h_c][D] bf16,
+ * 16-byte aligned: for every p, j:  oc[p][:,j,:] = softmax(qc[p][:,j,:] kc[p][:,j,:]^T * scale) vc[p][:,j,:].
+ */
+int hcms_attention_chunk(hcms_plan_t* plan, const void* qc, const void* kc, const void* vc, void* oc, int c,
+                         float scale, void* stream);
+
+/* Number of kernels + async copies the last hcms_attention_forward on this plan enqueued. */
+int hcms_plan_last_launch_count(const hcms_plan_t* plan);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HCMS_H_ */

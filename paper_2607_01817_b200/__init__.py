@@ -1,0 +1,272 @@
+"""Python binding of libhcms (include/hcms.h): argument marshalling only.
+
+Every step of the HCMS hot path (Alg. 1 lines 4-26: head-chunked all-to-all layout
+kernels, bf16 attention, dual-stream scheduler) runs inside ``libhcms.so`` (CUDA, sm_100a).
+The functions here carry the same names as the C entry points and only turn torch tensors /
+numpy arrays / ints into pointers.  There is no CPU fallback: importing this package without a
+built ``libhcms.so`` raises, and a compute call without a B200 returns the library's error.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import POINTER, c_char_p, c_double, c_float, c_int, c_int64, c_size_t, c_uint32, c_void_p
+
+_PKG_DIR = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG_DIR, "libhcms.so")
+
+# status codes / dtypes / flags (mirrors include/hcms.h)
+HCMS_OK = 0
+HCMS_ERR_INVALID_ARG = -1
+HCMS_ERR_UNSUPPORTED_SHAPE = -2
+HCMS_ERR_UNSUPPORTED_DTYPE = -3
+HCMS_ERR_UNSUPPORTED_DEVICE = -4
+HCMS_ERR_MISALIGNED = -5
+HCMS_ERR_ALIAS = -6
+HCMS_ERR_PLAN_MISMATCH = -7
+HCMS_ERR_WORKSPACE_TOO_SMALL = -8
+HCMS_ERR_CUDA = -9
+
+HCMS_DTYPE_BF16 = 0
+HCMS_DTYPE_F32 = 1
+HCMS_DTYPE_F16 = 2
+
+HCMS_FLAG_SERIAL = 0x1
+HCMS_FLAG_LAYOUT_TMA = 0x2
+HCMS_FLAG_SPLIT_COMM = 0x4
+HCMS_FLAG_HOST_ROUTE_Q = 0x10
+HCMS_FLAG_HOST_ROUTE_K = 0x20
+HCMS_FLAG_HOST_ROUTE_V = 0x40
+HCMS_FLAG_HOST_ROUTE_O = 0x80
+HCMS_FLAG_DEBUG_NO_COMM_WAIT = 0x100
+
+# every symbol include/hcms.h declares: name -> (restype, argtypes)
+_SIGNATURES = {
+    "hcms_version": (c_int, []),
+    "hcms_status_string": (c_char_p, [c_int]),
+    "hcms_last_error": (c_char_p, []),
+    "hcms_chunk_table_host": (c_int, [c_int, c_int, POINTER(c_int), POINTER(c_int)]),
+    "hcms_model_t_hcms": (c_double, [c_int, c_double, c_double, c_double, c_double]),
+    "hcms_model_c_star": (c_double, [c_double, c_double]),
+    "hcms_model_speedup": (c_double, [c_int, c_double, c_double, c_double]),
+    "hcms_model_s_max": (c_double, [c_double]),
+    "hcms_plan": (c_int, [POINTER(c_void_p), c_int64, c_int, c_int, c_int, c_int, c_int, c_uint32]),
+    "hcms_plan_destroy": (c_int, [c_void_p]),
+    "hcms_plan_workspace_bytes": (c_size_t, [c_void_p]),
+    "hcms_plan_set_workspace": (c_int, [c_void_p, c_void_p, c_size_t]),
+    "hcms_chunk_table": (c_int, [c_void_p, POINTER(c_int), POINTER(c_int)]),
+    "hcms_chunk_layout": (c_int, [c_void_p, c_int] + [POINTER(c_size_t)] * 5),
+    "hcms_plan_workspace": (c_void_p, [c_void_p]),
+    "hcms_attention_forward": (c_int, [c_void_p] * 5 + [c_int64, c_int, c_int, c_int, c_int, c_float, c_void_p]),
+    "hcms_attention_forward_host": (c_int, [c_void_p] * 5 + [c_int64, c_int, c_int, c_int, c_int, c_float, c_void_p]),
+    "hcms_a2a_scatter": (c_int, [c_void_p, c_int, POINTER(c_void_p), POINTER(c_void_p), c_int, c_void_p]),
+    "hcms_a2a_gather": (c_int, [c_void_p, c_void_p, c_void_p, c_int, c_void_p]),
+    "hcms_attention_chunk": (c_int, [c_void_p] * 5 + [c_int, c_float, c_void_p]),
+    "hcms_plan_last_launch_count": (c_int, [c_void_p]),
+}
+
+
+class HcmsError(RuntimeError):
+    """A libhcms call returned a negative status."""
+
+    def __init__(self, status: int, name: str, text: str):
+        super().__init__(f"{name}: {text} [{status}]")
+        self.status = status
+
+
+def _load() -> ctypes.CDLL:
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(
+            f"{LIB_PATH} is missing: build it with `python -m paper_2607_01817_b200.build` "
+            "(the HCMS hot path exists only as CUDA code; there is no CPU fallback)")
+    lib = ctypes.CDLL(LIB_PATH)
+    for name, (res, args) in _SIGNATURES.items():
+        fn = getattr(lib, name)      # AttributeError if the library lacks a declared symbol
+        fn.restype = res
+        fn.argtypes = args
+    return lib
+
+
+class _LazyLib:
+    """Loads libhcms.so on first use, so that ``python -m paper_2607_01817_b200.build`` can import
+    the package before the library exists.  Any call without the library raises ImportError."""
+
+    _cdll = None
+
+    def __getattr__(self, name):
+        if _LazyLib._cdll is None:
+            _LazyLib._cdll = _load()
+        return getattr(_LazyLib._cdll, name)
+
+
+lib = _LazyLib()
+
+
+def _check(status: int, name: str) -> None:
+    if status != HCMS_OK:
+        raise HcmsError(status, lib.hcms_status_string(status).decode(), f"{name}: {lib.hcms_last_error().decode()}")
+
+
+def _ptr(x) -> int:
+    """Address of a torch tensor / numpy array / raw int pointer (no copies, no conversions)."""
+    if x is None:
+        return 0
+    if isinstance(x, int):
+        return x
+    if hasattr(x, "data_ptr"):          # torch.Tensor
+        if not x.is_contiguous():
+            raise ValueError("libhcms needs contiguous tensors")
+        return x.data_ptr()
+    if hasattr(x, "ctypes"):            # numpy.ndarray
+        if not x.flags["C_CONTIGUOUS"]:
+            raise ValueError("libhcms needs C-contiguous arrays")
+        return x.ctypes.data
+    raise TypeError(f"cannot take the address of {type(x)}")
+
+
+def _stream(stream) -> int:
+    """cudaStream_t of a torch.cuda.Stream / int / None (None = torch's current stream)."""
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    if isinstance(stream, int):
+        return stream
+    return stream.cuda_stream
+
+
+# ---- host-only entry points ------------------------------------------------------------------
+
+def hcms_version() -> int:
+    return lib.hcms_version()
+
+
+def hcms_status_string(status: int) -> str:
+    return lib.hcms_status_string(status).decode()
+
+
+def hcms_last_error() -> str:
+    return lib.hcms_last_error().decode()
+
+
+def hcms_chunk_table_host(heads_per_rank: int, C: int):
+    """Eq. 3 on the per-rank head count -> ([o_c], [h_c])."""
+    n = max(int(C), 1)
+    o, h = (c_int * n)(), (c_int * n)()
+    _check(lib.hcms_chunk_table_host(heads_per_rank, C, o, h), "hcms_chunk_table_host")
+    return list(o)[:C], list(h)[:C]
+
+
+def hcms_model_t_hcms(C, t0, t_comm, t_attn, beta) -> float:
+    return lib.hcms_model_t_hcms(C, t0, t_comm, t_attn, beta)
+
+
+def hcms_model_c_star(t_comm, beta) -> float:
+    return lib.hcms_model_c_star(t_comm, beta)
+
+
+def hcms_model_speedup(C, rho, beta, t_total) -> float:
+    return lib.hcms_model_speedup(C, rho, beta, t_total)
+
+
+def hcms_model_s_max(rho) -> float:
+    return lib.hcms_model_s_max(rho)
+
+
+# ---- plan ------------------------------------------------------------------------------------
+
+class Plan:
+    """Owner of one ``hcms_plan_t*`` (destroyed on ``close()`` / garbage collection)."""
+
+    def __init__(self, handle: int, S, H, D, P, C, dtype, flags):
+        self.handle = handle
+        self.S, self.H, self.D, self.P, self.C = int(S), int(H), int(D), int(P), int(C)
+        self.dtype, self.flags = dtype, flags
+
+    def close(self) -> None:
+        if self.handle:
+            lib.hcms_plan_destroy(self.handle)
+            self.handle = 0
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def hcms_plan(S, H, D, P, C, dtype=HCMS_DTYPE_BF16, flags=0) -> Plan:
+    h = c_void_p()
+    _check(lib.hcms_plan(ctypes.byref(h), S, H, D, P, C, dtype, flags), "hcms_plan")
+    return Plan(h.value, S, H, D, P, C, dtype, flags)
+
+
+def hcms_plan_destroy(plan: Plan) -> None:
+    plan.close()
+
+
+def hcms_plan_workspace_bytes(plan: Plan) -> int:
+    return lib.hcms_plan_workspace_bytes(plan.handle)
+
+
+def hcms_plan_workspace(plan: Plan) -> int:
+    return lib.hcms_plan_workspace(plan.handle) or 0
+
+
+def hcms_plan_set_workspace(plan: Plan, dev, nbytes: int) -> None:
+    _check(lib.hcms_plan_set_workspace(plan.handle, _ptr(dev), nbytes), "hcms_plan_set_workspace")
+
+
+def hcms_chunk_table(plan: Plan):
+    o, h = (c_int * plan.C)(), (c_int * plan.C)()
+    _check(lib.hcms_chunk_table(plan.handle, o, h), "hcms_chunk_table")
+    return list(o), list(h)
+
+
+def hcms_chunk_layout(plan: Plan, c: int):
+    """-> dict(bytes, q_off, k_off, v_off, o_off) of chunk c inside the workspace."""
+    vals = [c_size_t() for _ in range(5)]
+    _check(lib.hcms_chunk_layout(plan.handle, c, *[ctypes.byref(v) for v in vals]), "hcms_chunk_layout")
+    return dict(zip(("bytes", "q_off", "k_off", "v_off", "o_off"), (v.value for v in vals)))
+
+
+def hcms_plan_last_launch_count(plan: Plan) -> int:
+    return lib.hcms_plan_last_launch_count(plan.handle)
+
+
+# ---- the hot path ------------------------------------------------------------------------------
+
+def hcms_attention_forward(plan: Plan, q, k, v, out, scale: float, stream=None) -> None:
+    """Alg. 1 lines 4-26 on device tensors [S,H,D] bf16; asynchronous on ``stream``."""
+    _check(lib.hcms_attention_forward(plan.handle, _ptr(q), _ptr(k), _ptr(v), _ptr(out), plan.S, plan.H, plan.D,
+                                      plan.P, plan.C, scale, _stream(stream)), "hcms_attention_forward")
+
+
+def hcms_attention_forward_host(plan: Plan, q, k, v, out, scale: float, stream=None) -> None:
+    """Same with HOST buffers (numpy uint16 / pinned torch tensors); synchronises ``stream``."""
+    _check(lib.hcms_attention_forward_host(plan.handle, _ptr(q), _ptr(k), _ptr(v), _ptr(out), plan.S, plan.H,
+                                           plan.D, plan.P, plan.C, scale, _stream(stream)),
+           "hcms_attention_forward_host")
+
+
+def hcms_a2a_scatter(plan: Plan, srcs, dsts, c: int, stream=None) -> None:
+    n = len(srcs)
+    if n != len(dsts):
+        raise ValueError("srcs and dsts differ in length")
+    s = (c_void_p * n)(*[_ptr(x) for x in srcs])
+    d = (c_void_p * n)(*[_ptr(x) for x in dsts])
+    _check(lib.hcms_a2a_scatter(plan.handle, n, s, d, c, _stream(stream)), "hcms_a2a_scatter")
+
+
+def hcms_a2a_gather(plan: Plan, src, dst, c: int, stream=None) -> None:
+    _check(lib.hcms_a2a_gather(plan.handle, _ptr(src), _ptr(dst), c, _stream(stream)), "hcms_a2a_gather")
+
+
+def hcms_attention_chunk(plan: Plan, qc, kc, vc, oc, c: int, scale: float, stream=None) -> None:
+    _check(lib.hcms_attention_chunk(plan.handle, _ptr(qc), _ptr(kc), _ptr(vc), _ptr(oc), c, scale, _stream(stream)),
+           "hcms_attention_chunk")

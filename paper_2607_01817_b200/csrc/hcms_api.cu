@@ -1,0 +1,487 @@
+// libhcms entry points: plan, chunk table, dual-stream chunk scheduler (section 3.4-3.6,
+// Algorithm 1), single-step hooks, host-buffer convenience call.  See include/hcms.h.
+#include <cmath>
+#include <cstdarg>
+#include <cstring>
+#include <new>
+
+#include "hcms_internal.h"
+
+namespace hcms {
+
+// ------------------------------------------------------------------------------------------
+// errors
+// ------------------------------------------------------------------------------------------
+static thread_local char g_last_error[512] = "";
+
+int fail(int status, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_last_error, sizeof(g_last_error), fmt, ap);
+  va_end(ap);
+  return status;
+}
+int fail_cuda(cudaError_t e, const char* what) {
+  return fail(HCMS_ERR_CUDA, "CUDA error %d (%s: %s) in %s", static_cast<int>(e), cudaGetErrorName(e),
+              cudaGetErrorString(e), what);
+}
+
+// ------------------------------------------------------------------------------------------
+// host-only math
+// ------------------------------------------------------------------------------------------
+static int chunk_table(int Hl, int C, int* o, int* h) {
+  if (Hl <= 0 || C <= 0) return fail(HCMS_ERR_INVALID_ARG, "heads_per_rank=%d and C=%d must be positive", Hl, C);
+  if (C > Hl) return fail(HCMS_ERR_UNSUPPORTED_SHAPE, "C=%d exceeds heads per rank %d (every chunk needs a head)", C, Hl);
+  int off = 0;
+  for (int c = 0; c < C; ++c) {
+    const int hc = Hl / C + (c < Hl % C ? 1 : 0);  // Eq. 3, larger chunks first (L221)
+    if (o) o[c] = off;
+    if (h) h[c] = hc;
+    off += hc;
+  }
+  return HCMS_OK;
+}
+
+static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+}  // namespace hcms
+
+using namespace hcms;
+
+// ------------------------------------------------------------------------------------------
+// plan
+// ------------------------------------------------------------------------------------------
+struct hcms_plan {
+  Shape sh{};
+  int dtype = 0;
+  uint32_t flags = 0;
+  int device = 0;
+  int num_sms = 0;
+  std::vector<Chunk> chunks;
+  size_t ws_bytes = 0;
+  void* ws = nullptr;
+  bool ws_owned = false;
+  cudaStream_t s_comm = nullptr, s_comm_out = nullptr, s_comp = nullptr;
+  cudaEvent_t e_main = nullptr, e_fin_comm = nullptr, e_fin_comp = nullptr, e_fin_in = nullptr;
+  std::vector<cudaEvent_t> e_comm, e_comp;
+  // host route (config 5)
+  void* pinned[4] = {nullptr, nullptr, nullptr, nullptr};
+  // host-buffer entry point staging
+  void* staging[4] = {nullptr, nullptr, nullptr, nullptr};
+  int last_launches = 0;
+};
+
+static void plan_free(hcms_plan_t* p) {
+  if (!p) return;
+  if (p->s_comm) cudaStreamSynchronize(p->s_comm);
+  if (p->s_comm_out) cudaStreamSynchronize(p->s_comm_out);
+  if (p->s_comp) cudaStreamSynchronize(p->s_comp);
+  for (auto e : p->e_comm) cudaEventDestroy(e);
+  for (auto e : p->e_comp) cudaEventDestroy(e);
+  if (p->e_main) cudaEventDestroy(p->e_main);
+  if (p->e_fin_comm) cudaEventDestroy(p->e_fin_comm);
+  if (p->e_fin_comp) cudaEventDestroy(p->e_fin_comp);
+  if (p->e_fin_in) cudaEventDestroy(p->e_fin_in);
+  if (p->s_comm) cudaStreamDestroy(p->s_comm);
+  if (p->s_comm_out) cudaStreamDestroy(p->s_comm_out);
+  if (p->s_comp) cudaStreamDestroy(p->s_comp);
+  if (p->ws_owned && p->ws) cudaFree(p->ws);
+  for (auto& h : p->pinned)
+    if (h) cudaFreeHost(h);
+  for (auto& d : p->staging)
+    if (d) cudaFree(d);
+  delete p;
+}
+
+static int elem_size(int dtype) {
+  switch (dtype) {
+    case HCMS_DTYPE_BF16:
+    case HCMS_DTYPE_F16:
+      return 2;
+    case HCMS_DTYPE_F32:
+      return 4;
+    default:
+      return 0;
+  }
+}
+
+extern "C" {
+
+int hcms_version(void) { return HCMS_VERSION; }
+
+const char* hcms_status_string(int status) {
+  switch (status) {
+    case HCMS_OK: return "HCMS_OK";
+    case HCMS_ERR_INVALID_ARG: return "HCMS_ERR_INVALID_ARG";
+    case HCMS_ERR_UNSUPPORTED_SHAPE: return "HCMS_ERR_UNSUPPORTED_SHAPE";
+    case HCMS_ERR_UNSUPPORTED_DTYPE: return "HCMS_ERR_UNSUPPORTED_DTYPE";
+    case HCMS_ERR_UNSUPPORTED_DEVICE: return "HCMS_ERR_UNSUPPORTED_DEVICE";
+    case HCMS_ERR_MISALIGNED: return "HCMS_ERR_MISALIGNED";
+    case HCMS_ERR_ALIAS: return "HCMS_ERR_ALIAS";
+    case HCMS_ERR_PLAN_MISMATCH: return "HCMS_ERR_PLAN_MISMATCH";
+    case HCMS_ERR_WORKSPACE_TOO_SMALL: return "HCMS_ERR_WORKSPACE_TOO_SMALL";
+    case HCMS_ERR_CUDA: return "HCMS_ERR_CUDA";
+    default: return "HCMS_ERR_UNKNOWN";
+  }
+}
+
+const char* hcms_last_error(void) { return g_last_error; }
+
+int hcms_chunk_table_host(int heads_per_rank, int C, int* o, int* h) { return chunk_table(heads_per_rank, C, o, h); }
+
+double hcms_model_t_hcms(int C, double t0, double t_comm, double t_attn, double beta) {
+  if (C <= 0) return NAN;
+  return t0 + t_comm / C + t_attn + C * beta;  // Eq. 10 (L417)
+}
+double hcms_model_c_star(double t_comm, double beta) {
+  if (!(beta > 0) || !(t_comm >= 0)) return NAN;
+  return std::sqrt(t_comm / beta);  // Theorem 1 (L156, L421)
+}
+double hcms_model_speedup(int C, double rho, double beta, double t_total) {
+  if (C <= 0 || !(t_total > 0)) return NAN;
+  return 1.0 / (1.0 - rho * (C - 1) / C + C * beta / t_total);  // Eq. 11 (L427)
+}
+double hcms_model_s_max(double rho) {
+  if (!(rho < 1)) return NAN;
+  return 1.0 / (1.0 - rho);  // Theorem 2 (L158, L429)
+}
+
+int hcms_plan(hcms_plan_t** out, int64_t S, int H, int D, int P, int C, int dtype, uint32_t flags) {
+  if (!out) return fail(HCMS_ERR_INVALID_ARG, "plan output pointer is NULL");
+  *out = nullptr;
+  if (S <= 0 || H <= 0 || D <= 0 || P <= 0 || C <= 0)
+    return fail(HCMS_ERR_INVALID_ARG, "S=%lld H=%d D=%d P=%d C=%d must all be positive", static_cast<long long>(S), H, D,
+                P, C);
+  const int es = elem_size(dtype);
+  if (es == 0) return fail(HCMS_ERR_UNSUPPORTED_DTYPE, "unknown dtype %d", dtype);
+  if (S % P) return fail(HCMS_ERR_UNSUPPORTED_SHAPE, "S=%lld is not divisible by P=%d", static_cast<long long>(S), P);
+  if (H % P) return fail(HCMS_ERR_UNSUPPORTED_SHAPE, "H=%d is not divisible by P=%d", H, P);
+  if (D != 64 && D != 128) return fail(HCMS_ERR_UNSUPPORTED_SHAPE, "D=%d: only head dimensions 64 and 128 are built", D);
+  if (S > (1ll << 30)) return fail(HCMS_ERR_UNSUPPORTED_SHAPE, "S=%lld too large", static_cast<long long>(S));
+  const int Hl = H / P;
+  if (C > Hl) return fail(HCMS_ERR_UNSUPPORTED_SHAPE, "C=%d exceeds heads per rank H/P=%d", C, Hl);
+
+  int dev = 0, n = 0;
+  cudaError_t ce = cudaGetDeviceCount(&n);
+  if (ce != cudaSuccess || n == 0) {
+    cudaGetLastError();
+    return fail(HCMS_ERR_UNSUPPORTED_DEVICE, "no CUDA device (%s); libhcms has no CPU fallback",
+                ce == cudaSuccess ? "count is 0" : cudaGetErrorString(ce));
+  }
+  HCMS_CUDA(cudaGetDevice(&dev));
+  cudaDeviceProp prop;
+  HCMS_CUDA(cudaGetDeviceProperties(&prop, dev));
+  if (prop.major != 10)
+    return fail(HCMS_ERR_UNSUPPORTED_DEVICE, "device %d is sm_%d%d; libhcms is built for sm_100a only", dev, prop.major,
+                prop.minor);
+
+  hcms_plan_t* p = new (std::nothrow) hcms_plan_t();
+  if (!p) return fail(HCMS_ERR_INVALID_ARG, "out of host memory");
+  p->sh = Shape{S, H, D, P, C, es, Hl};
+  p->dtype = dtype;
+  p->flags = flags;
+  p->device = dev;
+  p->num_sms = prop.multiProcessorCount;
+  p->chunks.resize(C);
+  std::vector<int> o(C), h(C);
+  chunk_table(Hl, C, o.data(), h.data());
+  size_t off = 0;
+  for (int c = 0; c < C; ++c) {
+    Chunk& ck = p->chunks[c];
+    ck.o = o[c];
+    ck.h = h[c];
+    ck.bytes = static_cast<size_t>(P) * S * h[c] * D * es;
+    for (int t = 0; t < 4; ++t) {
+      ck.off[t] = off;
+      off += align_up(ck.bytes, 1024);
+    }
+  }
+  p->ws_bytes = off;
+
+  auto bail = [&](int st) {
+    plan_free(p);
+    return st;
+  };
+#define PLAN_CUDA(expr)                                              \
+  do {                                                               \
+    cudaError_t e__ = (expr);                                        \
+    if (e__ != cudaSuccess) return bail(fail_cuda(e__, #expr));      \
+  } while (0)
+  int prio_lo = 0, prio_hi = 0;
+  PLAN_CUDA(cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi));
+  // the communication stream outranks the compute stream so that copy CTAs are placed as soon as
+  // an SM has room, instead of queueing behind the attention grid
+  PLAN_CUDA(cudaStreamCreateWithPriority(&p->s_comm, cudaStreamNonBlocking, prio_hi));
+  PLAN_CUDA(cudaStreamCreateWithPriority(&p->s_comm_out, cudaStreamNonBlocking, prio_hi));
+  PLAN_CUDA(cudaStreamCreateWithPriority(&p->s_comp, cudaStreamNonBlocking, prio_lo));
+  PLAN_CUDA(cudaEventCreateWithFlags(&p->e_main, cudaEventDisableTiming));
+  PLAN_CUDA(cudaEventCreateWithFlags(&p->e_fin_comm, cudaEventDisableTiming));
+  PLAN_CUDA(cudaEventCreateWithFlags(&p->e_fin_comp, cudaEventDisableTiming));
+  PLAN_CUDA(cudaEventCreateWithFlags(&p->e_fin_in, cudaEventDisableTiming));
+  p->e_comm.assign(C, nullptr);
+  p->e_comp.assign(C, nullptr);
+  for (int c = 0; c < C; ++c) {
+    PLAN_CUDA(cudaEventCreateWithFlags(&p->e_comm[c], cudaEventDisableTiming));
+    PLAN_CUDA(cudaEventCreateWithFlags(&p->e_comp[c], cudaEventDisableTiming));
+  }
+  PLAN_CUDA(cudaMalloc(&p->ws, p->ws_bytes));
+  p->ws_owned = true;
+  if (dtype == HCMS_DTYPE_BF16) PLAN_CUDA(attention_init());
+  if (flags & (HCMS_FLAG_HOST_ROUTE_Q | HCMS_FLAG_HOST_ROUTE_K | HCMS_FLAG_HOST_ROUTE_V | HCMS_FLAG_HOST_ROUTE_O)) {
+    size_t max_chunk = 0;
+    for (auto& ck : p->chunks) max_chunk = ck.bytes > max_chunk ? ck.bytes : max_chunk;
+    for (int t = 0; t < 4; ++t)
+      if (flags & (HCMS_FLAG_HOST_ROUTE_Q << t)) PLAN_CUDA(cudaMallocHost(&p->pinned[t], max_chunk));
+  }
+#undef PLAN_CUDA
+  *out = p;
+  return HCMS_OK;
+}
+
+int hcms_plan_destroy(hcms_plan_t* plan) {
+  plan_free(plan);
+  return HCMS_OK;
+}
+
+size_t hcms_plan_workspace_bytes(const hcms_plan_t* plan) { return plan ? plan->ws_bytes : 0; }
+void* hcms_plan_workspace(const hcms_plan_t* plan) { return plan ? plan->ws : nullptr; }
+
+int hcms_plan_set_workspace(hcms_plan_t* plan, void* dev, size_t bytes) {
+  if (!plan || !dev) return fail(HCMS_ERR_INVALID_ARG, "plan or workspace pointer is NULL");
+  if (reinterpret_cast<uintptr_t>(dev) % 256) return fail(HCMS_ERR_MISALIGNED, "workspace must be 256-byte aligned");
+  if (bytes < plan->ws_bytes)
+    return fail(HCMS_ERR_WORKSPACE_TOO_SMALL, "workspace has %zu bytes, plan needs %zu", bytes, plan->ws_bytes);
+  if (plan->ws_owned && plan->ws) {
+    cudaStreamSynchronize(plan->s_comm);
+    cudaStreamSynchronize(plan->s_comm_out);
+    cudaStreamSynchronize(plan->s_comp);
+    cudaFree(plan->ws);
+  }
+  plan->ws = dev;
+  plan->ws_owned = false;
+  return HCMS_OK;
+}
+
+int hcms_chunk_table(const hcms_plan_t* plan, int* o, int* h) {
+  if (!plan) return fail(HCMS_ERR_INVALID_ARG, "plan is NULL");
+  for (int c = 0; c < plan->sh.C; ++c) {
+    if (o) o[c] = plan->chunks[c].o;
+    if (h) h[c] = plan->chunks[c].h;
+  }
+  return HCMS_OK;
+}
+
+int hcms_chunk_layout(const hcms_plan_t* plan, int c, size_t* bytes, size_t* q_off, size_t* k_off, size_t* v_off,
+                      size_t* o_off) {
+  if (!plan) return fail(HCMS_ERR_INVALID_ARG, "plan is NULL");
+  if (c < 0 || c >= plan->sh.C) return fail(HCMS_ERR_PLAN_MISMATCH, "chunk %d outside [0,%d)", c, plan->sh.C);
+  const Chunk& ck = plan->chunks[c];
+  if (bytes) *bytes = ck.bytes;
+  if (q_off) *q_off = ck.off[0];
+  if (k_off) *k_off = ck.off[1];
+  if (v_off) *v_off = ck.off[2];
+  if (o_off) *o_off = ck.off[3];
+  return HCMS_OK;
+}
+
+int hcms_plan_last_launch_count(const hcms_plan_t* plan) { return plan ? plan->last_launches : 0; }
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------
+// single steps
+// ------------------------------------------------------------------------------------------
+static bool aligned16(const void* p) { return reinterpret_cast<uintptr_t>(p) % 16 == 0; }
+
+static int do_layout(hcms_plan_t* p, int n, const void* const* src, void* const* dst, int c, bool gather,
+                     cudaStream_t st) {
+  const Chunk& ck = p->chunks[c];
+  LayoutArgs a{};
+  for (int t = 0; t < n; ++t) {
+    a.src[t] = src[t];
+    a.dst[t] = dst[t];
+  }
+  a.n_tensors = n;
+  a.S = p->sh.S;
+  a.H = p->sh.H;
+  a.D = p->sh.D;
+  a.P = p->sh.P;
+  a.Hl = p->sh.Hl;
+  a.es = p->sh.es;
+  a.o_c = ck.o;
+  a.h_c = ck.h;
+  a.gather = gather;
+  cudaError_t e = (p->flags & HCMS_FLAG_LAYOUT_TMA) ? launch_layout_tma(a, st, p->num_sms) : launch_layout_vec(a, st);
+  if (e != cudaSuccess) return fail_cuda(e, gather ? "a2a gather launch" : "a2a scatter launch");
+  p->last_launches += 1;
+  return HCMS_OK;
+}
+
+static int do_attention(hcms_plan_t* p, const void* qc, const void* kc, const void* vc, void* oc, int c, float scale,
+                        cudaStream_t st) {
+  const Chunk& ck = p->chunks[c];
+  AttnArgs a{qc, kc, vc, oc, p->sh.S, p->sh.D, p->sh.P, ck.h, scale};
+  cudaError_t e = launch_attention(a, st);
+  if (e != cudaSuccess) return fail_cuda(e, "attention launch");
+  p->last_launches += 1;
+  return HCMS_OK;
+}
+
+static int check_scale(float scale) {
+  if (!std::isfinite(scale) || scale < 0.f) return fail(HCMS_ERR_INVALID_ARG, "scale=%g must be finite and >= 0", scale);
+  return HCMS_OK;
+}
+
+extern "C" {
+
+int hcms_a2a_scatter(hcms_plan_t* plan, int n_tensors, const void* const* src, void* const* dst, int c, void* stream) {
+  if (!plan || !src || !dst) return fail(HCMS_ERR_INVALID_ARG, "NULL argument");
+  if (n_tensors < 1 || n_tensors > 3) return fail(HCMS_ERR_INVALID_ARG, "n_tensors=%d must be 1..3", n_tensors);
+  if (c < 0 || c >= plan->sh.C) return fail(HCMS_ERR_PLAN_MISMATCH, "chunk %d outside [0,%d)", c, plan->sh.C);
+  for (int t = 0; t < n_tensors; ++t) {
+    if (!src[t] || !dst[t]) return fail(HCMS_ERR_INVALID_ARG, "tensor %d pointer is NULL", t);
+    if (!aligned16(src[t]) || !aligned16(dst[t])) return fail(HCMS_ERR_MISALIGNED, "tensor %d is not 16-byte aligned", t);
+  }
+  plan->last_launches = 0;
+  return do_layout(plan, n_tensors, src, dst, c, false, static_cast<cudaStream_t>(stream));
+}
+
+int hcms_a2a_gather(hcms_plan_t* plan, const void* src, void* dst, int c, void* stream) {
+  if (!plan || !src || !dst) return fail(HCMS_ERR_INVALID_ARG, "NULL argument");
+  if (c < 0 || c >= plan->sh.C) return fail(HCMS_ERR_PLAN_MISMATCH, "chunk %d outside [0,%d)", c, plan->sh.C);
+  if (!aligned16(src) || !aligned16(dst)) return fail(HCMS_ERR_MISALIGNED, "pointer is not 16-byte aligned");
+  const void* s[1] = {src};
+  void* d[1] = {dst};
+  plan->last_launches = 0;
+  return do_layout(plan, 1, s, d, c, true, static_cast<cudaStream_t>(stream));
+}
+
+int hcms_attention_chunk(hcms_plan_t* plan, const void* qc, const void* kc, const void* vc, void* oc, int c, float scale,
+                         void* stream) {
+  if (!plan || !qc || !kc || !vc || !oc) return fail(HCMS_ERR_INVALID_ARG, "NULL argument");
+  if (plan->dtype != HCMS_DTYPE_BF16) return fail(HCMS_ERR_UNSUPPORTED_DTYPE, "attention needs a bf16 plan");
+  if (c < 0 || c >= plan->sh.C) return fail(HCMS_ERR_PLAN_MISMATCH, "chunk %d outside [0,%d)", c, plan->sh.C);
+  if (!aligned16(qc) || !aligned16(kc) || !aligned16(vc) || !aligned16(oc))
+    return fail(HCMS_ERR_MISALIGNED, "pointer is not 16-byte aligned");
+  int st = check_scale(scale);
+  if (st) return st;
+  plan->last_launches = 0;
+  return do_attention(plan, qc, kc, vc, oc, c, scale, static_cast<cudaStream_t>(stream));
+}
+
+// ------------------------------------------------------------------------------------------
+// the dual-stream chunk scheduler (Algorithm 1 lines 4-25)
+// ------------------------------------------------------------------------------------------
+int hcms_attention_forward(hcms_plan_t* plan, const void* q, const void* k, const void* v, void* out, int64_t S, int H,
+                           int D, int P, int C, float scale, void* stream) {
+  if (!plan || !q || !k || !v || !out) return fail(HCMS_ERR_INVALID_ARG, "NULL argument");
+  const Shape& sh = plan->sh;
+  if (S != sh.S || H != sh.H || D != sh.D || P != sh.P || C != sh.C)
+    return fail(HCMS_ERR_PLAN_MISMATCH, "call (S=%lld,H=%d,D=%d,P=%d,C=%d) != plan (S=%lld,H=%d,D=%d,P=%d,C=%d)",
+                static_cast<long long>(S), H, D, P, C, static_cast<long long>(sh.S), sh.H, sh.D, sh.P, sh.C);
+  if (plan->dtype != HCMS_DTYPE_BF16) return fail(HCMS_ERR_UNSUPPORTED_DTYPE, "attention needs a bf16 plan");
+  int st = check_scale(scale);
+  if (st) return st;
+  if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(out))
+    return fail(HCMS_ERR_MISALIGNED, "q, k, v and out must be 16-byte aligned");
+  const size_t bytes = static_cast<size_t>(S) * H * D * sh.es;
+  const char* ob = static_cast<const char*>(out);
+  for (const void* in : {q, k, v}) {
+    const char* ib = static_cast<const char*>(in);
+    if (ob < ib + bytes && ib < ob + bytes) return fail(HCMS_ERR_ALIAS, "out overlaps an input tensor");
+  }
+  if (!plan->ws) return fail(HCMS_ERR_WORKSPACE_TOO_SMALL, "plan has no workspace");
+
+  cudaStream_t caller = static_cast<cudaStream_t>(stream);
+  const bool serial = plan->flags & HCMS_FLAG_SERIAL;
+  const bool split = (plan->flags & HCMS_FLAG_SPLIT_COMM) && !serial;
+  cudaStream_t s_in = serial ? caller : plan->s_comm;
+  cudaStream_t s_out = serial ? caller : (split ? plan->s_comm_out : plan->s_comm);
+  cudaStream_t s_comp = serial ? caller : plan->s_comp;
+  char* ws = static_cast<char*>(plan->ws);
+  plan->last_launches = 0;
+
+  auto host_route = [&](int t, const Chunk& ck, cudaStream_t s) -> int {
+    if (!(plan->flags & (HCMS_FLAG_HOST_ROUTE_Q << t))) return HCMS_OK;
+    // the emulated wire: device -> pinned host -> device, same bits
+    HCMS_CUDA(cudaMemcpyAsync(plan->pinned[t], ws + ck.off[t], ck.bytes, cudaMemcpyDeviceToHost, s));
+    HCMS_CUDA(cudaMemcpyAsync(ws + ck.off[t], plan->pinned[t], ck.bytes, cudaMemcpyHostToDevice, s));
+    plan->last_launches += 2;
+    return HCMS_OK;
+  };
+
+  if (!serial) {
+    HCMS_CUDA(cudaEventRecord(plan->e_main, caller));            // Alg. 1 line 5
+    HCMS_CUDA(cudaStreamWaitEvent(s_in, plan->e_main, 0));       // line 7
+    HCMS_CUDA(cudaStreamWaitEvent(s_comp, plan->e_main, 0));     // line 13
+    if (split) HCMS_CUDA(cudaStreamWaitEvent(s_out, plan->e_main, 0));
+  }
+  // Phase 1 -- input all-to-all of every chunk on S_comm (lines 8-11)
+  for (int c = 0; c < sh.C; ++c) {
+    const Chunk& ck = plan->chunks[c];
+    const void* src[3] = {q, k, v};
+    void* dst[3] = {ws + ck.off[0], ws + ck.off[1], ws + ck.off[2]};
+    st = do_layout(plan, 3, src, dst, c, false, s_in);
+    if (st) return st;
+    for (int t = 0; t < 3; ++t) {
+      st = host_route(t, ck, s_in);
+      if (st) return st;
+    }
+    if (!serial) HCMS_CUDA(cudaEventRecord(plan->e_comm[c], s_in));  // E_c^comm
+  }
+  // Phase 2 -- attention per chunk on S_comp (lines 14-18); Attn_c <- wait(E_c^comm)  (Eq. 6)
+  for (int c = 0; c < sh.C; ++c) {
+    const Chunk& ck = plan->chunks[c];
+    if (!serial && !(plan->flags & HCMS_FLAG_DEBUG_NO_COMM_WAIT))
+      HCMS_CUDA(cudaStreamWaitEvent(s_comp, plan->e_comm[c], 0));
+    st = do_attention(plan, ws + ck.off[0], ws + ck.off[1], ws + ck.off[2], ws + ck.off[3], c, scale, s_comp);
+    if (st) return st;
+    if (!serial) HCMS_CUDA(cudaEventRecord(plan->e_comp[c], s_comp));  // E_c^comp
+  }
+  // Phase 3 -- output all-to-all per chunk on S_comm (lines 20-23); A_c^out <- wait(E_c^comp)  (Eq. 7)
+  for (int c = 0; c < sh.C; ++c) {
+    const Chunk& ck = plan->chunks[c];
+    if (!serial) HCMS_CUDA(cudaStreamWaitEvent(s_out, plan->e_comp[c], 0));
+    st = host_route(3, ck, s_out);
+    if (st) return st;
+    const void* src[1] = {ws + ck.off[3]};
+    void* dst[1] = {out};
+    st = do_layout(plan, 1, src, dst, c, true, s_out);
+    if (st) return st;
+  }
+  if (!serial) {
+    // line 25: Synchronize(S_comm, S_comp) -- expressed as stream waits, the host is not blocked
+    HCMS_CUDA(cudaEventRecord(plan->e_fin_comm, s_out));
+    HCMS_CUDA(cudaEventRecord(plan->e_fin_comp, s_comp));
+    HCMS_CUDA(cudaStreamWaitEvent(caller, plan->e_fin_comm, 0));
+    HCMS_CUDA(cudaStreamWaitEvent(caller, plan->e_fin_comp, 0));
+    if (split) {
+      HCMS_CUDA(cudaEventRecord(plan->e_fin_in, s_in));
+      HCMS_CUDA(cudaStreamWaitEvent(caller, plan->e_fin_in, 0));
+    }
+  }
+  return HCMS_OK;
+}
+
+int hcms_attention_forward_host(hcms_plan_t* plan, const void* q, const void* k, const void* v, void* out, int64_t S,
+                                int H, int D, int P, int C, float scale, void* stream) {
+  if (!plan || !q || !k || !v || !out) return fail(HCMS_ERR_INVALID_ARG, "NULL argument");
+  const Shape& sh = plan->sh;
+  if (S != sh.S || H != sh.H || D != sh.D || P != sh.P || C != sh.C)
+    return fail(HCMS_ERR_PLAN_MISMATCH, "call shape differs from the plan's");
+  const size_t bytes = static_cast<size_t>(S) * H * D * sh.es;
+  for (int t = 0; t < 4; ++t)
+    if (!plan->staging[t]) HCMS_CUDA(cudaMalloc(&plan->staging[t], bytes));
+  cudaStream_t caller = static_cast<cudaStream_t>(stream);
+  const void* host_in[3] = {q, k, v};
+  for (int t = 0; t < 3; ++t)
+    HCMS_CUDA(cudaMemcpyAsync(plan->staging[t], host_in[t], bytes, cudaMemcpyHostToDevice, caller));
+  int st = hcms_attention_forward(plan, plan->staging[0], plan->staging[1], plan->staging[2], plan->staging[3], S, H, D,
+                                  P, C, scale, stream);
+  if (st) return st;
+  HCMS_CUDA(cudaMemcpyAsync(out, plan->staging[3], bytes, cudaMemcpyDeviceToHost, caller));
+  HCMS_CUDA(cudaStreamSynchronize(caller));
+  return HCMS_OK;
+}
+
+}  // extern "C"

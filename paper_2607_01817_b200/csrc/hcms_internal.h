@@ -1,0 +1,73 @@
+// Internal declarations shared by the translation units of libhcms (not installed).
+#pragma once
+
+#include <cuda.h>  // CUtensorMap and enums only; libcuda is reached through cudaGetDriverEntryPoint
+#include <cuda_runtime.h>
+
+#include <cstddef>
+#include <cstdint>
+#include <cstdio>
+#include <vector>
+
+#include "hcms.h"
+
+namespace hcms {
+
+// ---- error plumbing ---------------------------------------------------------------------
+int fail(int status, const char* fmt, ...);  // records thread-local text, returns status
+int fail_cuda(cudaError_t e, const char* what);
+
+#define HCMS_CUDA(expr)                                        \
+  do {                                                         \
+    cudaError_t e__ = (expr);                                  \
+    if (e__ != cudaSuccess) return ::hcms::fail_cuda(e__, #expr); \
+  } while (0)
+
+// ---- chunk geometry (Eq. 3 L83-84 on Hl = H/P; Table 8) ------------------------
+struct Chunk {
+  int o;             // first local head
+  int h;             // number of local heads
+  size_t bytes;      // P*S*h*D*es
+  size_t off[4];     // workspace byte offsets of Q'_c, K'_c, V'_c, O'_c
+};
+
+struct Shape {
+  int64_t S;
+  int H, D, P, C;
+  int es;            // element size in bytes
+  int Hl;            // heads per logical rank
+};
+
+// ---- layout kernels (layout_kernels.cu) -------------------------------------------------
+struct LayoutArgs {
+  const void* src[3];
+  void* dst[3];
+  int n_tensors;
+  int64_t S;
+  int H, D, P, Hl, es;
+  int o_c, h_c;
+  bool gather;       // false: [S,H,D] -> [P][S][h_c][D];  true: the inverse
+};
+cudaError_t launch_layout_vec(const LayoutArgs& a, cudaStream_t stream);
+cudaError_t launch_layout_tma(const LayoutArgs& a, cudaStream_t stream, int num_sms);
+
+// ---- attention kernel (attention_fwd.cu) ------------------------------------------------
+struct AttnArgs {
+  const void* q;     // [P][S][h_c][D] bf16
+  const void* k;
+  const void* v;
+  void* o;
+  int64_t S;
+  int D, P, h_c;
+  float scale;
+};
+cudaError_t launch_attention(const AttnArgs& a, cudaStream_t stream);
+cudaError_t attention_init();  // sets kernel attributes once; resolves cuTensorMapEncodeTiled
+
+// ---- driver entry point for tensor maps (tma_desc.cu) ------------------------------------
+// dims/strides innermost first; strides[0] is implied (element size). Returns cudaSuccess or an error.
+cudaError_t encode_tensor_map(CUtensorMap* out, CUtensorMapDataType dt, int rank, const void* base,
+                              const uint64_t* dims, const uint64_t* strides_bytes, const uint32_t* box,
+                              CUtensorMapSwizzle swizzle);
+
+}  // namespace hcms

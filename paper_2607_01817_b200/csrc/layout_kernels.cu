@@ -1,0 +1,240 @@
+// All-to-all layout kernels: the on-device stand-in for Ulysses' input / output all-to-all
+// (Algorithm 1 lines 8 and 21) for ONE head chunk.
+//
+//   scatter:  dense[p][s][j][d] = strided[s][p*Hl + o_c + j][d]      (input all-to-all)
+//   gather :  strided[s][p*Hl + o_c + j][d] = dense[p][s][j][d]      (output all-to-all + Concat)
+//
+// "strided" is the global [S,H,D] tensor (the P ranks' shards back to back), "dense" the
+// head-sharded chunk buffer [P][S][h_c][D].  Pure byte movement: every element is read once
+// and written once, so the roofline is HBM bandwidth (2*P*S*h_c*D*es bytes per tensor).
+//
+// Two variants, same bits out:
+//   * vec: 128-bit ld.global.nc / st.global, four independent requests per thread, one launch
+//          for Q,K,V (grid.z), destination-contiguous thread order;
+//   * tma: one elected thread per CTA drives a ring of shared-memory stages: a TMA bulk-tensor
+//          load of a [rows][h_c][D] box per (rank, head-chunk) tile, then a bulk store of the
+//          now contiguous tile (scatter), or the reverse (gather).  Few registers, no LSU work.
+#include "hcms_internal.h"
+#include "ptx.cuh"
+
+namespace hcms {
+using namespace ptx;
+
+// ------------------------------------------------------------------------------------------
+// vec variant
+// ------------------------------------------------------------------------------------------
+struct LayoutVecParams {
+  const uint4* src[3];
+  uint4* dst[3];
+  uint32_t n_per_rank;       // S * run_vecs  (16-byte vectors of one rank's dense block)
+  uint32_t run_vecs;         // h_c*D*es/16   (contiguous run in the strided tensor)
+  uint32_t row_stride_vecs;  // H*D*es/16
+  uint32_t rank_stride_vecs; // Hl*D*es/16
+  uint32_t chunk_off_vecs;   // o_c*D*es/16
+};
+
+__device__ __forceinline__ uint4 ld_stream(const uint4* p) {
+  uint4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+               : "l"(p));
+  return r;
+}
+__device__ __forceinline__ void st_stream(uint4* p, const uint4& v) {
+  asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x), "r"(v.y),
+               "r"(v.z), "r"(v.w)
+               : "memory");
+}
+
+constexpr int kVecThreads = 256;
+constexpr int kVecUnroll = 4;
+
+template <bool kGather>
+__global__ void __launch_bounds__(kVecThreads) layout_vec_kernel(const LayoutVecParams p) {
+  const uint32_t rank = blockIdx.y;
+  const uint4* __restrict__ src = p.src[blockIdx.z];
+  uint4* __restrict__ dst = p.dst[blockIdx.z];
+  const uint32_t i0 = blockIdx.x * (kVecThreads * kVecUnroll) + threadIdx.x;
+  const size_t dense_base = static_cast<size_t>(rank) * p.n_per_rank;
+  const size_t strided_base = static_cast<size_t>(rank) * p.rank_stride_vecs + p.chunk_off_vecs;
+
+  uint4 val[kVecUnroll];
+  size_t out_idx[kVecUnroll];
+#pragma unroll
+  for (int u = 0; u < kVecUnroll; ++u) {
+    const uint32_t i = i0 + u * kVecThreads;
+    if (i < p.n_per_rank) {
+      const uint32_t s = i / p.run_vecs;
+      const uint32_t w = i - s * p.run_vecs;
+      const size_t strided = static_cast<size_t>(s) * p.row_stride_vecs + strided_base + w;
+      const size_t dense = dense_base + i;
+      val[u] = ld_stream(src + (kGather ? dense : strided));
+      out_idx[u] = kGather ? strided : dense;
+    }
+  }
+#pragma unroll
+  for (int u = 0; u < kVecUnroll; ++u) {
+    const uint32_t i = i0 + u * kVecThreads;
+    if (i < p.n_per_rank) st_stream(dst + out_idx[u], val[u]);
+  }
+}
+
+cudaError_t launch_layout_vec(const LayoutArgs& a, cudaStream_t stream) {
+  LayoutVecParams p{};
+  const size_t run_bytes = static_cast<size_t>(a.h_c) * a.D * a.es;
+  const size_t n_per_rank = static_cast<size_t>(a.S) * (run_bytes / 16);
+  if (run_bytes % 16 || n_per_rank >= (1ull << 31)) return cudaErrorInvalidValue;
+  for (int t = 0; t < a.n_tensors; ++t) {
+    p.src[t] = static_cast<const uint4*>(a.src[t]);
+    p.dst[t] = static_cast<uint4*>(a.dst[t]);
+  }
+  p.n_per_rank = static_cast<uint32_t>(n_per_rank);
+  p.run_vecs = static_cast<uint32_t>(run_bytes / 16);
+  p.row_stride_vecs = static_cast<uint32_t>(static_cast<size_t>(a.H) * a.D * a.es / 16);
+  p.rank_stride_vecs = static_cast<uint32_t>(static_cast<size_t>(a.Hl) * a.D * a.es / 16);
+  p.chunk_off_vecs = static_cast<uint32_t>(static_cast<size_t>(a.o_c) * a.D * a.es / 16);
+  const uint32_t per_block = kVecThreads * kVecUnroll;
+  dim3 grid((p.n_per_rank + per_block - 1) / per_block, a.P, a.n_tensors);
+  if (a.gather)
+    layout_vec_kernel<true><<<grid, kVecThreads, 0, stream>>>(p);
+  else
+    layout_vec_kernel<false><<<grid, kVecThreads, 0, stream>>>(p);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------
+// tma variant
+// ------------------------------------------------------------------------------------------
+struct alignas(64) LayoutTmaMaps {
+  CUtensorMap strided[3];   // rank-3 maps over the global [S][H][D] tensors, box [rows][h_c][D]
+};
+
+struct LayoutTmaParams {
+  const uint8_t* dense_src[3];  // gather: dense buffers read with cp.async.bulk
+  uint8_t* dense_dst[3];        // scatter: dense buffers written with cp.async.bulk
+  int64_t S;
+  int P, Hl, o_c, n_tensors;
+  int rows;                     // rows per tile (box dim 2)
+  uint32_t row_bytes;           // h_c*D*es
+  uint32_t tiles_per_rank;      // ceil(S/rows)
+  uint32_t n_tiles;             // n_tensors*P*tiles_per_rank
+};
+
+constexpr int kTmaStages = 4;
+
+template <bool kGather>
+__global__ void __launch_bounds__(32) layout_tma_kernel(const __grid_constant__ LayoutTmaMaps maps,
+                                                         const LayoutTmaParams p) {
+  extern __shared__ __align__(128) uint8_t smem_raw[];
+  __shared__ __align__(8) uint64_t full_bar[kTmaStages];
+  if (threadIdx.x != 0) return;
+
+  const uint32_t tile_bytes = static_cast<uint32_t>(p.rows) * p.row_bytes;
+  const uint32_t smem_base = (smem_u32(smem_raw) + 127u) & ~127u;
+  for (int s = 0; s < kTmaStages; ++s) mbar_init(smem_u32(&full_bar[s]), 1);
+  fence_mbar_init();
+  fence_proxy_async_smem();
+
+  const uint32_t first = blockIdx.x, step = gridDim.x;
+  const uint32_t my_tiles = first < p.n_tiles ? (p.n_tiles - first + step - 1) / step : 0;
+
+  auto issue_load = [&](uint32_t k) {
+    const uint32_t tile = first + k * step;
+    const uint32_t stage = k % kTmaStages;
+    const uint32_t t = tile / (p.P * p.tiles_per_rank);
+    const uint32_t rem = tile - t * (p.P * p.tiles_per_rank);
+    const uint32_t rank = rem / p.tiles_per_rank;
+    const uint32_t rt = rem - rank * p.tiles_per_rank;
+    const int64_t s0 = static_cast<int64_t>(rt) * p.rows;
+    const uint32_t dst = smem_base + stage * tile_bytes;
+    const uint32_t bar = smem_u32(&full_bar[stage]);
+    if (!kGather) {
+      mbar_expect_tx(bar, tile_bytes);  // OOB rows are zero-filled and still counted
+      tma_load_3d(dst, &maps.strided[t], bar, 0, static_cast<int>(rank * p.Hl + p.o_c), static_cast<int>(s0));
+    } else {
+      const int64_t rows_valid = (p.S - s0) < p.rows ? (p.S - s0) : p.rows;
+      const uint32_t bytes = static_cast<uint32_t>(rows_valid) * p.row_bytes;
+      const uint8_t* src = p.dense_src[t] + (static_cast<size_t>(rank) * p.S + s0) * p.row_bytes;
+      mbar_expect_tx(bar, bytes);
+      bulk_load(dst, src, bytes, bar);
+    }
+  };
+
+  const uint32_t prologue = my_tiles < kTmaStages ? my_tiles : kTmaStages;
+  for (uint32_t k = 0; k < prologue; ++k) issue_load(k);
+
+  for (uint32_t k = 0; k < my_tiles; ++k) {
+    const uint32_t tile = first + k * step;
+    const uint32_t stage = k % kTmaStages;
+    const uint32_t t = tile / (p.P * p.tiles_per_rank);
+    const uint32_t rem = tile - t * (p.P * p.tiles_per_rank);
+    const uint32_t rank = rem / p.tiles_per_rank;
+    const uint32_t rt = rem - rank * p.tiles_per_rank;
+    const int64_t s0 = static_cast<int64_t>(rt) * p.rows;
+    const uint32_t src = smem_base + stage * tile_bytes;
+    mbar_wait(smem_u32(&full_bar[stage]), (k / kTmaStages) & 1);
+    if (!kGather) {
+      const int64_t rows_valid = (p.S - s0) < p.rows ? (p.S - s0) : p.rows;
+      const uint32_t bytes = static_cast<uint32_t>(rows_valid) * p.row_bytes;
+      uint8_t* dst = p.dense_dst[t] + (static_cast<size_t>(rank) * p.S + s0) * p.row_bytes;
+      bulk_store(dst, src, bytes);
+    } else {
+      tma_store_3d(&maps.strided[t], src, 0, static_cast<int>(rank * p.Hl + p.o_c), static_cast<int>(s0));
+    }
+    bulk_commit();
+    // stage (k-1)%N is free once the store issued in iteration k-1 has finished reading it
+    if (k >= 1 && (k - 1 + kTmaStages) < my_tiles) {
+      bulk_wait_read<1>();
+      issue_load(k - 1 + kTmaStages);
+    }
+  }
+  bulk_wait<0>();
+}
+
+cudaError_t launch_layout_tma(const LayoutArgs& a, cudaStream_t stream, int num_sms) {
+  const uint32_t row_bytes = static_cast<uint32_t>(a.h_c) * a.D * a.es;
+  if (row_bytes % 16 || a.D > 256) return cudaErrorInvalidValue;
+  // ~16 KB tiles: 4 stages x 16 KB x 3 CTAs/SM = 192 KB in flight per SM
+  int rows = static_cast<int>(16384 / row_bytes);
+  if (rows < 1) rows = 1;
+  if (rows > 256) rows = 256;
+  LayoutTmaMaps maps;
+  LayoutTmaParams p{};
+  const CUtensorMapDataType dt = a.es == 2 ? CU_TENSOR_MAP_DATA_TYPE_UINT16 : CU_TENSOR_MAP_DATA_TYPE_UINT32;
+  for (int t = 0; t < a.n_tensors; ++t) {
+    const void* strided = a.gather ? a.dst[t] : a.src[t];
+    const uint64_t dims[3] = {static_cast<uint64_t>(a.D), static_cast<uint64_t>(a.H), static_cast<uint64_t>(a.S)};
+    const uint64_t strides[2] = {static_cast<uint64_t>(a.D) * a.es, static_cast<uint64_t>(a.H) * a.D * a.es};
+    const uint32_t box[3] = {static_cast<uint32_t>(a.D), static_cast<uint32_t>(a.h_c), static_cast<uint32_t>(rows)};
+    cudaError_t e = encode_tensor_map(&maps.strided[t], dt, 3, strided, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_NONE);
+    if (e != cudaSuccess) return e;
+    p.dense_src[t] = static_cast<const uint8_t*>(a.src[t]);
+    p.dense_dst[t] = static_cast<uint8_t*>(a.dst[t]);
+  }
+  for (int t = a.n_tensors; t < 3; ++t) maps.strided[t] = maps.strided[0];
+  p.S = a.S;
+  p.P = a.P;
+  p.Hl = a.Hl;
+  p.o_c = a.o_c;
+  p.n_tensors = a.n_tensors;
+  p.rows = rows;
+  p.row_bytes = row_bytes;
+  p.tiles_per_rank = static_cast<uint32_t>((a.S + rows - 1) / rows);
+  p.n_tiles = static_cast<uint32_t>(a.n_tensors) * a.P * p.tiles_per_rank;
+  const size_t smem = static_cast<size_t>(kTmaStages) * rows * row_bytes + 128;
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaFuncSetAttribute(layout_tma_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+    cudaFuncSetAttribute(layout_tma_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+    attr_set = true;
+  }
+  uint32_t grid = static_cast<uint32_t>(num_sms) * 3;
+  if (grid > p.n_tiles) grid = p.n_tiles;
+  if (a.gather)
+    layout_tma_kernel<true><<<grid, 32, smem, stream>>>(maps, p);
+  else
+    layout_tma_kernel<false><<<grid, 32, smem, stream>>>(maps, p);
+  return cudaGetLastError();
+}
+
+}  // namespace hcms
