@@ -1,0 +1,411 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the HCMS hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl hcms|reference]
+
+A "step" is one pass of the whole hot path (Alg. 1 lines 4-26: per head chunk scatter ->
+attention -> gather on the comm / compute streams) over one batch of seeded synthetic Q/K/V of a
+BASELINE.json workload (default: configs[2], the video-DiT 720P-like shape SURVEY 8(d) names as
+the headline).  `value` = attention TFLOP/s of the layer = 4*S^2*D*H / wall time per step, with
+inputs resident in HBM; `ms_per_step` is the HCMS layer time in ms; `e2e` is the same metric
+through hcms_attention_forward_host with pinned HOST buffers (H2D of q,k,v and D2H of out inside
+the timed region).  `roofline` describes the attention kernel (the dominant kernel) against the
+measured dense bf16 peak; `layout` reports the all-to-all kernels in GB/s against the measured
+HBM copy bandwidth; `cpu_baseline` is the fp64 oracle timed on this box's host cores on a bounded
+sample (a baseline, not a target).  Under torchrun (N > 1) every rank runs an independent replica
+of the layer ("replicas only": the north star excludes a second GPU and NCCL from the data path).
+
+`--impl reference` times the oracle (oracle/hcms_oracle.py, as it stands) on the host cores on a
+bounded sample per step and prints the same line with "impl": "reference".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import hcms_inputs as I  # noqa: E402  (seeded inputs only; no method arithmetic)
+
+METRIC = "hcms_layer_attention_tflops"
+UNIT = "TFLOP/s"
+NOMINAL_BF16_TFLOPS = 2250.0
+NOMINAL_HBM_GBS = 8000.0
+FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}  # B200_PROFILING.md
+
+
+def parse_args(argv=None):
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", type=int, default=3, choices=sorted(I.WORKLOADS))
+    ap.add_argument("--chunks", type=int, default=0, help="override the workload's C")
+    ap.add_argument("--impl", default="hcms", choices=["hcms", "reference"])
+    ap.add_argument("--layout", default="vec", choices=["vec", "tma"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--cpu-rows", type=int, default=512, help="query rows per head in the cpu_baseline sample")
+    ap.add_argument("--ref-rows", type=int, default=96, help="query rows per head per step for --impl reference")
+    return ap.parse_args(argv)
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return {k: float(p[k]) for k in FALLBACK_PEAKS if k in p} | {"source": "measured"}
+    return dict(FALLBACK_PEAKS) | {"source": "fallback"}
+
+
+# ---------------------------------------------------------------------------------------------
+# multi-process plumbing (one process per GPU; gloo on CPU for the tests)
+# ---------------------------------------------------------------------------------------------
+
+def dist_init(use_cuda: bool):
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch.distributed as dist
+        if not dist.is_initialized():
+            os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+            os.environ.setdefault("MASTER_PORT", "29500")
+            dist.init_process_group("nccl" if use_cuda else "gloo", rank=rank, world_size=world)
+    return rank, local, world
+
+
+def barrier(world: int, use_cuda: bool):
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+    if use_cuda:
+        import torch
+        torch.cuda.synchronize()
+
+
+def max_over_ranks(x: float, world: int, use_cuda: bool) -> float:
+    """MAX over ranks of a per-rank duration (the job is as slow as its slowest replica)."""
+    if world == 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(x)], dtype=torch.float64, device="cuda" if use_cuda else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(units_per_rank_step: float, steps: int, world: int, local_ms_total: float, use_cuda: bool):
+    """Whole-job throughput: units all ranks processed / max-over-ranks time.  -> (value_per_s, ms_per_step)."""
+    ms_total = max_over_ranks(local_ms_total, world, use_cuda)
+    ms_per_step = ms_total / steps
+    return units_per_rank_step * world / (ms_per_step * 1e-3), ms_per_step
+
+
+# ---------------------------------------------------------------------------------------------
+# clocks during the timed region (B200_PROFILING.md recipe)
+# ---------------------------------------------------------------------------------------------
+
+class ClockSampler:
+    QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.lines, self.proc = [], None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), f"--query-gpu={self.QUERY}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append((time.time(), line.strip()))
+
+    def mark(self):
+        return time.time()
+
+    def stop(self, t0: float, t1: float):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, smax, power, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        rows = [l for (t, l) in self.lines if t0 <= t <= t1 + 0.1] or [l for (_, l) in self.lines[-3:]]
+        for l in rows:
+            c = [x.strip() for x in l.split(",")]
+            try:
+                sm.append(float(c[0])); smax.append(float(c[1])); power.append(float(c[2]))
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, c[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---------------------------------------------------------------------------------------------
+# the oracle on the host cores (cpu_baseline leg and --impl reference)
+# ---------------------------------------------------------------------------------------------
+
+def blas_threads() -> int:
+    try:
+        from threadpoolctl import threadpool_info
+        n = [i.get("num_threads", 1) for i in threadpool_info() if i.get("user_api") == "blas"]
+        return max(n) if n else 1
+    except Exception:
+        return 1
+
+
+def oracle_sample_rows(S: int, n_rows: int) -> np.ndarray:
+    return np.unique(np.linspace(0, S - 1, n_rows).astype(np.int64))
+
+
+def time_oracle_sample(w, q, k, v, rows) -> float:
+    """Seconds the oracle takes for `rows` query rows of every head (exact, independent evaluations)."""
+    from oracle import hcms_oracle as O          # test infrastructure: only this leg may touch it
+    t0 = time.perf_counter()
+    O.attention_sampled(q, k, v, w.scale, rows)
+    return time.perf_counter() - t0
+
+
+# ---------------------------------------------------------------------------------------------
+# the CUDA arm
+# ---------------------------------------------------------------------------------------------
+
+L2_BYTES = 126 * 1024 * 1024
+
+
+def run_hcms(args):
+    import torch
+    import paper_2607_01817_b200 as H   # raises if libhcms.so is missing: there is no fallback
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the HCMS hot path has no CPU fallback "
+                         "(use --impl reference for the oracle timing)")
+    rank, local, world = dist_init(True)
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    pk = peaks()
+
+    w = I.workload(args.config)
+    C = args.chunks or w.C
+    S, Hh, D, P = w.S, w.H, w.D, w.P
+    threads = max(1, (os.cpu_count() or 8) // max(1, world))
+    q, k, v = I.make_qkv(w, threads=threads)
+    if w.dtype == "f32":                      # config 1: the attention path takes the bf16 copy (reading R-12)
+        q, k, v = (I.f32_to_bf16_bits(t) for t in (q, k, v))
+    host = [torch.from_numpy(t.view(np.int16)).pin_memory() for t in (q, k, v)]
+    host_out = torch.empty_like(host[0]).pin_memory()
+    qd, kd, vd = (t.to(dev, non_blocking=True) for t in host)
+    out = torch.empty_like(qd)
+    torch.cuda.synchronize()
+
+    flop_step = 4.0 * S * S * D * Hh
+    tensor_bytes = S * Hh * D * 2
+    flush = 3 * tensor_bytes < 2 * L2_BYTES
+    flush_buf = torch.empty(2 * L2_BYTES, dtype=torch.uint8, device=dev) if flush else None
+    base_flags = H.HCMS_FLAG_PROFILE | (H.HCMS_FLAG_LAYOUT_TMA if args.layout == "tma" else 0)
+    stream = torch.cuda.current_stream()
+
+    def timed(plan, steps, fn):
+        """-> total ms of `steps` calls of fn on the current stream (CUDA events on that stream)."""
+        if flush:
+            total = 0.0
+            for _ in range(steps):
+                flush_buf.fill_(1)
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream); fn(); e1.record(stream)
+                e1.synchronize()
+                total += e0.elapsed_time(e1)
+            return total
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(steps):
+            fn()
+        e1.record(stream)
+        e1.synchronize()
+        return e0.elapsed_time(e1)
+
+    def kernel_times(plan, steps):
+        """Mean per-step (scatter, attention, gather) device ms per chunk over the last `steps` calls."""
+        n = min(steps, H.HCMS_PROFILE_RING)
+        acc = np.zeros((3, plan.C))
+        for back in range(n):
+            acc += np.asarray(H.hcms_plan_timings(plan, back))
+        return acc / n
+
+    # ---- main measurement: HCMS dual-stream pipeline ---------------------------------------
+    plan = H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, base_flags)
+    step = lambda: H.hcms_attention_forward(plan, qd, kd, vd, out, w.scale)
+    for _ in range(args.warmup):
+        step()
+    barrier(world, True)
+    sampler = ClockSampler(local)
+    time.sleep(0.25)
+    t_wall0 = sampler.mark()
+    ms_total = timed(plan, args.steps, step)
+    torch.cuda.synchronize()
+    t_wall1 = sampler.mark()
+    barrier(world, True)
+    clocks = sampler.stop(t_wall0, t_wall1)
+    launches = H.hcms_plan_last_launch_count(plan) * args.steps
+    kt = kernel_times(plan, args.steps)
+    value_per_s, ms_per_step = aggregate_value(flop_step, args.steps, world, ms_total, True)
+    _, h_c = H.hcms_chunk_table(plan)
+    attn_flop = [4.0 * S * S * D * P * h for h in h_c]
+    attn_ms = float(kt[1].sum())
+    achieved = sum(attn_flop) / (attn_ms * 1e-3) / 1e12
+    peak_tf = pk["bf16_tflops_sustained"]
+    result = {
+        "metric": METRIC, "value": round(value_per_s / 1e12, 2), "unit": UNIT, "n_gpus": world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(ms_per_step, 4),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[{args.config - 1}] ({w.name}): S={S} H={Hh} D={D} "
+                               f"P={P} C={C} chunks={h_c} non-causal scale=1/sqrt(D)",
+                   "S": S, "H": Hh, "D": D, "P": P, "C": C, "layout_kernel": args.layout,
+                   "l2": "flushed between steps" if flush else "inputs larger than L2 (3 x %d MB)" % (tensor_bytes >> 20),
+                   "multi_gpu": "replicas only" if world > 1 else "single GPU",
+                   "inputs": "hcms_inputs counter-based N(0,1) -> bf16 (seed %d)" % w.seed},
+        "clocks": clocks, "gpu_launches": launches,
+        "roofline": {"kernel": "attention_fwd_kernel<%d>" % D, "bound": "tensor", "achieved": round(achieved, 1),
+                     "peak": peak_tf, "unit": "TFLOP/s", "frac": round(achieved / peak_tf, 4),
+                     "peak_kind": "bf16 dense, sustained, %s" % pk["source"], "traffic": ATTN_TRAFFIC.get(args.config),
+                     "frac_of_burst": round(achieved / pk["bf16_tflops"], 4),
+                     "frac_of_nominal": round(achieved / NOMINAL_BF16_TFLOPS, 4),
+                     "attn_ms_per_step": round(attn_ms, 4), "flop_per_step": sum(attn_flop)},
+    }
+    plan.close()
+
+    # ---- serial (Ulysses, Eq. 1) pass: solo kernel times and the pipeline ratio ---------------
+    n_ser = min(args.steps, 10)
+    plan_s = H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, base_flags | H.HCMS_FLAG_SERIAL)
+    step_s = lambda: H.hcms_attention_forward(plan_s, qd, kd, vd, out, w.scale)
+    for _ in range(min(args.warmup, 3)):
+        step_s()
+    torch.cuda.synchronize()
+    ser_ms = timed(plan_s, n_ser, step_s) / n_ser
+    ks = kernel_times(plan_s, n_ser)
+    plan_s.close()
+    chunk_bytes = [2.0 * P * S * h * D * 2 for h in h_c]          # read + write, one tensor
+    copy_ms, comp_ms = float(ks[0].sum() + ks[2].sum()), float(ks[1].sum())
+    result["layout"] = {
+        "scatter_gbs": round(3 * sum(chunk_bytes) / (ks[0].sum() * 1e-3) / 1e9, 1),
+        "gather_gbs": round(sum(chunk_bytes) / (ks[2].sum() * 1e-3) / 1e9, 1),
+        "all_gbs": round(4 * sum(chunk_bytes) / (copy_ms * 1e-3) / 1e9, 1),
+        "peak_gbs": pk["hbm_gbs"], "peak_kind": "HBM copy, %s" % pk["source"],
+        "frac": round(4 * sum(chunk_bytes) / (copy_ms * 1e-3) / 1e9 / pk["hbm_gbs"], 4),
+        "frac_of_nominal": round(4 * sum(chunk_bytes) / (copy_ms * 1e-3) / 1e9 / NOMINAL_HBM_GBS, 4),
+        "bytes_per_step": 4 * sum(chunk_bytes), "copy_ms_per_step": round(copy_ms, 4),
+    }
+    result["pipeline"] = {
+        "hcms_ms": round(ms_per_step, 4), "serial_ms": round(ser_ms, 4), "speedup_vs_serial": round(ser_ms / ms_per_step, 4),
+        "attn_solo_ms": round(comp_ms, 4), "copy_solo_ms": round(copy_ms, 4), "rho": round(copy_ms / ser_ms, 4),
+        "wall_over_max_compute_copy": round(ms_per_step / max(comp_ms, copy_ms), 4),
+        "s_max_bound": round(H.hcms_model_s_max(copy_ms / ser_ms), 4),
+    }
+
+    # ---- end to end through the public host-buffer call --------------------------------------
+    if not args.no_e2e:
+        plan_e = H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, base_flags & ~H.HCMS_FLAG_PROFILE)
+        step_e = lambda: H.hcms_attention_forward_host(plan_e, host[0], host[1], host[2], host_out, w.scale)
+        n_e = min(args.steps, 10)
+        for _ in range(3):
+            step_e()
+        barrier(world, True)
+        t0 = time.perf_counter()
+        ms_e = timed(plan_e, n_e, step_e)
+        barrier(world, True)
+        wall_e = (time.perf_counter() - t0) * 1e3
+        ms_e = max(ms_e, 0.0)
+        v_e, ms_e_step = aggregate_value(flop_step, n_e, world, ms_e, True)
+        result["e2e"] = {"value": round(v_e / 1e12, 2), "unit": UNIT, "h2d_bytes_per_step": 3 * tensor_bytes,
+                         "d2h_bytes_per_step": tensor_bytes, "ms_per_step": round(ms_e_step, 3), "steps": n_e,
+                         "host_wall_ms_per_step": round(wall_e / n_e, 3),
+                         "api": "hcms_attention_forward_host (pinned host q,k,v -> out)"}
+        same = bool(torch.equal(host_out.to(dev), out))
+        result["e2e"]["bitwise_equal_to_device_path"] = same
+        plan_e.close()
+
+    # ---- the oracle on the host cores (rank 0, N = 1 only) -----------------------------------
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        rows = oracle_sample_rows(S, args.cpu_rows)
+        sec = time_oracle_sample(w, q, k, v, rows)
+        fl = 4.0 * len(rows) * S * D * Hh
+        result["cpu_baseline"] = {"value": round(fl / sec / 1e12, 6), "unit": UNIT, "cores": blas_threads(),
+                                  "host_cores": os.cpu_count(), "kind": "oracle", "seconds": round(sec, 2),
+                                  "sample": f"{len(rows)} evenly spaced query rows x all {Hh} heads "
+                                            f"({100.0 * len(rows) / S:.2f}% of the layer), fp64 numpy"}
+    if rank == 0:
+        print(json.dumps(result), flush=True)
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per attention launch summed over one step, from the
+# ncu --set full capture committed under profiles/ (bytes; None until captured for that config)
+ATTN_TRAFFIC = {}
+
+
+# ---------------------------------------------------------------------------------------------
+# the reference arm: the oracle, as it stands, on the host cores
+# ---------------------------------------------------------------------------------------------
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:           # under torchrun only rank 0 works; the others leave without touching the rendezvous
+        return
+    w = I.workload(args.config)
+    C = args.chunks or w.C
+    S, Hh, D, P = w.S, w.H, w.D, w.P
+    q, k, v = I.make_qkv(w, threads=os.cpu_count() or 8)
+    rows = oracle_sample_rows(S, args.ref_rows)
+    fl = 4.0 * len(rows) * S * D * Hh
+    for _ in range(args.warmup):
+        time_oracle_sample(w, q, k, v, rows)
+    t = [time_oracle_sample(w, q, k, v, rows) for _ in range(args.steps)]
+    sec = sum(t) / len(t)
+    val = round(fl / sec / 1e12, 6)
+    sample = (f"each step = {len(rows)} evenly spaced query rows x all {Hh} heads "
+              f"({100.0 * len(rows) / S:.2f}% of the layer), fp64 numpy oracle")
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": round(sec * 1e3, 3), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[{args.config - 1}] ({w.name}): S={S} H={Hh} D={D} P={P} C={C}",
+                   "S": S, "H": Hh, "D": D, "P": P, "C": C, "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": blas_threads(), "host_cores": os.cpu_count(),
+                         "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }), flush=True)
+
+
+def main(argv=None):
+    args = parse_args(argv)
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_hcms(args)
+
+
+if __name__ == "__main__":
+    main()

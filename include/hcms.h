@@ -77,6 +77,10 @@ enum {
 #define HCMS_FLAG_DEBUG_NO_COMM_WAIT 0x100u /* TEST ONLY: drop the compute stream's wait on E_c^comm
                                           (Eq. 6) so a negative test can observe the race */
 
+#define HCMS_FLAG_PROFILE 0x200u       /* record timing-enabled CUDA events around every scatter, attention
+                                          and gather of hcms_attention_forward, each on the stream it runs on;
+                                          read them with hcms_plan_timings */
+
 typedef struct hcms_plan hcms_plan_t;
 
 /* ---- introspection (host only, no GPU needed) ---------------------------------------- */
@@ -189,6 +193,20 @@ int hcms_attention_chunk(hcms_plan_t* plan, const void* qc, const void* kc, cons
 
 /* Number of kernels + async copies the last hcms_attention_forward on this plan enqueued. */
 int hcms_plan_last_launch_count(const hcms_plan_t* plan);
+
+/*
+ * Device durations, in milliseconds, of the steps of a recent hcms_attention_forward on a plan made
+ * with HCMS_FLAG_PROFILE.  calls_back = 0 is the last call, 1 the one before, ... up to
+ * HCMS_PROFILE_RING-1 calls are kept.  scatter_ms[c] = input all-to-all of chunk c (T_in share, incl.
+ * the host route if any), attn_ms[c] = attention of chunk c, gather_ms[c] = output all-to-all of
+ * chunk c; host arrays of C floats, any may be NULL.  Each is the elapsed time between two events
+ * recorded on the stream the step ran on, so time spent queueing behind another stream's kernels
+ * for the same SMs is included.  SYNCHRONISES the host with those events.
+ * Errors: INVALID_ARG (NULL plan, plan without HCMS_FLAG_PROFILE, calls_back out of range or
+ * older than the first call), CUDA.
+ */
+#define HCMS_PROFILE_RING 64
+int hcms_plan_timings(hcms_plan_t* plan, int calls_back, float* scatter_ms, float* attn_ms, float* gather_ms);
 
 #ifdef __cplusplus
 }

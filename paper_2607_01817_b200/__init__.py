@@ -39,6 +39,7 @@ HCMS_FLAG_HOST_ROUTE_K = 0x20
 HCMS_FLAG_HOST_ROUTE_V = 0x40
 HCMS_FLAG_HOST_ROUTE_O = 0x80
 HCMS_FLAG_DEBUG_NO_COMM_WAIT = 0x100
+HCMS_FLAG_PROFILE = 0x200
 
 # every symbol include/hcms.h declares: name -> (restype, argtypes)
 _SIGNATURES = {
@@ -63,6 +64,7 @@ _SIGNATURES = {
     "hcms_a2a_gather": (c_int, [c_void_p, c_void_p, c_void_p, c_int, c_void_p]),
     "hcms_attention_chunk": (c_int, [c_void_p] * 5 + [c_int, c_float, c_void_p]),
     "hcms_plan_last_launch_count": (c_int, [c_void_p]),
+    "hcms_plan_timings": (c_int, [c_void_p, c_int, POINTER(c_float), POINTER(c_float), POINTER(c_float)]),
 }
 
 
@@ -237,6 +239,16 @@ def hcms_chunk_layout(plan: Plan, c: int):
 
 def hcms_plan_last_launch_count(plan: Plan) -> int:
     return lib.hcms_plan_last_launch_count(plan.handle)
+
+
+HCMS_PROFILE_RING = 64
+
+
+def hcms_plan_timings(plan: Plan, calls_back: int = 0):
+    """-> (scatter_ms[C], attn_ms[C], gather_ms[C]) of a recent forward call (HCMS_FLAG_PROFILE plans)."""
+    arrs = [(c_float * plan.C)() for _ in range(3)]
+    _check(lib.hcms_plan_timings(plan.handle, calls_back, *arrs), "hcms_plan_timings")
+    return tuple(list(a) for a in arrs)
 
 
 # ---- the hot path ------------------------------------------------------------------------------

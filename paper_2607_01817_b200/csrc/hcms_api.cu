@@ -69,6 +69,9 @@ struct hcms_plan {
   // host-buffer entry point staging
   void* staging[4] = {nullptr, nullptr, nullptr, nullptr};
   int last_launches = 0;
+  // HCMS_FLAG_PROFILE: [step 0=scatter,1=attention,2=gather][begin,end][ring slot * C + chunk]
+  std::vector<cudaEvent_t> prof[3][2];
+  long long prof_calls = 0;   // forward calls that recorded a full set of events
 };
 
 static void plan_free(hcms_plan_t* p) {
@@ -82,6 +85,10 @@ static void plan_free(hcms_plan_t* p) {
   if (p->e_fin_comm) cudaEventDestroy(p->e_fin_comm);
   if (p->e_fin_comp) cudaEventDestroy(p->e_fin_comp);
   if (p->e_fin_in) cudaEventDestroy(p->e_fin_in);
+  for (auto& step : p->prof)
+    for (auto& side : step)
+      for (auto e : side)
+        if (e) cudaEventDestroy(e);
   if (p->s_comm) cudaStreamDestroy(p->s_comm);
   if (p->s_comm_out) cudaStreamDestroy(p->s_comm_out);
   if (p->s_comp) cudaStreamDestroy(p->s_comp);
@@ -224,6 +231,12 @@ int hcms_plan(hcms_plan_t** out, int64_t S, int H, int D, int P, int C, int dtyp
     PLAN_CUDA(cudaEventCreateWithFlags(&p->e_comm[c], cudaEventDisableTiming));
     PLAN_CUDA(cudaEventCreateWithFlags(&p->e_comp[c], cudaEventDisableTiming));
   }
+  if (flags & HCMS_FLAG_PROFILE)
+    for (auto& step : p->prof)
+      for (auto& side : step) {
+        side.assign(static_cast<size_t>(C) * HCMS_PROFILE_RING, nullptr);
+        for (auto& e : side) PLAN_CUDA(cudaEventCreate(&e));
+      }
   PLAN_CUDA(cudaMalloc(&p->ws, p->ws_bytes));
   p->ws_owned = true;
   if (dtype == HCMS_DTYPE_BF16) PLAN_CUDA(attention_init());
@@ -410,6 +423,12 @@ int hcms_attention_forward(hcms_plan_t* plan, const void* q, const void* k, cons
     return HCMS_OK;
   };
 
+  const bool profile = plan->flags & HCMS_FLAG_PROFILE;
+  auto mark = [&](int step, int c, int side, cudaStream_t s) -> cudaError_t {
+    const size_t slot = static_cast<size_t>(plan->prof_calls % HCMS_PROFILE_RING) * sh.C + c;
+    return profile ? cudaEventRecord(plan->prof[step][side][slot], s) : cudaSuccess;
+  };
+
   if (!serial) {
     HCMS_CUDA(cudaEventRecord(plan->e_main, caller));            // Alg. 1 line 5
     HCMS_CUDA(cudaStreamWaitEvent(s_in, plan->e_main, 0));       // line 7
@@ -421,12 +440,14 @@ int hcms_attention_forward(hcms_plan_t* plan, const void* q, const void* k, cons
     const Chunk& ck = plan->chunks[c];
     const void* src[3] = {q, k, v};
     void* dst[3] = {ws + ck.off[0], ws + ck.off[1], ws + ck.off[2]};
+    HCMS_CUDA(mark(0, c, 0, s_in));
     st = do_layout(plan, 3, src, dst, c, false, s_in);
     if (st) return st;
     for (int t = 0; t < 3; ++t) {
       st = host_route(t, ck, s_in);
       if (st) return st;
     }
+    HCMS_CUDA(mark(0, c, 1, s_in));
     if (!serial) HCMS_CUDA(cudaEventRecord(plan->e_comm[c], s_in));  // E_c^comm
   }
   // Phase 2 -- attention per chunk on S_comp (lines 14-18); Attn_c <- wait(E_c^comm)  (Eq. 6)
@@ -434,21 +455,26 @@ int hcms_attention_forward(hcms_plan_t* plan, const void* q, const void* k, cons
     const Chunk& ck = plan->chunks[c];
     if (!serial && !(plan->flags & HCMS_FLAG_DEBUG_NO_COMM_WAIT))
       HCMS_CUDA(cudaStreamWaitEvent(s_comp, plan->e_comm[c], 0));
+    HCMS_CUDA(mark(1, c, 0, s_comp));
     st = do_attention(plan, ws + ck.off[0], ws + ck.off[1], ws + ck.off[2], ws + ck.off[3], c, scale, s_comp);
     if (st) return st;
+    HCMS_CUDA(mark(1, c, 1, s_comp));
     if (!serial) HCMS_CUDA(cudaEventRecord(plan->e_comp[c], s_comp));  // E_c^comp
   }
   // Phase 3 -- output all-to-all per chunk on S_comm (lines 20-23); A_c^out <- wait(E_c^comp)  (Eq. 7)
   for (int c = 0; c < sh.C; ++c) {
     const Chunk& ck = plan->chunks[c];
     if (!serial) HCMS_CUDA(cudaStreamWaitEvent(s_out, plan->e_comp[c], 0));
+    HCMS_CUDA(mark(2, c, 0, s_out));
     st = host_route(3, ck, s_out);
     if (st) return st;
     const void* src[1] = {ws + ck.off[3]};
     void* dst[1] = {out};
     st = do_layout(plan, 1, src, dst, c, true, s_out);
     if (st) return st;
+    HCMS_CUDA(mark(2, c, 1, s_out));
   }
+  if (profile) plan->prof_calls += 1;
   if (!serial) {
     // line 25: Synchronize(S_comm, S_comp) -- expressed as stream waits, the host is not blocked
     HCMS_CUDA(cudaEventRecord(plan->e_fin_comm, s_out));
@@ -460,6 +486,24 @@ int hcms_attention_forward(hcms_plan_t* plan, const void* q, const void* k, cons
       HCMS_CUDA(cudaStreamWaitEvent(caller, plan->e_fin_in, 0));
     }
   }
+  return HCMS_OK;
+}
+
+int hcms_plan_timings(hcms_plan_t* plan, int calls_back, float* scatter_ms, float* attn_ms, float* gather_ms) {
+  if (!plan) return fail(HCMS_ERR_INVALID_ARG, "plan is NULL");
+  if (!(plan->flags & HCMS_FLAG_PROFILE)) return fail(HCMS_ERR_INVALID_ARG, "plan was made without HCMS_FLAG_PROFILE");
+  if (calls_back < 0 || calls_back >= HCMS_PROFILE_RING || calls_back >= plan->prof_calls)
+    return fail(HCMS_ERR_INVALID_ARG, "calls_back=%d: %lld profiled calls so far, ring keeps %d", calls_back,
+                plan->prof_calls, HCMS_PROFILE_RING);
+  const size_t base = static_cast<size_t>((plan->prof_calls - 1 - calls_back) % HCMS_PROFILE_RING) * plan->sh.C;
+  float* outs[3] = {scatter_ms, attn_ms, gather_ms};
+  for (int step = 0; step < 3; ++step)
+    for (int c = 0; c < plan->sh.C; ++c) {
+      HCMS_CUDA(cudaEventSynchronize(plan->prof[step][1][base + c]));
+      float ms = 0.f;
+      HCMS_CUDA(cudaEventElapsedTime(&ms, plan->prof[step][0][base + c], plan->prof[step][1][base + c]));
+      if (outs[step]) outs[step][c] = ms;
+    }
   return HCMS_OK;
 }
 

@@ -1,0 +1,148 @@
+"""CPU-only checks of the C-ABI boundary: libhcms.so loads, exports every symbol include/hcms.h
+declares, and its host-only entry points (chunk table, time model, argument validation) behave as
+the header says.  No compute call is made here (there is no GPU on the CI box)."""
+import math
+import os
+import re
+
+import pytest
+
+import paper_2607_01817_b200 as H
+from paper_2607_01817_b200 import build as hbuild
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module", autouse=True)
+def built_library():
+    hbuild.build()          # no-op when libhcms.so is newer than its sources
+    assert os.path.exists(H.LIB_PATH)
+
+
+def _declared_symbols():
+    text = open(os.path.join(ROOT, "include", "hcms.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)          # strip comments
+    return sorted(set(re.findall(r"\b(hcms_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_every_declared_symbol_is_exported_and_bound():
+    declared = _declared_symbols()
+    assert len(declared) >= 20
+    for name in declared:
+        assert getattr(H.lib, name) is not None, name           # dlsym succeeds
+    assert sorted(H._SIGNATURES) == declared                       # binding covers the header, nothing more
+
+
+def test_binding_mirrors_header_constants():
+    text = open(os.path.join(ROOT, "include", "hcms.h")).read()
+    for name, val in re.findall(r"#define\s+(HCMS_FLAG_[A-Z_]+)\s+(0x[0-9a-fA-F]+)u", text):
+        assert getattr(H, name) == int(val, 16), name
+    for name, val in re.findall(r"(HCMS_(?:OK|ERR_[A-Z_]+|DTYPE_[A-Z0-9]+))\s*=\s*(-?\d+)", text):
+        assert getattr(H, name) == int(val), name
+    assert H.hcms_version() == int(re.search(r"#define\s+HCMS_VERSION\s+(\d+)", text).group(1))
+
+
+def test_status_strings():
+    assert H.hcms_status_string(0) == "HCMS_OK"
+    assert H.hcms_status_string(H.HCMS_ERR_ALIAS) == "HCMS_ERR_ALIAS"
+    assert H.hcms_status_string(-1234) == "HCMS_ERR_UNKNOWN"
+
+
+def test_chunk_table_matches_table8(golden_rows):
+    # PAPER.md Table 8 (L292-300): H_per_rank = 10
+    for cells in golden_rows("table8_chunks.txt"):
+        C, sizes = int(cells[0]), [int(s) for s in cells[1].split()]
+        o, h = H.hcms_chunk_table_host(10, C)
+        assert h == sizes
+        assert o == [sum(sizes[:i]) for i in range(C)]
+
+
+@pytest.mark.parametrize("Hl", [1, 2, 3, 5, 10, 24, 40])
+def test_chunk_table_invariants(Hl):
+    for C in range(1, Hl + 1):
+        o, h = H.hcms_chunk_table_host(Hl, C)
+        assert sum(h) == Hl and min(h) >= 1 and max(h) - min(h) <= 1
+        assert h == sorted(h, reverse=True)                        # "more-first-less-later" (L221)
+        assert all(h[c] == Hl // C + (1 if c < Hl % C else 0) for c in range(C))   # Eq. 3
+        assert o == [sum(h[:i]) for i in range(C)]
+
+
+def test_chunk_table_errors():
+    for args, code in [((0, 1), H.HCMS_ERR_INVALID_ARG), ((4, 0), H.HCMS_ERR_INVALID_ARG),
+                       ((4, -2), H.HCMS_ERR_INVALID_ARG), ((3, 4), H.HCMS_ERR_UNSUPPORTED_SHAPE)]:
+        with pytest.raises(H.HcmsError) as ei:
+            H.hcms_chunk_table_host(*args)
+        assert ei.value.status == code
+        assert H.hcms_last_error() != ""
+
+
+def test_time_model(golden_rows):
+    # Table 13 (L449-456): S_max = 1/(1-rho)
+    for cells in golden_rows("table13_smax.txt"):
+        rho, smax = float(cells[0]) / 100.0, float(cells[1])
+        assert abs(H.hcms_model_s_max(rho) - smax) < 6e-3
+    # Table 12 row 1 (L440) + Table 17 (L515): rho, beta, T_total -> C* rounds to the printed 5
+    rows = golden_rows("table12_cstar.txt")
+    rho, beta, t_total, c_pred = (float(x) for x in rows[0][:4])
+    rho /= 100.0
+    assert round(H.hcms_model_c_star(rho * t_total, beta)) == int(c_pred)
+    # Eq. 11 == T_base / T_hcms (Eq. 9 / Eq. 10) for any parameters
+    t0, t_comm, t_attn, beta = 3.0, 29.0, 41.3, 1.41
+    t_base = t0 + t_comm + t_attn
+    for C in range(1, 9):
+        s = t_base / H.hcms_model_t_hcms(C, t0, t_comm, t_attn, beta)
+        assert abs(s - H.hcms_model_speedup(C, t_comm / t_base, beta, t_base)) < 1e-12
+    assert H.hcms_model_t_hcms(1, t0, t_comm, t_attn, 0.0) == t_base        # C=1, beta=0 is the baseline
+    # d/dC T_hcms vanishes at C*: neighbours are not better
+    cs = H.hcms_model_c_star(t_comm, beta)
+    f = lambda c: t0 + t_comm / c + t_attn + c * beta
+    assert f(cs) <= f(cs * 1.01) and f(cs) <= f(cs * 0.99)
+    # domain errors yield NaN
+    assert math.isnan(H.hcms_model_c_star(1.0, 0.0)) and math.isnan(H.hcms_model_s_max(1.0))
+    assert math.isnan(H.hcms_model_t_hcms(0, 1, 1, 1, 1)) and math.isnan(H.hcms_model_speedup(0, .1, .1, 1))
+
+
+def test_plan_argument_validation_precedes_device_use():
+    bf16 = H.HCMS_DTYPE_BF16
+    cases = [
+        ((0, 4, 64, 2, 2, bf16), H.HCMS_ERR_INVALID_ARG),
+        ((1024, 4, 64, 2, 0, bf16), H.HCMS_ERR_INVALID_ARG),
+        ((1024, 4, 64, 2, 2, 77), H.HCMS_ERR_UNSUPPORTED_DTYPE),
+        ((1023, 4, 64, 2, 2, bf16), H.HCMS_ERR_UNSUPPORTED_SHAPE),     # S % P
+        ((1024, 5, 64, 2, 2, bf16), H.HCMS_ERR_UNSUPPORTED_SHAPE),     # H % P
+        ((1024, 4, 96, 2, 2, bf16), H.HCMS_ERR_UNSUPPORTED_SHAPE),     # D not in {64,128}
+        ((1024, 4, 64, 2, 3, bf16), H.HCMS_ERR_UNSUPPORTED_SHAPE),     # C > H/P
+    ]
+    for args, code in cases:
+        with pytest.raises(H.HcmsError) as ei:
+            H.hcms_plan(*args)
+        assert ei.value.status == code, args
+
+
+def test_no_cpu_fallback_without_device():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    with pytest.raises(H.HcmsError) as ei:
+        H.hcms_plan(1024, 4, 64, 2, 2)
+    assert ei.value.status in (H.HCMS_ERR_UNSUPPORTED_DEVICE, H.HCMS_ERR_CUDA)
+
+
+def test_null_plan_queries():
+    assert H.lib.hcms_plan_workspace_bytes(None) == 0
+    assert H.lib.hcms_plan_last_launch_count(None) == 0
+    assert H.lib.hcms_plan_destroy(None) == 0
+    assert H.lib.hcms_attention_forward(None, None, None, None, None, 1, 1, 64, 1, 1, 1.0, None) == H.HCMS_ERR_INVALID_ARG
+
+
+def test_product_does_not_import_oracle():
+    """The product path shares nothing with the oracle (and has no CPU fallback to route through)."""
+    pkg = os.path.join(ROOT, "paper_2607_01817_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert "oracle" not in text.replace("no CPU fallback", ""), f
+                assert "hcms_inputs" not in text, f
+    otext = open(os.path.join(ROOT, "oracle", "hcms_oracle.py")).read()
+    assert "import paper_2607_01817_b200" not in otext and "ctypes" not in otext

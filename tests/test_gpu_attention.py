@@ -1,0 +1,246 @@
+"""-m gpu: the whole hot path (hcms_attention_forward: scatter -> attention -> gather per head chunk on
+two streams) and the attention kernel alone (hcms_attention_chunk), through the C ABI, against the
+fp64 oracle.
+
+Tolerance (BASELINE.json north_star, bf16 inputs): max-abs <= 2e-2 and mean-abs <= 2e-3 over the
+compared elements; plus relative L2 <= 1e-2 (for long sequences |O| ~ 1/sqrt(S/e), so
+the absolute gates alone would pass an all-zero output).  Integer/bit claims are exact: one-hot
+rows reproduce a V row bit for bit, and the output is bitwise independent of P and C (PAPER.md
+L304, Table 14).
+"""
+import numpy as np
+import pytest
+import torch
+
+import hcms_inputs as I
+import paper_2607_01817_b200 as H
+from oracle import hcms_oracle as O
+from gpu_util import DEV, bf16_bits_to_f64, nan_fill_, to_dev, to_host
+
+pytestmark = pytest.mark.gpu
+
+MAX_ABS, MEAN_ABS, REL_L2 = 2e-2, 2e-3, 1e-2
+
+
+def run_forward(q, k, v, S, Hh, D, P, C, scale, flags=0, poison=True):
+    """q,k,v: uint16 bf16 bit patterns [S,H,D] on the host -> uint16 [S,H,D] output bits.
+
+    Dependency poison test: ``out`` and the chunk workspace start as bf16 NaN, so a
+    chunk whose attention ran before its scatter, or a gather before its attention, shows up as NaN."""
+    qd, kd, vd = to_dev(q), to_dev(k), to_dev(v)
+    out = nan_fill_(torch.empty_like(qd))
+    with H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, flags) as plan:
+        if poison:
+            n = H.hcms_plan_workspace_bytes(plan)
+            ws = nan_fill_(torch.empty((n + 1) // 2, dtype=torch.int16, device=DEV))
+            H.hcms_plan_set_workspace(plan, ws, n)
+        H.hcms_attention_forward(plan, qd, kd, vd, out, scale)
+        torch.cuda.synchronize()
+    return to_host(out)
+
+
+def check(got_bits, ref, what=""):
+    got = bf16_bits_to_f64(got_bits)
+    assert not np.isnan(got).any(), f"{what}: NaN in the output (a chunk ran before its all-to-all?)"
+    err = np.abs(got - ref)
+    rel = np.linalg.norm(got - ref) / np.linalg.norm(ref)
+    assert err.max() <= MAX_ABS and err.mean() <= MEAN_ABS and rel <= REL_L2, \
+        f"{what}: max_abs={err.max():.3e} mean_abs={err.mean():.3e} rel_l2={rel:.3e}"
+    return err.max(), err.mean(), rel
+
+
+# ---------------------------------------------------------------------------------------------
+# full-tensor parity on the configs the oracle finishes in seconds, and ragged shapes
+# ---------------------------------------------------------------------------------------------
+
+def test_config1_tiny_full():
+    w = I.workload(1)                                  # fp32 N(0,1) from seed 0 (BASELINE.json configs[0])
+    q32, k32, v32 = I.make_qkv(w)
+    q, k, v = (I.f32_to_bf16_bits(t) for t in (q32, k32, v32))       # reading R-12: bf16 copy of the same data
+    got = run_forward(q, k, v, w.S, w.H, w.D, w.P, w.C, w.scale)
+    check(got, O.attention_full(q, k, v, w.scale), "cfg1")
+    # ungated report vs the unrounded fp32 inputs
+    err32 = np.abs(bf16_bits_to_f64(got) - O.attention_full(q32, k32, v32, w.scale)).max()
+    print(f"cfg1 vs fp32-input oracle: max_abs={err32:.3e}")
+
+
+def test_config2_uneven_full():
+    w = I.workload(2)                                  # Hl = 3 split 2+1
+    q, k, v = I.make_qkv(w)
+    got = run_forward(q, k, v, w.S, w.H, w.D, w.P, w.C, w.scale)
+    check(got, O.attention_full(q, k, v, w.scale), "cfg2")
+
+
+RAGGED = [  # S, H, D, P, C  -- S = 128k + r for r in {1, 96, 120, 127}, Sl not 128-aligned, 1-2 tile cases
+    (129, 2, 128, 1, 2), (224, 2, 64, 2, 1), (2168, 4, 128, 2, 2), (1151, 3, 128, 1, 3),
+    (1000, 6, 64, 2, 3), (64, 2, 128, 2, 1), (2, 2, 64, 2, 1), (384, 2, 128, 2, 1), (2046, 20, 128, 2, 4),
+]
+
+
+@pytest.mark.parametrize("S,Hh,D,P,C", RAGGED)
+def test_ragged_shapes_full(S, Hh, D, P, C):
+    w = I.Workload("ragged", S, Hh, D, P, C, 100 + S, "bf16", 1.0)
+    q, k, v = I.make_qkv(w)
+    got = run_forward(q, k, v, S, Hh, D, P, C, w.scale)
+    ref = O.attention_full(q, k, v, w.scale)
+    check(got, ref, f"S={S}")
+    # the last (partial) KV tile and the last Q tile specifically
+    tail = S - (S % 128 or 128)
+    err_tail = np.abs(bf16_bits_to_f64(got[tail:]) - ref[tail:])
+    assert err_tail.max() <= MAX_ABS
+
+
+# ---------------------------------------------------------------------------------------------
+# closed forms with O(1) outputs
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("S,Hh,D,P,C", [(1000, 4, 128, 2, 2), (777, 2, 64, 1, 2)])
+def test_uniform_v_gives_v(S, Hh, D, P, C):
+    w = I.Workload("uv", S, Hh, D, P, C, 5, "bf16", 1.0)
+    q, k, _ = I.make_qkv(w)
+    c_h = I.f32_to_bf16_bits(np.float32([1.0 + 0.25 * h for h in range(Hh)]))        # exact in bf16
+    v = np.broadcast_to(c_h[None, :, None], (S, Hh, D)).copy()
+    got = bf16_bits_to_f64(run_forward(q, k, v, S, Hh, D, P, C, w.scale))
+    ref = np.broadcast_to(bf16_bits_to_f64(c_h)[None, :, None], (S, Hh, D))
+    # softmax weights sum to 1 up to the fp32 sum and bf16 P rounding: O = c_h within bf16 resolution
+    assert np.abs(got - ref).max() <= 2 ** -7 * 2.0, np.abs(got - ref).max()
+    assert np.array_equal(np.round(got[0, :, 0] * 4), np.round(ref[0, :, 0] * 4))   # heads not mixed up
+
+
+@pytest.mark.parametrize("S,Hh,D,P,C", [(1144, 2, 128, 2, 1), (500, 2, 64, 1, 2)])
+def test_one_hot_scores_select_v_row_bitwise(S, Hh, D, P, C):
+    """Q[i] = alpha*K[pi(i)] with a margin of >= 30 nats: O[i] = V[pi(i)], on the GPU bit-equal to that
+    bf16 row; targets include keys in the last partial KV tile."""
+    w = I.Workload("onehot", S, Hh, D, P, C, 9, "bf16", 1.0)
+    _, k, v = I.make_qkv(w)
+    rng = np.random.default_rng(1)
+    pi = rng.permutation(S)
+    pi[:8] = S - 1 - np.arange(8)                           # force targets into the ragged tail
+    kf = I.bf16_bits_to_f32(k)
+    alpha = np.float32(64.0)                                 # exact scaling in bf16
+    q = I.f32_to_bf16_bits(alpha * kf[pi])
+    # margin check in fp64 (oracle side): s_target - max_other >= 30 nats for every row
+    ref = O.attention_full(q, k, v, w.scale)
+    vf = bf16_bits_to_f64(v)
+    assert np.abs(ref - vf[pi]).max() < 1e-9                 # oracle closed form
+    got = run_forward(q, k, v, S, Hh, D, P, C, w.scale)
+    assert np.array_equal(got, v[pi])
+
+
+def test_scale_zero_is_mean_of_v():
+    S, Hh, D, P, C = 1000, 2, 128, 2, 1
+    w = I.Workload("s0", S, Hh, D, P, C, 3, "bf16", 1.0)
+    q, k, v = I.make_qkv(w)
+    got = bf16_bits_to_f64(run_forward(q, k, v, S, Hh, D, P, C, 0.0))
+    ref = bf16_bits_to_f64(v).mean(axis=0, keepdims=True)
+    assert np.abs(got - ref).max() <= 2e-3 + 2 ** -8 * np.abs(ref).max()
+
+
+# ---------------------------------------------------------------------------------------------
+# the paper's equivalence claim on the GPU: bitwise independent of C, P, schedule and entry point
+# ---------------------------------------------------------------------------------------------
+
+def test_output_bitwise_independent_of_C_P_and_schedule():
+    S, Hh, D = 2040, 12, 128
+    w = I.Workload("inv", S, Hh, D, 1, 1, 21, "bf16", 1.0)
+    q, k, v = I.make_qkv(w)
+    base = run_forward(q, k, v, S, Hh, D, 1, 1, w.scale, flags=H.HCMS_FLAG_SERIAL)      # Ulysses C=1, P=1
+    check(base, O.attention_full(q, k, v, w.scale), "invariance base")
+    for P in (1, 2, 3, 4, 6):
+        for C in range(1, Hh // P + 1):
+            for flags in (0, H.HCMS_FLAG_SERIAL, H.HCMS_FLAG_LAYOUT_TMA, H.HCMS_FLAG_SPLIT_COMM):
+                if flags and C not in (2, Hh // P):
+                    continue
+                got = run_forward(q, k, v, S, Hh, D, P, C, w.scale, flags=flags)
+                assert np.array_equal(got, base), (P, C, flags)          # max error 0 (Table 14)
+
+
+def test_repeated_calls_and_host_entry_point_agree():
+    w = I.workload(1)
+    q, k, v = (I.f32_to_bf16_bits(t) for t in I.make_qkv(w))
+    qd, kd, vd = to_dev(q), to_dev(k), to_dev(v)
+    out = nan_fill_(torch.empty_like(qd))
+    with H.hcms_plan(w.S, w.H, w.D, w.P, w.C) as plan:
+        stream = torch.cuda.Stream()
+        with torch.cuda.stream(stream):
+            for _ in range(3):                                            # back-to-back reuse of events/workspace
+                H.hcms_attention_forward(plan, qd, kd, vd, out, w.scale)
+            assert H.hcms_plan_last_launch_count(plan) == 3 * w.C          # scatter + attention + gather per chunk
+        stream.synchronize()
+        dev_bits = to_host(out)
+        host_out = np.zeros_like(q)
+        H.hcms_attention_forward_host(plan, q, k, v, host_out, w.scale)
+        assert np.array_equal(host_out, dev_bits)
+    check(dev_bits, O.attention_full(q, k, v, w.scale), "cfg1 repeat")
+
+
+def test_attention_chunk_alone_matches_oracle_on_sharded_buffers():
+    S, Hh, D, P, C = 1280, 6, 128, 2, 2
+    w = I.Workload("chunk", S, Hh, D, P, C, 33, "bf16", 1.0)
+    q, k, v = I.make_qkv(w)
+    with H.hcms_plan(S, Hh, D, P, C) as plan:
+        _, h = H.hcms_chunk_table(plan)
+        for c in range(C):
+            qc, kc, vc = (O.scatter_chunk(t, P, C, c) for t in (q, k, v))   # oracle-made head-sharded inputs
+            oc = nan_fill_(torch.empty((P, S, h[c], D), dtype=torch.int16, device=DEV))
+            H.hcms_attention_chunk(plan, to_dev(qc), to_dev(kc), to_dev(vc), oc, c, w.scale)
+            torch.cuda.synchronize()
+            got = to_host(oc)
+            for p in range(P):
+                for j in range(h[c]):
+                    ref = O.attention_rows(O.widen_to_f64(qc[p, :, j]), O.widen_to_f64(kc[p, :, j]),
+                                           O.widen_to_f64(vc[p, :, j]), w.scale)
+                    check(got[p, :, j], ref, f"chunk {c} rank {p} head {j}")
+
+
+# ---------------------------------------------------------------------------------------------
+# BASELINE.json configs[2..4] at full size, sampled rows (each an exact, independent evaluation)
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("cfg", [3, 4, 5])
+def test_full_size_configs_sampled_rows(cfg):
+    w = I.workload(cfg)
+    q, k, v = I.make_qkv(w, threads=16)
+    got = run_forward(q, k, v, w.S, w.H, w.D, w.P, w.C, w.scale, poison=True)
+    rows = O.sample_rows(w.S, w.P, n_random=24 if cfg == 5 else 48, seed=cfg)
+    ref = O.attention_sampled(q, k, v, w.scale, rows)
+    mx, mean, rel = check(got[rows], ref, f"cfg{cfg}")
+    print(f"cfg{cfg}: rows={len(rows)} max_abs={mx:.3e} mean_abs={mean:.3e} rel_l2={rel:.3e}")
+    # a property of every element, at any size: each output coordinate lies in [min_s V, max_s V]
+    vf = I.bf16_bits_to_f32(v)
+    gf = I.bf16_bits_to_f32(got)
+    assert not np.isnan(gf).any()
+    assert (gf <= vf.max(axis=0, keepdims=True)).all() and (gf >= vf.min(axis=0, keepdims=True)).all()
+    # sanity against an all-zero / wrong-magnitude output: sampled norm within 2 % of the oracle's
+    assert abs(np.linalg.norm(bf16_bits_to_f64(got[rows])) / np.linalg.norm(ref) - 1) < 2e-2
+
+
+# ---------------------------------------------------------------------------------------------
+# error behaviour with a device present
+# ---------------------------------------------------------------------------------------------
+
+def test_forward_argument_errors():
+    S, Hh, D, P, C = 256, 4, 64, 2, 2
+    n = S * Hh * D
+    buf = torch.zeros(4 * n + 64, dtype=torch.int16, device=DEV)
+    q, k, v, out = (buf[i * n:(i + 1) * n] for i in range(4))
+    with H.hcms_plan(S, Hh, D, P, C) as plan:
+        def status(fn):
+            with pytest.raises(H.HcmsError) as ei:
+                fn()
+            return ei.value.status
+        assert status(lambda: H.hcms_attention_forward(plan, q, k, v, q, 0.125)) == H.HCMS_ERR_ALIAS
+        assert status(lambda: H.hcms_attention_forward(plan, q, k, v, buf[3 * n - 8:4 * n - 8], 0.125)) == H.HCMS_ERR_ALIAS
+        assert status(lambda: H.hcms_attention_forward(plan, q, k, v, buf[3 * n + 1:4 * n + 1], 0.125)) == H.HCMS_ERR_MISALIGNED
+        assert status(lambda: H.hcms_attention_forward(plan, q, k, v, out, float("nan"))) == H.HCMS_ERR_INVALID_ARG
+        assert status(lambda: H.hcms_attention_forward(plan, q, k, v, out, -1.0)) == H.HCMS_ERR_INVALID_ARG
+        assert status(lambda: H.hcms_attention_forward(plan, q, None, v, out, 0.125)) == H.HCMS_ERR_INVALID_ARG
+        st = H.lib.hcms_attention_forward(plan.handle, q.data_ptr(), k.data_ptr(), v.data_ptr(), out.data_ptr(),
+                                          S, Hh, D, P, C + 1, 0.125, None)
+        assert st == H.HCMS_ERR_PLAN_MISMATCH
+        H.hcms_attention_forward(plan, q, k, v, out, 0.125)              # and a valid call still works
+        torch.cuda.synchronize()
+    with H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_F32) as plan32:
+        with pytest.raises(H.HcmsError) as ei:
+            H.hcms_attention_forward(plan32, q, k, v, out, 0.125)
+        assert ei.value.status == H.HCMS_ERR_UNSUPPORTED_DTYPE
