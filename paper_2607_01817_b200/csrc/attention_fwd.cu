@@ -5,18 +5,29 @@
 //     O'[p][i][j][:] = sum_k softmax_k(scale * Q'[p][i][j] . K'[p][k][j]) V'[p][k][j][:]
 // on head-sharded buffers [P][S][h_c][D] (bf16 in, fp32 scores/softmax/accumulate, bf16 out).
 //
-// One CTA = one head x 256 query rows (two 128-row Q tiles that ping-pong), 384 threads:
-//   warp 0      TMA producer: Q tiles once, then K_j / V_j tiles through a shared-memory ring
-//   warp 1      MMA issuer (one lane): S_t = Q_t K_j^T (SS, M=128,N=128), O_t += P_t V_j (TS: P read from TMEM)
-//   warp 2      TMEM allocator (512 columns: S_0,S_1 at 0/128 (P_t aliases S_t as packed bf16), O_0,O_1 at 256+)
-//   warps 4-7   softmax warpgroup of tile 0: one thread per query row, online softmax in fp32 with lazy
-//   warps 8-11  softmax warpgroup of tile 1    rescaling of O (only when the row max grew by > 2^8), epilogue
-// While softmax_t works on S_t(j) the tensor core runs PV_{1-t}(j-1) and QK_{1-t}(j).
+// One CTA = one head x 256 query rows (two 128-row Q tiles), 384 threads:
+//   warp 0      TMA producer: Q tiles once, then K/V tiles through a shared-memory ring, in the order the
+//               tensor core consumes them (K_0, K_1, V_0, K_2, V_1, ...)
+//   warp 1      MMA issuer (one lane): S_t = Q_t K_j^T (SS, M=128, N=128) and O_t += P_t V_j (SS: P_t is read
+//               from SHARED memory, V_j MN-major)
+//   warp 2      TMEM allocator (512 columns: S_0, S_1 at 0/128, O_0, O_1 at 256/256+D)
+//   warps 4-7   softmax warpgroup of tile 0: one thread per query row; online softmax in fp32 with lazy
+//   warps 8-11  softmax warpgroup of tile 1   rescaling of O (only when the row max grew by > 2^8); epilogue
+//
+// Pipeline.  P_t goes through shared memory, not TMEM, so that S_t's TMEM columns are free as soon as the
+// softmax warpgroup has pulled S_t(j) into registers: the MMA warp issues QK_t(j+1) right then, and PV_t(j)
+// when P_t(j) has been stored.  The softmax chain (S(j) -> P(j) -> S(j+1) ...) therefore never waits for a
+// tensor-core round trip, and the tensor queue always holds the next GEMM (measured: the QK/PV instruction
+// mix runs at the full 8192 flop/clk/SM with P in shared memory, with or without concurrent P stores).
+// The exponentials are split between the MUFU pipe (ex2.approx) and a degree-3 polynomial on the FMA pipe
+// (packed f32x2 arithmetic), since 16 ex2/clk/SM would otherwise co-limit the kernel at exactly the MMA time.
 //
 // The KV iteration order per (head, query tile) is fixed (j = 0..ceil(S/128)-1) and does not depend
 // on how many heads a launch holds, so the output is bitwise independent of the chunking
 // (the paper's "max error 0" claim, L304 / Table 14).
 #include <cuda_bf16.h>
+
+#include <cstdlib>
 
 #include "hcms_internal.h"
 #include "ptx.cuh"
@@ -29,19 +40,21 @@ namespace {
 constexpr int kBM = 128;          // query rows per tile (UMMA M)
 constexpr int kBN = 128;          // keys per KV tile (UMMA N of QK^T, K extent of PV)
 constexpr int kQTiles = 2;        // Q tiles per CTA
-constexpr int kStages = 4;        // KV ring stages (each holds one K tile or one V tile)
 constexpr int kThreads = 384;
 constexpr int kTmemCols = 512;
 constexpr float kRescaleThreshold = 8.0f;  // log2 units: rescale O only if the max grew by > 2^8
+constexpr int kPanelBytes = 128 * 128;     // one 128-byte-swizzle panel: 128 rows x 128 B
+constexpr int kPTileBytes = 2 * kPanelBytes;  // P_t: 128 rows x 128 keys bf16
 
 template <int D>
 struct Cfg {
-  static constexpr int kPanels = D / 64;                 // 128-byte swizzle panels along D
-  static constexpr int kPanelBytes = 128 * 128;          // 128 rows x 128 B
+  static constexpr int kPanels = D / 64;                    // 128-byte swizzle panels along D
   static constexpr int kTileBytes = kPanels * kPanelBytes;  // one Q / K / V tile
-  static constexpr int kSmemBytes = (kQTiles + kStages) * kTileBytes + 1024 /*align*/ + 256 /*barriers*/;
-  static constexpr int kTmemS = 0;                       // S_t at kTmemS + t*128
-  static constexpr int kTmemO = 256;                     // O_t at kTmemO + t*D
+  static constexpr int kStages = D == 128 ? 3 : 6;          // KV ring stages (each holds one K tile or one V tile)
+  static constexpr int kSmemBytes =
+      kQTiles * kTileBytes + kQTiles * kPTileBytes + kStages * kTileBytes + 1024 /*align*/ + 256 /*barriers*/;
+  static constexpr int kTmemS = 0;                          // S_t at kTmemS + t*128
+  static constexpr int kTmemO = 256;                        // O_t at kTmemO + t*D
 };
 
 // Shared-memory matrix descriptor, 128-byte swizzle (cute::UMMA::SmemDescriptor bit layout):
@@ -54,6 +67,15 @@ __device__ __forceinline__ uint64_t make_desc(uint32_t smem_addr, uint32_t lbo_b
   d |= 1ull << 46;
   d |= 2ull << 61;
   return d;
+}
+
+// The same descriptor as two 32-bit words: the high word is a constant, so per-MMA address stepping is one
+// 32-bit add on the low word (shared-memory addresses are < 2^18, the start field never carries).
+__host__ __device__ constexpr uint32_t desc_hi(uint32_t sbo_bytes) {
+  return ((sbo_bytes >> 4) & 0x3FFF) | (1u << 14) | (2u << 29);
+}
+__device__ __forceinline__ uint32_t desc_lo(uint32_t smem_addr, uint32_t lbo_bytes) {
+  return ((smem_addr >> 4) & 0x3FFF) | (((lbo_bytes >> 4) & 0x3FFF) << 16);
 }
 
 // Instruction descriptor for kind::f16: fp32 accumulate, bf16 A and B.
@@ -73,30 +95,102 @@ struct AttnParams {
   float scale_log2;  // scale * log2(e)
 };
 
+// ---- packed fp32x2 arithmetic (FFMA2 / FADD2 on sm_100) and helpers ----------------------------------
+__device__ __forceinline__ uint64_t pack2(float lo, float hi) {
+  uint64_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void unpack2(uint64_t v, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c) {
+  uint64_t d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
+}
+__device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b) {
+  uint64_t d;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+__device__ __forceinline__ uint64_t add2_rm(uint64_t a, uint64_t b) {
+  uint64_t d;
+  asm("add.rm.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+__device__ __forceinline__ uint64_t sub2(uint64_t a, uint64_t b) {
+  uint64_t d;
+  asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+__device__ __forceinline__ float max3(float a, float b, float c) {
+  float d;
+  asm("max.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c));
+  return d;
+}
 __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
-  __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
-  return *reinterpret_cast<uint32_t*>(&v);
+  uint32_t r;
+  asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+  return r;
 }
 
-template <int D>
+// 2^x for a pair on the FMA pipe: x = n + f (n = floor x via the 1.5*2^23 round-down trick), 2^f by a
+// degree-3 polynomial with p(0) = 1 (max relative error 8.6e-5, far below P's bf16 rounding 2^-9), and
+// n added into the exponent field.  x is clamped to >= -126 so that the exponent never underflows.
+struct PolyConsts {
+  uint64_t magic, c1, c2, c3, one;
+};
+__device__ __forceinline__ PolyConsts poly_consts() {
+  PolyConsts c;
+  c.magic = pack2(12582912.f, 12582912.f);
+  c.c1 = pack2(0.6951168179512024f, 0.6951168179512024f);
+  c.c2 = pack2(0.22764474153518677f, 0.22764474153518677f);
+  c.c3 = pack2(0.07706727087497711f, 0.07706727087497711f);
+  c.one = pack2(1.0f, 1.0f);
+  return c;
+}
+__device__ __forceinline__ uint64_t exp2_poly2(float x0, float x1, const PolyConsts& c) {
+  const uint64_t x = pack2(fmaxf(x0, -126.f), fmaxf(x1, -126.f));
+  const uint64_t t = add2_rm(x, c.magic);
+  const uint64_t f = sub2(x, sub2(t, c.magic));
+  uint64_t p = fma2(f, c.c3, c.c2);
+  p = fma2(p, f, c.c1);
+  p = fma2(p, f, c.one);
+  float p0, p1, t0, t1;
+  unpack2(p, p0, p1);
+  unpack2(t, t0, t1);
+  p0 = __uint_as_float(__float_as_uint(p0) + (__float_as_uint(t0) << 23));
+  p1 = __uint_as_float(__float_as_uint(p1) + (__float_as_uint(t1) << 23));
+  return pack2(p0, p1);
+}
+
+__device__ __forceinline__ void st_shared_v4(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+  asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
+
+// kPoly: of every 8 consecutive column pairs, this many take the polynomial path (the rest MUFU).
+template <int D, int kPoly>
 __global__ void __launch_bounds__(kThreads, 1)
 attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm) {
   using C = Cfg<D>;
+  constexpr int kStages = C::kStages;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-  const uint32_t q_smem = smem_base;                                  // kQTiles tiles
-  const uint32_t kv_smem = smem_base + kQTiles * C::kTileBytes;       // kStages tiles
+  const uint32_t q_smem = smem_base;                                  // kQTiles Q tiles
+  const uint32_t p_smem = q_smem + kQTiles * C::kTileBytes;           // kQTiles P tiles
+  const uint32_t kv_smem = p_smem + kQTiles * kPTileBytes;            // kStages K/V tiles
   const uint32_t bar_base = kv_smem + kStages * C::kTileBytes;        // 8-byte barriers
-  // barrier indices
-  const uint32_t bar_q_full = bar_base;                // [2]
-  const uint32_t bar_kv_full = bar_base + 16;          // [kStages]
-  const uint32_t bar_kv_empty = bar_kv_full + 8 * kStages;
-  const uint32_t bar_s_full = bar_kv_empty + 8 * kStages;  // [2]
-  const uint32_t bar_p_full = bar_s_full + 16;             // [2]
-  const uint32_t bar_o_full = bar_p_full + 16;             // [2]
-  const uint32_t tmem_slot = bar_o_full + 16;              // 4 bytes
+  const uint32_t bar_q_full = bar_base;                       // [2]  TMA -> MMA
+  const uint32_t bar_kv_full = bar_q_full + 16;               // [kStages] TMA -> MMA
+  const uint32_t bar_kv_empty = bar_kv_full + 8 * kStages;    // [kStages] MMA -> TMA
+  const uint32_t bar_s_full = bar_kv_empty + 8 * kStages;     // [2]  MMA -> softmax: S_t(j) is in TMEM
+  const uint32_t bar_s_free = bar_s_full + 16;                // [2]  softmax -> MMA: S_t(j) is in registers
+  const uint32_t bar_p_full = bar_s_free + 16;                // [2]  softmax -> MMA: P_t(j) is in shared memory
+  const uint32_t bar_pv_done = bar_p_full + 16;               // [2]  MMA -> softmax: PV_t(j) has completed
+  const uint32_t tmem_slot = bar_pv_done + 16;                // 4 bytes
 
-  const int warp = threadIdx.x >> 5;
+  const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);   // warp-uniform by construction
   const int lane = threadIdx.x & 31;
   const int head = blockIdx.y;                 // p*h_c + j
   const int rank = head / prm.h_c;
@@ -108,8 +202,9 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
     for (int t = 0; t < kQTiles; ++t) {
       mbar_init(bar_q_full + 8 * t, 1);
       mbar_init(bar_s_full + 8 * t, 1);
-      mbar_init(bar_p_full + 8 * t, kBM);
-      mbar_init(bar_o_full + 8 * t, 1);
+      mbar_init(bar_s_free + 8 * t, 4);     // one elected lane per softmax warp
+      mbar_init(bar_p_full + 8 * t, 4);
+      mbar_init(bar_pv_done + 8 * t, 1);
     }
     for (int s = 0; s < kStages; ++s) {
       mbar_init(bar_kv_full + 8 * s, 1);
@@ -130,97 +225,129 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
 
   if (warp < 4) {
     // ================================ producer / MMA warpgroup ================================
+    // Both roles run warp-uniformly (all 32 lanes walk the loops and poll the barriers); only the TMA /
+    // tcgen05 instructions themselves are guarded by elect.sync.  A whole role under `lane == 0` makes
+    // ptxas wrap every uniform-datapath instruction in a divergence loop (~100 clk per MMA issue).
     setmaxnreg_dec<56>();
-    if (warp == 0 && lane == 0) {
+    if (warp == 0) {
       // ---------------- TMA producer ----------------
-      prefetch_tensormap(&maps.q);
-      prefetch_tensormap(&maps.k);
-      prefetch_tensormap(&maps.v);
+      const bool leader = elect_one();
+      if (leader) {
+        prefetch_tensormap(&maps.q);
+        prefetch_tensormap(&maps.k);
+        prefetch_tensormap(&maps.v);
+      }
       auto load_tile = [&](const CUtensorMap* tm, uint32_t dst, uint32_t bar, int row0) {
-        mbar_expect_tx(bar, C::kTileBytes);
+        if (leader) {
+          mbar_expect_tx(bar, C::kTileBytes);
 #pragma unroll
-        for (int pn = 0; pn < C::kPanels; ++pn)
-          tma_load_4d(dst + pn * C::kPanelBytes, tm, bar, pn * 64, hj, row0, rank);
+          for (int pn = 0; pn < C::kPanels; ++pn) tma_load_4d(dst + pn * kPanelBytes, tm, bar, pn * 64, hj, row0, rank);
+        }
+        __syncwarp();
+      };
+      int stage = 0;
+      uint32_t phase = 0;  // ring items are loaded in consumption order
+      auto load_kv = [&](const CUtensorMap* tm, int j) {
+        mbar_wait(bar_kv_empty + 8 * stage, phase ^ 1);
+        load_tile(tm, kv_smem + stage * C::kTileBytes, bar_kv_full + 8 * stage, j * kBN);
+        if (++stage == kStages) {
+          stage = 0;
+          phase ^= 1;
+        }
       };
       load_tile(&maps.q, q_smem, bar_q_full, q_row0);
-      int it = 0;  // ring item: K_j is item 2j, V_j is item 2j+1
+      load_kv(&maps.k, 0);
+      load_tile(&maps.q, q_smem + C::kTileBytes, bar_q_full + 8, q_row0 + kBM);
       for (int j = 0; j < n_kv; ++j) {
-#pragma unroll
-        for (int kv = 0; kv < 2; ++kv, ++it) {
-          const int stage = it % kStages;
-          const uint32_t round = it / kStages;
-          mbar_wait(bar_kv_empty + 8 * stage, (round & 1) ^ 1);
-          load_tile(kv == 0 ? &maps.k : &maps.v, kv_smem + stage * C::kTileBytes, bar_kv_full + 8 * stage,
-                    j * kBN);
-          if (it == 0) load_tile(&maps.q, q_smem + C::kTileBytes, bar_q_full + 8, q_row0 + kBM);
-        }
+        if (j + 1 < n_kv) load_kv(&maps.k, j + 1);
+        load_kv(&maps.v, j);
       }
-    } else if (warp == 1 && lane == 0) {
+    } else if (warp == 1) {
       // ---------------- MMA issuer ----------------
+      const bool leader = elect_one();
       constexpr uint32_t idesc_qk = make_idesc(kBM, kBN, false);
       constexpr uint32_t idesc_pv = make_idesc(kBM, D, true);
+      constexpr uint32_t hi = desc_hi(1024);                 // SBO = 1024 B for every operand
       auto issue_qk = [&](int t, uint32_t k_tile) {
         // S_t[128 x 128] = Q_t[128 x D] * K_j[128 x D]^T ; both operands K-major, 128B-swizzled panels
         const uint32_t d_tmem = tmem_base + C::kTmemS + t * kBN;
-        const uint32_t q_tile = q_smem + t * C::kTileBytes;
+        const uint32_t q_lo = desc_lo(q_smem + t * C::kTileBytes, 16);
+        const uint32_t k_lo = desc_lo(k_tile, 16);
 #pragma unroll
         for (int ks = 0; ks < D / 16; ++ks) {
-          const uint32_t off = (ks >> 2) * C::kPanelBytes + (ks & 3) * 32;
-          mma_ss(d_tmem, make_desc(q_tile + off, 16, 1024), make_desc(k_tile + off, 16, 1024), idesc_qk,
-                 ks > 0 ? 1u : 0u);
+          const uint32_t off = ((ks >> 2) * kPanelBytes + (ks & 3) * 32) >> 4;
+          mma_ss_lohi(d_tmem, q_lo + off, k_lo + off, hi, hi, idesc_qk, ks > 0 ? 1u : 0u);
         }
       };
       auto issue_pv = [&](int t, uint32_t v_tile, bool accumulate) {
-        // O_t[128 x D] += P_t[128 x 128 (TMEM, packed bf16)] * V_j[128 keys x D] ; B is MN-major:
-        // 64-wide D panels (LBO = panel stride), 8-key groups 1024 B apart (SBO)
+        // O_t[128 x D] += P_t[128 x 128 keys] * V_j[128 keys x D]; A = P_t K-major from shared memory (two
+        // 64-key panels), B = V_j MN-major: 64-wide D panels (LBO = panel stride), 8-key groups 1024 B apart
         const uint32_t d_tmem = tmem_base + C::kTmemO + t * D;
-        const uint32_t p_tmem = tmem_base + C::kTmemS + t * kBN;
+        const uint32_t p_lo = desc_lo(p_smem + t * kPTileBytes, 16);
+        const uint32_t v_lo = desc_lo(v_tile, kPanelBytes);
 #pragma unroll
         for (int ks = 0; ks < kBN / 16; ++ks) {
-          mma_ts(d_tmem, p_tmem + ks * 8, make_desc(v_tile + ks * 2048, C::kPanelBytes, 1024), idesc_pv,
-                 (accumulate || ks > 0) ? 1u : 0u);
+          const uint32_t off = ((ks >> 2) * kPanelBytes + (ks & 3) * 32) >> 4;
+          mma_ss_lohi(d_tmem, p_lo + off, v_lo + ks * (2048 >> 4), hi, hi, idesc_pv, (accumulate || ks > 0) ? 1u : 0u);
         }
       };
-      auto kv_wait = [&](int it) -> uint32_t {
-        const int stage = it % kStages;
-        mbar_wait(bar_kv_full + 8 * stage, (it / kStages) & 1);
+      int stage = 0;
+      uint32_t phase = 0;
+      auto kv_wait = [&]() -> uint32_t {
+        mbar_wait(bar_kv_full + 8 * stage, phase);
         return kv_smem + stage * C::kTileBytes;
       };
-      auto kv_release = [&](int it) { tc_commit(bar_kv_empty + 8 * (it % kStages)); };
+      auto kv_release = [&]() {
+        if (leader) tc_commit(bar_kv_empty + 8 * stage);
+        __syncwarp();
+        if (++stage == kStages) {
+          stage = 0;
+          phase ^= 1;
+        }
+      };
 
       // prologue: S_0(0), S_1(0)
       {
-        const uint32_t k_tile = kv_wait(0);
-        mbar_wait(bar_q_full, 0);
-        tc_fence_after();
-        issue_qk(0, k_tile);
-        tc_commit(bar_s_full);
-        mbar_wait(bar_q_full + 8, 0);
-        tc_fence_after();
-        issue_qk(1, k_tile);
-        tc_commit(bar_s_full + 8);
-        kv_release(0);
-      }
-      for (int j = 0; j < n_kv; ++j) {
-        const uint32_t v_tile = kv_wait(2 * j + 1);
-        uint32_t k_next = 0;
+        const uint32_t k_tile = kv_wait();
 #pragma unroll
         for (int t = 0; t < kQTiles; ++t) {
-          mbar_wait(bar_p_full + 8 * t, j & 1);   // P_t(j) written, O_t rescaled if needed
+          mbar_wait(bar_q_full + 8 * t, 0);
           tc_fence_after();
-          issue_pv(t, v_tile, j > 0);
-          tc_commit(bar_o_full + 8 * t);
-          if (t == kQTiles - 1) kv_release(2 * j + 1);
-          if (j + 1 < n_kv) {
-            if (t == 0) {
-              k_next = kv_wait(2 * j + 2);
-              tc_fence_after();
-            }
-            issue_qk(t, k_next);
+          if (leader) {
+            issue_qk(t, k_tile);
             tc_commit(bar_s_full + 8 * t);
-            if (t == kQTiles - 1) kv_release(2 * j + 2);
           }
+          __syncwarp();
         }
+        kv_release();
+      }
+      for (int j = 0; j < n_kv; ++j) {
+        if (j + 1 < n_kv) {
+          const uint32_t k_tile = kv_wait();
+#pragma unroll
+          for (int t = 0; t < kQTiles; ++t) {
+            mbar_wait(bar_s_free + 8 * t, j & 1);     // S_t(j) sits in the softmax registers
+            tc_fence_after();
+            if (leader) {
+              issue_qk(t, k_tile);
+              tc_commit(bar_s_full + 8 * t);
+            }
+            __syncwarp();
+          }
+          kv_release();
+        }
+        const uint32_t v_tile = kv_wait();
+#pragma unroll
+        for (int t = 0; t < kQTiles; ++t) {
+          mbar_wait(bar_p_full + 8 * t, j & 1);       // P_t(j) stored, O_t rescaled if needed
+          tc_fence_after();
+          if (leader) {
+            issue_pv(t, v_tile, j > 0);
+            tc_commit(bar_pv_done + 8 * t);
+          }
+          __syncwarp();
+        }
+        kv_release();
       }
     }
     __syncwarp();
@@ -232,11 +359,15 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
     const uint32_t lane_addr = static_cast<uint32_t>((warp & 3) * 32) << 16;
     const uint32_t s_tmem = tmem_base + lane_addr + C::kTmemS + t * kBN;
     const uint32_t o_tmem = tmem_base + lane_addr + C::kTmemO + t * D;
+    const uint32_t p_row = p_smem + t * kPTileBytes + row * 128;   // + panel*kPanelBytes + ((chunk ^ (row&7)) << 4)
+    const uint32_t swz = static_cast<uint32_t>(row & 7);
     const float scale_log2 = prm.scale_log2;
+    const uint64_t scale2 = pack2(scale_log2, scale_log2);
     const int tail_valid = prm.S - (n_kv - 1) * kBN;     // valid keys in the last KV tile (1..128)
+    const PolyConsts pc = poly_consts();
 
     float m_run = -INFINITY;   // running (possibly stale) row max, raw score units
-    float l_run = 0.f;         // running row sum of exp2((s - m_run)*scale_log2)
+    uint64_t l2 = pack2(0.f, 0.f), l2b = pack2(0.f, 0.f);   // running row sum, four partial lanes
 
     for (int j = 0; j < n_kv; ++j) {
       mbar_wait(bar_s_full + 8 * t, j & 1);
@@ -245,6 +376,9 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
 #pragma unroll
       for (int c4 = 0; c4 < kBN / 32; ++c4) tmem_ld32(s_tmem + c4 * 32, &sr[c4 * 32]);
       tmem_wait_ld();
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar_s_free + 8 * t);    // QK_t(j+1) may overwrite S_t now
       if (j == n_kv - 1 && tail_valid < kBN) {
 #pragma unroll
         for (int c = 0; c < kBN; ++c)
@@ -253,24 +387,26 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
       float mx0 = __uint_as_float(sr[0]), mx1 = __uint_as_float(sr[1]);
       float mx2 = __uint_as_float(sr[2]), mx3 = __uint_as_float(sr[3]);
 #pragma unroll
-      for (int c = 4; c < kBN; c += 4) {
-        mx0 = fmaxf(mx0, __uint_as_float(sr[c]));
-        mx1 = fmaxf(mx1, __uint_as_float(sr[c + 1]));
-        mx2 = fmaxf(mx2, __uint_as_float(sr[c + 2]));
-        mx3 = fmaxf(mx3, __uint_as_float(sr[c + 3]));
+      for (int c = 4; c < kBN; c += 8) {
+        mx0 = max3(mx0, __uint_as_float(sr[c]), __uint_as_float(sr[c + 1]));
+        mx1 = max3(mx1, __uint_as_float(sr[c + 2]), __uint_as_float(sr[c + 3]));
+        if (c + 4 < kBN) {
+          mx2 = max3(mx2, __uint_as_float(sr[c + 4]), __uint_as_float(sr[c + 5]));
+          mx3 = max3(mx3, __uint_as_float(sr[c + 6]), __uint_as_float(sr[c + 7]));
+        }
       }
-      const float m_tile = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
-      if (j == 0) {
-        m_run = m_tile;
-      } else {
+      const float m_tile = max3(mx0, mx1, fmaxf(mx2, mx3));
+      // PV_t(j-1) must have completed before P_t's buffer is rewritten (and before O_t is rescaled)
+      if (j > 0) {
+        mbar_wait(bar_pv_done + 8 * t, (j - 1) & 1);
         const bool need = (m_tile - m_run) * scale_log2 > kRescaleThreshold;
         if (__any_sync(0xffffffffu, need)) {
-          // O_t currently holds sum_k p_k V_k relative to m_run: wait for PV_t(j-1), then rescale
-          mbar_wait(bar_o_full + 8 * t, (j - 1) & 1);
+          // O_t holds sum_k p_k V_k relative to m_run: rescale it to the new max
           tc_fence_after();
           const float alpha = need ? ex2((m_run - m_tile) * scale_log2) : 1.0f;
           if (need) {
-            l_run *= alpha;
+            l2 = fma2(l2, pack2(alpha, alpha), pack2(0.f, 0.f));
+            l2b = fma2(l2b, pack2(alpha, alpha), pack2(0.f, 0.f));
             m_run = m_tile;
           }
 #pragma unroll
@@ -282,38 +418,53 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
             for (int c = 0; c < 32; ++c) orr[c] = __float_as_uint(__uint_as_float(orr[c]) * alpha);
             tmem_st32(o_tmem + c4 * 32, orr);
           }
+          tmem_wait_st();
+          tc_fence_before();
         }
+      } else {
+        m_run = m_tile;
       }
       const float neg_m = -m_run * scale_log2;
-      float sum0 = 0.f, sum1 = 0.f, sum2 = 0.f, sum3 = 0.f;
-      uint32_t pr[kBN / 2];
+      const uint64_t neg_m2 = pack2(neg_m, neg_m);
+      // 16 chunks of 8 keys: x = s*scale_log2 - m*scale_log2, p = 2^x, row sum in fp32, P rounded to bf16
 #pragma unroll
-      for (int c = 0; c < kBN; c += 4) {
-        const float p0 = ex2(fmaf(__uint_as_float(sr[c]), scale_log2, neg_m));
-        const float p1 = ex2(fmaf(__uint_as_float(sr[c + 1]), scale_log2, neg_m));
-        const float p2 = ex2(fmaf(__uint_as_float(sr[c + 2]), scale_log2, neg_m));
-        const float p3 = ex2(fmaf(__uint_as_float(sr[c + 3]), scale_log2, neg_m));
-        sum0 += p0;
-        sum1 += p1;
-        sum2 += p2;
-        sum3 += p3;
-        pr[c / 2] = pack_bf16(p0, p1);
-        pr[c / 2 + 1] = pack_bf16(p2, p3);
+      for (int ch = 0; ch < kBN / 8; ++ch) {
+        uint32_t w[4];
+#pragma unroll
+        for (int pr = 0; pr < 4; ++pr) {
+          const int c = ch * 8 + pr * 2;
+          const int pair = ch * 4 + pr;                 // 0..63
+          const uint64_t x = fma2(pack2(__uint_as_float(sr[c]), __uint_as_float(sr[c + 1])), scale2, neg_m2);
+          uint64_t p;
+          if ((pair & 7) < kPoly) {
+            float x0, x1;
+            unpack2(x, x0, x1);
+            p = exp2_poly2(x0, x1, pc);
+          } else {
+            float x0, x1;
+            unpack2(x, x0, x1);
+            p = pack2(ex2(x0), ex2(x1));
+          }
+          if (pr & 1) l2b = add2(l2b, p); else l2 = add2(l2, p);
+          float p0, p1;
+          unpack2(p, p0, p1);
+          w[pr] = pack_bf16(p0, p1);
+        }
+        st_shared_v4(p_row + (ch >> 3) * kPanelBytes + (((ch & 7) ^ swz) << 4), w[0], w[1], w[2], w[3]);
       }
-      l_run += (sum0 + sum1) + (sum2 + sum3);
-      // P_t aliases the first 64 columns of S_t (two bf16 per 32-bit column, element 2c in the low half)
-      tmem_st32(s_tmem, &pr[0]);
-      tmem_st32(s_tmem + 32, &pr[32]);
-      tmem_wait_st();
-      tc_fence_before();
-      mbar_arrive(bar_p_full + 8 * t);
+      fence_proxy_async_smem();     // generic-proxy stores -> visible to the tensor core's async-proxy reads
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar_p_full + 8 * t);
     }
 
-    // ---------------- epilogue: O_t / l -> bf16 -> swizzled smem (Q_t's buffer) -> TMA store ----------------
-    mbar_wait(bar_o_full + 8 * t, (n_kv - 1) & 1);
+    // ---------------- epilogue: O_t / l -> bf16 -> swizzled smem (P_t's buffer) -> TMA store ----------------
+    mbar_wait(bar_pv_done + 8 * t, (n_kv - 1) & 1);
     tc_fence_after();
-    const float inv_l = 1.0f / l_run;
-    const uint32_t o_smem = q_smem + t * C::kTileBytes;   // all QK_t MMAs have completed
+    float la, lb, lc, ld;
+    unpack2(l2, la, lb);
+    unpack2(l2b, lc, ld);
+    const float inv_l = 1.0f / ((la + lb) + (lc + ld));
+    const uint32_t o_smem = p_smem + t * kPTileBytes;     // PV_t(n_kv-1) has finished reading it
 #pragma unroll
     for (int c4 = 0; c4 < D / 32; ++c4) {
       uint32_t orr[32];
@@ -328,10 +479,7 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
           w[e] = pack_bf16(__uint_as_float(orr[q4 * 8 + 2 * e]) * inv_l,
                            __uint_as_float(orr[q4 * 8 + 2 * e + 1]) * inv_l);
         const uint32_t chunk = (c4 & 1) * 4 + q4;                  // 16-byte chunk inside the 128-byte row
-        const uint32_t addr = o_smem + panel * C::kPanelBytes + row * 128 + ((chunk ^ (row & 7)) << 4);
-        asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "r"(w[0]), "r"(w[1]), "r"(w[2]),
-                     "r"(w[3])
-                     : "memory");
+        st_shared_v4(o_smem + panel * kPanelBytes + row * 128 + ((chunk ^ swz) << 4), w[0], w[1], w[2], w[3]);
       }
     }
     fence_proxy_async_smem();
@@ -341,7 +489,7 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
       if (row0 < prm.S) {
 #pragma unroll
         for (int pn = 0; pn < C::kPanels; ++pn)
-          tma_store_4d(&maps.o, o_smem + pn * C::kPanelBytes, pn * 64, hj, row0, rank);
+          tma_store_4d(&maps.o, o_smem + pn * kPanelBytes, pn * 64, hj, row0, rank);
         bulk_commit();
         bulk_wait<0>();
       }
@@ -369,14 +517,45 @@ cudaError_t make_maps(const AttnArgs& a, AttnMaps* m) {
   return cudaSuccess;
 }
 
+using KernelFn = void (*)(const AttnMaps, const AttnParams);
+
+// Number of column pairs (of every 8) whose exponential runs on the FMA pipe.  The default was tuned on
+// B200 (profiles/); HCMS_ATTN_POLY=0..8 overrides it for tuning runs (read once).
+int poly_setting() {
+  static int v = -1;
+  if (v < 0) {
+    const char* e = std::getenv("HCMS_ATTN_POLY");
+    v = e ? std::atoi(e) : 3;
+    if (v < 0 || v > 8) v = 3;
+  }
+  return v;
+}
+
+template <int D>
+KernelFn pick_kernel(int poly) {
+  switch (poly) {
+    case 0: return attention_fwd_kernel<D, 0>;
+    case 1: return attention_fwd_kernel<D, 1>;
+    case 2: return attention_fwd_kernel<D, 2>;
+    case 4: return attention_fwd_kernel<D, 4>;
+    case 5: return attention_fwd_kernel<D, 5>;
+    case 6: return attention_fwd_kernel<D, 6>;
+    case 8: return attention_fwd_kernel<D, 8>;
+    default: return attention_fwd_kernel<D, 3>;
+  }
+}
+
 }  // namespace
 
 cudaError_t attention_init() {
-  cudaError_t e = cudaFuncSetAttribute(attention_fwd_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                       Cfg<128>::kSmemBytes);
-  if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(attention_fwd_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                              Cfg<64>::kSmemBytes);
+  for (int poly : {0, 1, 2, 3, 4, 5, 6, 8}) {
+    cudaError_t e = cudaFuncSetAttribute(pick_kernel<128>(poly), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         Cfg<128>::kSmemBytes);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(pick_kernel<64>(poly), cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg<64>::kSmemBytes);
+    if (e != cudaSuccess) return e;
+  }
+  return cudaSuccess;
 }
 
 cudaError_t launch_attention(const AttnArgs& a, cudaStream_t stream) {
@@ -391,10 +570,11 @@ cudaError_t launch_attention(const AttnArgs& a, cudaStream_t stream) {
   // masked tail keys while exp2(s*1e-30) is exactly 1 in fp32.
   prm.scale_log2 = fmaxf(a.scale * 1.4426950408889634f, 1e-30f);
   dim3 grid(static_cast<unsigned>((a.S + kQTiles * kBM - 1) / (kQTiles * kBM)), static_cast<unsigned>(a.P * a.h_c));
+  const int poly = poly_setting();
   if (a.D == 128)
-    attention_fwd_kernel<128><<<grid, kThreads, Cfg<128>::kSmemBytes, stream>>>(maps, prm);
+    pick_kernel<128>(poly)<<<grid, kThreads, Cfg<128>::kSmemBytes, stream>>>(maps, prm);
   else if (a.D == 64)
-    attention_fwd_kernel<64><<<grid, kThreads, Cfg<64>::kSmemBytes, stream>>>(maps, prm);
+    pick_kernel<64>(poly)<<<grid, kThreads, Cfg<64>::kSmemBytes, stream>>>(maps, prm);
   else
     return cudaErrorInvalidValue;
   return cudaGetLastError();
