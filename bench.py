@@ -53,6 +53,7 @@ def parse_args(argv=None):
     ap.add_argument("--chunks", type=int, default=0, help="override the workload's C")
     ap.add_argument("--impl", default="hcms", choices=["hcms", "reference"])
     ap.add_argument("--layout", default="vec", choices=["vec", "tma"])
+    ap.add_argument("--single-comp", action="store_true", help="HCMS_FLAG_SINGLE_COMP: one compute stream, as Alg. 1")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-rows", type=int, default=512, help="query rows per head in the cpu_baseline sample")
@@ -118,47 +119,62 @@ def aggregate_value(units_per_rank_step: float, steps: int, world: int, local_ms
 # ---------------------------------------------------------------------------------------------
 
 class ClockSampler:
-    QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
-             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
-             "clocks_event_reasons.sw_power_cap")
+    """SM clock, power and throttle reasons sampled every ~10 ms through NVML while the timed region runs
+    (B200_PROFILING.md's clocks line; NVML is what nvidia-smi reads, without a process spawn per sample)."""
 
     def __init__(self, gpu_index: int):
-        self.lines, self.proc = [], None
+        self.rows, self.stop_flag, self.err = [], False, None
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), f"--query-gpu={self.QUERY}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
-                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(self._physical_index(gpu_index))
+            self.smax = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
             self.thread = threading.Thread(target=self._pump, daemon=True)
             self.thread.start()
-        except OSError:
-            self.proc = None
+        except Exception as e:  # no NVML: report it, never fake a clock
+            self.err = repr(e)
+
+    @staticmethod
+    def _physical_index(local: int) -> int:
+        vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+        if vis:
+            ids = [v.strip() for v in vis.split(",") if v.strip()]
+            if local < len(ids) and ids[local].isdigit():
+                return int(ids[local])
+        return local
 
     def _pump(self):
-        for line in self.proc.stdout:
-            self.lines.append((time.time(), line.strip()))
+        nv = self.nv
+        while not self.stop_flag:
+            try:
+                self.rows.append((time.time(), nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM),
+                                  nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0,
+                                  nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)))
+            except Exception as e:
+                self.err = repr(e)
+                return
+            time.sleep(0.01)
 
     def mark(self):
         return time.time()
 
     def stop(self, t0: float, t1: float):
-        if self.proc is None:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.15)
-        self.proc.terminate()
-        sm, smax, power, reasons = [], [], [], set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        rows = [l for (t, l) in self.lines if t0 <= t <= t1 + 0.1] or [l for (_, l) in self.lines[-3:]]
-        for l in rows:
-            c = [x.strip() for x in l.split(",")]
-            try:
-                sm.append(float(c[0])); smax.append(float(c[1])); power.append(float(c[2]))
-            except (ValueError, IndexError):
-                continue
-            for n, v in zip(names, c[3:7]):
-                if v.lower().startswith("active"):
-                    reasons.add(n)
-        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(smax) if smax else None,
-                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+        if self.err and not self.rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["NVML unavailable: " + self.err]}
+        self.stop_flag = True
+        self.thread.join(timeout=1.0)
+        nv = self.nv
+        names = {"hw_slowdown": nv.nvmlClocksEventReasonHwSlowdown,
+                 "hw_thermal_slowdown": nv.nvmlClocksEventReasonHwThermalSlowdown,
+                 "sw_thermal_slowdown": nv.nvmlClocksEventReasonSwThermalSlowdown,
+                 "sw_power_cap": nv.nvmlClocksEventReasonSwPowerCap}
+        rows = [r for r in self.rows if t0 <= r[0] <= t1] or self.rows[-3:]
+        reasons = sorted(n for n, bit in names.items() if any(r[3] & bit for r in rows))
+        sm = [r[1] for r in rows]
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_min_mhz": min(sm) if sm else None,
+                "sm_max_mhz": self.smax, "power_w_max": round(max(r[2] for r in rows), 1) if rows else None,
+                "samples": len(rows), "reasons": reasons}
 
 
 # ---------------------------------------------------------------------------------------------
@@ -222,7 +238,8 @@ def run_hcms(args):
     tensor_bytes = S * Hh * D * 2
     flush = 3 * tensor_bytes < 2 * L2_BYTES
     flush_buf = torch.empty(2 * L2_BYTES, dtype=torch.uint8, device=dev) if flush else None
-    base_flags = H.HCMS_FLAG_PROFILE | (H.HCMS_FLAG_LAYOUT_TMA if args.layout == "tma" else 0)
+    base_flags = (H.HCMS_FLAG_PROFILE | (H.HCMS_FLAG_LAYOUT_TMA if args.layout == "tma" else 0) |
+                  (H.HCMS_FLAG_SINGLE_COMP if args.single_comp else 0))
     stream = torch.cuda.current_stream()
 
     def timed(plan, steps, fn):
@@ -243,6 +260,12 @@ def run_hcms(args):
         e1.record(stream)
         e1.synchronize()
         return e0.elapsed_time(e1)
+
+    def attn_span(plan, steps):
+        """Mean per-step attention time: begin of chunk 0's launch to the end of the last one (launches of
+        consecutive chunks overlap on the two alternating compute streams, so durations must not be summed)."""
+        n = min(steps, H.HCMS_PROFILE_RING)
+        return sum(H.hcms_plan_step_span(plan, back, 1) for back in range(n)) / n
 
     def kernel_times(plan, steps):
         """Mean per-step (scatter, attention, gather) device ms per chunk over the last `steps` calls."""
@@ -271,7 +294,7 @@ def run_hcms(args):
     value_per_s, ms_per_step = aggregate_value(flop_step, args.steps, world, ms_total, True)
     _, h_c = H.hcms_chunk_table(plan)
     attn_flop = [4.0 * S * S * D * P * h for h in h_c]
-    attn_ms = float(kt[1].sum())
+    attn_ms = attn_span(plan, args.steps)
     achieved = sum(attn_flop) / (attn_ms * 1e-3) / 1e12
     peak_tf = pk["bf16_tflops_sustained"]
     result = {
@@ -281,6 +304,7 @@ def run_hcms(args):
         "config": {"workload": f"BASELINE.json configs[{args.config - 1}] ({w.name}): S={S} H={Hh} D={D} "
                                f"P={P} C={C} chunks={h_c} non-causal scale=1/sqrt(D)",
                    "S": S, "H": Hh, "D": D, "P": P, "C": C, "layout_kernel": args.layout,
+                   "compute_streams": 1 if args.single_comp else 2,
                    "l2": "flushed between steps" if flush else "inputs larger than L2 (3 x %d MB)" % (tensor_bytes >> 20),
                    "multi_gpu": "replicas only" if world > 1 else "single GPU",
                    "inputs": "hcms_inputs counter-based N(0,1) -> bf16 (seed %d)" % w.seed},

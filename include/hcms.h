@@ -81,6 +81,12 @@ enum {
                                           and gather of hcms_attention_forward, each on the stream it runs on;
                                           read them with hcms_plan_timings */
 
+#define HCMS_FLAG_SINGLE_COMP 0x400u   /* issue every attention launch on ONE compute stream, literally as
+                                          Alg. 1 does.  Default: S_comp is realised as two CUDA streams that
+                                          alternate by chunk parity, so that chunk c+1's thread blocks fill
+                                          the SMs vacated by the last (partial) wave of chunk c; the event
+                                          dependencies of Eq. 6-7 are unchanged and so are the bits. */
+
 typedef struct hcms_plan hcms_plan_t;
 
 /* ---- introspection (host only, no GPU needed) ---------------------------------------- */
@@ -207,6 +213,14 @@ int hcms_plan_last_launch_count(const hcms_plan_t* plan);
  */
 #define HCMS_PROFILE_RING 64
 int hcms_plan_timings(hcms_plan_t* plan, int calls_back, float* scatter_ms, float* attn_ms, float* gather_ms);
+/*
+ * Same events, read as a span: *span_ms = time from the begin event of chunk 0 to the end event of chunk
+ * C-1 of step kind `step` (0 = scatter, 1 = attention, 2 = gather) in that call.  Attention launches of
+ * consecutive chunks may overlap (two alternating compute streams), so the attention time of a layer is
+ * this span, not the sum of hcms_plan_timings' attn_ms.  SYNCHRONISES the host with those events.
+ * Errors: as hcms_plan_timings, plus INVALID_ARG for step outside 0..2 or NULL span_ms.
+ */
+int hcms_plan_step_span(hcms_plan_t* plan, int calls_back, int step, float* span_ms);
 
 #ifdef __cplusplus
 }

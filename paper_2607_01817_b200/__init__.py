@@ -40,6 +40,7 @@ HCMS_FLAG_HOST_ROUTE_V = 0x40
 HCMS_FLAG_HOST_ROUTE_O = 0x80
 HCMS_FLAG_DEBUG_NO_COMM_WAIT = 0x100
 HCMS_FLAG_PROFILE = 0x200
+HCMS_FLAG_SINGLE_COMP = 0x400
 
 # every symbol include/hcms.h declares: name -> (restype, argtypes)
 _SIGNATURES = {
@@ -65,6 +66,7 @@ _SIGNATURES = {
     "hcms_attention_chunk": (c_int, [c_void_p] * 5 + [c_int, c_float, c_void_p]),
     "hcms_plan_last_launch_count": (c_int, [c_void_p]),
     "hcms_plan_timings": (c_int, [c_void_p, c_int, POINTER(c_float), POINTER(c_float), POINTER(c_float)]),
+    "hcms_plan_step_span": (c_int, [c_void_p, c_int, c_int, POINTER(c_float)]),
 }
 
 
@@ -249,6 +251,13 @@ def hcms_plan_timings(plan: Plan, calls_back: int = 0):
     arrs = [(c_float * plan.C)() for _ in range(3)]
     _check(lib.hcms_plan_timings(plan.handle, calls_back, *arrs), "hcms_plan_timings")
     return tuple(list(a) for a in arrs)
+
+
+def hcms_plan_step_span(plan: Plan, calls_back: int = 0, step: int = 1) -> float:
+    """-> ms from chunk 0's begin event to the last end event of step kind ``step`` (0 scatter, 1 attention, 2 gather)."""
+    ms = c_float()
+    _check(lib.hcms_plan_step_span(plan.handle, calls_back, step, ctypes.byref(ms)), "hcms_plan_step_span")
+    return float(ms.value)
 
 
 # ---- the hot path ------------------------------------------------------------------------------

@@ -396,12 +396,11 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
         }
       }
       const float m_tile = max3(mx0, mx1, fmaxf(mx2, mx3));
-      // PV_t(j-1) must have completed before P_t's buffer is rewritten (and before O_t is rescaled)
       if (j > 0) {
-        mbar_wait(bar_pv_done + 8 * t, (j - 1) & 1);
         const bool need = (m_tile - m_run) * scale_log2 > kRescaleThreshold;
         if (__any_sync(0xffffffffu, need)) {
-          // O_t holds sum_k p_k V_k relative to m_run: rescale it to the new max
+          // O_t holds sum_k p_k V_k relative to m_run: once PV_t(j-1) has landed, rescale it to the new max
+          mbar_wait(bar_pv_done + 8 * t, (j - 1) & 1);
           tc_fence_after();
           const float alpha = need ? ex2((m_run - m_tile) * scale_log2) : 1.0f;
           if (need) {
@@ -426,7 +425,11 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
       }
       const float neg_m = -m_run * scale_log2;
       const uint64_t neg_m2 = pack2(neg_m, neg_m);
-      // 16 chunks of 8 keys: x = s*scale_log2 - m*scale_log2, p = 2^x, row sum in fp32, P rounded to bf16
+      // 16 chunks of 8 keys: x = s*scale_log2 - m*scale_log2, p = 2^x, row sum in fp32, P rounded to bf16.
+      // The first kHold chunks stay in registers: P_t's buffer may only be rewritten once PV_t(j-1) has
+      // completed, and by the time they are done that wait has normally been satisfied already.
+      constexpr int kHold = 8;
+      uint32_t held[kHold][4];
 #pragma unroll
       for (int ch = 0; ch < kBN / 8; ++ch) {
         uint32_t w[4];
@@ -435,22 +438,27 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
           const int c = ch * 8 + pr * 2;
           const int pair = ch * 4 + pr;                 // 0..63
           const uint64_t x = fma2(pack2(__uint_as_float(sr[c]), __uint_as_float(sr[c + 1])), scale2, neg_m2);
-          uint64_t p;
-          if ((pair & 7) < kPoly) {
-            float x0, x1;
-            unpack2(x, x0, x1);
-            p = exp2_poly2(x0, x1, pc);
-          } else {
-            float x0, x1;
-            unpack2(x, x0, x1);
-            p = pack2(ex2(x0), ex2(x1));
-          }
+          float x0, x1;
+          unpack2(x, x0, x1);
+          const uint64_t p = (pair & 7) < kPoly ? exp2_poly2(x0, x1, pc) : pack2(ex2(x0), ex2(x1));
           if (pr & 1) l2b = add2(l2b, p); else l2 = add2(l2, p);
           float p0, p1;
           unpack2(p, p0, p1);
           w[pr] = pack_bf16(p0, p1);
         }
-        st_shared_v4(p_row + (ch >> 3) * kPanelBytes + (((ch & 7) ^ swz) << 4), w[0], w[1], w[2], w[3]);
+        if (ch < kHold) {
+#pragma unroll
+          for (int e = 0; e < 4; ++e) held[ch][e] = w[e];
+        }
+        if (ch == kHold - 1) {
+          if (j > 0) mbar_wait(bar_pv_done + 8 * t, (j - 1) & 1);
+#pragma unroll
+          for (int h = 0; h < kHold; ++h)
+            st_shared_v4(p_row + (h >> 3) * kPanelBytes + (((h & 7) ^ swz) << 4), held[h][0], held[h][1], held[h][2],
+                         held[h][3]);
+        }
+        if (ch >= kHold)
+          st_shared_v4(p_row + (ch >> 3) * kPanelBytes + (((ch & 7) ^ swz) << 4), w[0], w[1], w[2], w[3]);
       }
       fence_proxy_async_smem();     // generic-proxy stores -> visible to the tensor core's async-proxy reads
       __syncwarp();

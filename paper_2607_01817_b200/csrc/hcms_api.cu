@@ -61,8 +61,8 @@ struct hcms_plan {
   size_t ws_bytes = 0;
   void* ws = nullptr;
   bool ws_owned = false;
-  cudaStream_t s_comm = nullptr, s_comm_out = nullptr, s_comp = nullptr;
-  cudaEvent_t e_main = nullptr, e_fin_comm = nullptr, e_fin_comp = nullptr, e_fin_in = nullptr;
+  cudaStream_t s_comm = nullptr, s_comm_out = nullptr, s_comp = nullptr, s_comp2 = nullptr;
+  cudaEvent_t e_main = nullptr, e_fin_comm = nullptr, e_fin_comp = nullptr, e_fin_comp2 = nullptr, e_fin_in = nullptr;
   std::vector<cudaEvent_t> e_comm, e_comp;
   // host route (config 5)
   void* pinned[4] = {nullptr, nullptr, nullptr, nullptr};
@@ -79,11 +79,13 @@ static void plan_free(hcms_plan_t* p) {
   if (p->s_comm) cudaStreamSynchronize(p->s_comm);
   if (p->s_comm_out) cudaStreamSynchronize(p->s_comm_out);
   if (p->s_comp) cudaStreamSynchronize(p->s_comp);
+  if (p->s_comp2) cudaStreamSynchronize(p->s_comp2);
   for (auto e : p->e_comm) cudaEventDestroy(e);
   for (auto e : p->e_comp) cudaEventDestroy(e);
   if (p->e_main) cudaEventDestroy(p->e_main);
   if (p->e_fin_comm) cudaEventDestroy(p->e_fin_comm);
   if (p->e_fin_comp) cudaEventDestroy(p->e_fin_comp);
+  if (p->e_fin_comp2) cudaEventDestroy(p->e_fin_comp2);
   if (p->e_fin_in) cudaEventDestroy(p->e_fin_in);
   for (auto& step : p->prof)
     for (auto& side : step)
@@ -92,6 +94,7 @@ static void plan_free(hcms_plan_t* p) {
   if (p->s_comm) cudaStreamDestroy(p->s_comm);
   if (p->s_comm_out) cudaStreamDestroy(p->s_comm_out);
   if (p->s_comp) cudaStreamDestroy(p->s_comp);
+  if (p->s_comp2) cudaStreamDestroy(p->s_comp2);
   if (p->ws_owned && p->ws) cudaFree(p->ws);
   for (auto& h : p->pinned)
     if (h) cudaFreeHost(h);
@@ -221,9 +224,11 @@ int hcms_plan(hcms_plan_t** out, int64_t S, int H, int D, int P, int C, int dtyp
   PLAN_CUDA(cudaStreamCreateWithPriority(&p->s_comm, cudaStreamNonBlocking, prio_hi));
   PLAN_CUDA(cudaStreamCreateWithPriority(&p->s_comm_out, cudaStreamNonBlocking, prio_hi));
   PLAN_CUDA(cudaStreamCreateWithPriority(&p->s_comp, cudaStreamNonBlocking, prio_lo));
+  PLAN_CUDA(cudaStreamCreateWithPriority(&p->s_comp2, cudaStreamNonBlocking, prio_lo));
   PLAN_CUDA(cudaEventCreateWithFlags(&p->e_main, cudaEventDisableTiming));
   PLAN_CUDA(cudaEventCreateWithFlags(&p->e_fin_comm, cudaEventDisableTiming));
   PLAN_CUDA(cudaEventCreateWithFlags(&p->e_fin_comp, cudaEventDisableTiming));
+  PLAN_CUDA(cudaEventCreateWithFlags(&p->e_fin_comp2, cudaEventDisableTiming));
   PLAN_CUDA(cudaEventCreateWithFlags(&p->e_fin_in, cudaEventDisableTiming));
   p->e_comm.assign(C, nullptr);
   p->e_comp.assign(C, nullptr);
@@ -268,6 +273,7 @@ int hcms_plan_set_workspace(hcms_plan_t* plan, void* dev, size_t bytes) {
     cudaStreamSynchronize(plan->s_comm);
     cudaStreamSynchronize(plan->s_comm_out);
     cudaStreamSynchronize(plan->s_comp);
+    cudaStreamSynchronize(plan->s_comp2);
     cudaFree(plan->ws);
   }
   plan->ws = dev;
@@ -410,7 +416,9 @@ int hcms_attention_forward(hcms_plan_t* plan, const void* q, const void* k, cons
   const bool split = (plan->flags & HCMS_FLAG_SPLIT_COMM) && !serial;
   cudaStream_t s_in = serial ? caller : plan->s_comm;
   cudaStream_t s_out = serial ? caller : (split ? plan->s_comm_out : plan->s_comm);
-  cudaStream_t s_comp = serial ? caller : plan->s_comp;
+  // S_comp: two CUDA streams alternating by chunk parity (see HCMS_FLAG_SINGLE_COMP in hcms.h)
+  const bool dual_comp = !serial && !(plan->flags & HCMS_FLAG_SINGLE_COMP) && sh.C > 1;
+  auto comp_stream = [&](int c) { return serial ? caller : ((dual_comp && (c & 1)) ? plan->s_comp2 : plan->s_comp); };
   char* ws = static_cast<char*>(plan->ws);
   plan->last_launches = 0;
 
@@ -432,7 +440,8 @@ int hcms_attention_forward(hcms_plan_t* plan, const void* q, const void* k, cons
   if (!serial) {
     HCMS_CUDA(cudaEventRecord(plan->e_main, caller));            // Alg. 1 line 5
     HCMS_CUDA(cudaStreamWaitEvent(s_in, plan->e_main, 0));       // line 7
-    HCMS_CUDA(cudaStreamWaitEvent(s_comp, plan->e_main, 0));     // line 13
+    HCMS_CUDA(cudaStreamWaitEvent(plan->s_comp, plan->e_main, 0));     // line 13
+    if (dual_comp) HCMS_CUDA(cudaStreamWaitEvent(plan->s_comp2, plan->e_main, 0));
     if (split) HCMS_CUDA(cudaStreamWaitEvent(s_out, plan->e_main, 0));
   }
   // Phase 1 -- input all-to-all of every chunk on S_comm (lines 8-11)
@@ -453,6 +462,7 @@ int hcms_attention_forward(hcms_plan_t* plan, const void* q, const void* k, cons
   // Phase 2 -- attention per chunk on S_comp (lines 14-18); Attn_c <- wait(E_c^comm)  (Eq. 6)
   for (int c = 0; c < sh.C; ++c) {
     const Chunk& ck = plan->chunks[c];
+    cudaStream_t s_comp = comp_stream(c);
     if (!serial && !(plan->flags & HCMS_FLAG_DEBUG_NO_COMM_WAIT))
       HCMS_CUDA(cudaStreamWaitEvent(s_comp, plan->e_comm[c], 0));
     HCMS_CUDA(mark(1, c, 0, s_comp));
@@ -478,9 +488,13 @@ int hcms_attention_forward(hcms_plan_t* plan, const void* q, const void* k, cons
   if (!serial) {
     // line 25: Synchronize(S_comm, S_comp) -- expressed as stream waits, the host is not blocked
     HCMS_CUDA(cudaEventRecord(plan->e_fin_comm, s_out));
-    HCMS_CUDA(cudaEventRecord(plan->e_fin_comp, s_comp));
+    HCMS_CUDA(cudaEventRecord(plan->e_fin_comp, plan->s_comp));
     HCMS_CUDA(cudaStreamWaitEvent(caller, plan->e_fin_comm, 0));
     HCMS_CUDA(cudaStreamWaitEvent(caller, plan->e_fin_comp, 0));
+    if (dual_comp) {
+      HCMS_CUDA(cudaEventRecord(plan->e_fin_comp2, plan->s_comp2));
+      HCMS_CUDA(cudaStreamWaitEvent(caller, plan->e_fin_comp2, 0));
+    }
     if (split) {
       HCMS_CUDA(cudaEventRecord(plan->e_fin_in, s_in));
       HCMS_CUDA(cudaStreamWaitEvent(caller, plan->e_fin_in, 0));
@@ -504,6 +518,26 @@ int hcms_plan_timings(hcms_plan_t* plan, int calls_back, float* scatter_ms, floa
       HCMS_CUDA(cudaEventElapsedTime(&ms, plan->prof[step][0][base + c], plan->prof[step][1][base + c]));
       if (outs[step]) outs[step][c] = ms;
     }
+  return HCMS_OK;
+}
+
+int hcms_plan_step_span(hcms_plan_t* plan, int calls_back, int step, float* span_ms) {
+  if (!plan || !span_ms) return fail(HCMS_ERR_INVALID_ARG, "plan or span_ms is NULL");
+  if (!(plan->flags & HCMS_FLAG_PROFILE)) return fail(HCMS_ERR_INVALID_ARG, "plan was made without HCMS_FLAG_PROFILE");
+  if (step < 0 || step > 2) return fail(HCMS_ERR_INVALID_ARG, "step=%d must be 0 (scatter), 1 (attention) or 2 (gather)", step);
+  if (calls_back < 0 || calls_back >= HCMS_PROFILE_RING || calls_back >= plan->prof_calls)
+    return fail(HCMS_ERR_INVALID_ARG, "calls_back=%d: %lld profiled calls so far, ring keeps %d", calls_back,
+                plan->prof_calls, HCMS_PROFILE_RING);
+  const size_t base = static_cast<size_t>((plan->prof_calls - 1 - calls_back) % HCMS_PROFILE_RING) * plan->sh.C;
+  // chunk 0 begins first and chunk C-1 ends last on every stream arrangement (in-order streams, Eq. 6-7 waits)
+  for (int c = 0; c < plan->sh.C; ++c) HCMS_CUDA(cudaEventSynchronize(plan->prof[step][1][base + c]));
+  float best = 0.f;
+  for (int c = 0; c < plan->sh.C; ++c) {
+    float ms = 0.f;
+    HCMS_CUDA(cudaEventElapsedTime(&ms, plan->prof[step][0][base], plan->prof[step][1][base + c]));
+    best = ms > best ? ms : best;
+  }
+  *span_ms = best;
   return HCMS_OK;
 }
 
