@@ -52,6 +52,11 @@ def parse_args(argv=None):
     ap.add_argument("--config", type=int, default=3, choices=sorted(I.WORKLOADS))
     ap.add_argument("--chunks", type=int, default=0, help="override the workload's C")
     ap.add_argument("--impl", default="hcms", choices=["hcms", "reference"])
+    ap.add_argument("--mode", default="bench", choices=["bench", "c-sweep", "rho-sweep", "timeline"],
+                    help="bench: the contract line (default).  c-sweep: every C in 1..H/P, Eq. 10 fit, C* (Table 7/12 "
+                         "analogue).  rho-sweep: host-routed all-to-all, speedup vs rho against 1/(1-rho) (Table 13 "
+                         "analogue; meant for --config 5).  timeline: per-chunk begin/end of scatter, attention, "
+                         "gather on their streams (Fig. 2 analogue)")
     ap.add_argument("--layout", default="vec", choices=["vec", "tma"])
     ap.add_argument("--single-comp", action="store_true", help="HCMS_FLAG_SINGLE_COMP: one compute stream, as Alg. 1")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -384,6 +389,149 @@ def run_hcms(args):
         dist.destroy_process_group()
 
 
+# ---------------------------------------------------------------------------------------------
+# measurement modes beyond the contract line (C sweep, rho sweep, timeline)
+# ---------------------------------------------------------------------------------------------
+
+class Session:
+    """Device-resident seeded inputs of one workload plus the timing helpers the sweep modes share."""
+
+    def __init__(self, args):
+        import torch
+        import paper_2607_01817_b200 as H
+        if not torch.cuda.is_available():
+            raise SystemExit("bench.py: no CUDA device; the HCMS hot path has no CPU fallback")
+        self.torch, self.H, self.args = torch, H, args
+        torch.cuda.set_device(0)
+        self.dev = torch.device("cuda", 0)
+        self.w = w = I.workload(args.config)
+        q, k, v = I.make_qkv(w, threads=os.cpu_count() or 8)
+        if w.dtype == "f32":
+            q, k, v = (I.f32_to_bf16_bits(t) for t in (q, k, v))
+        self.q, self.k, self.v = (torch.from_numpy(t.view(np.int16)).to(self.dev) for t in (q, k, v))
+        self.out = torch.empty_like(self.q)
+        self.flop = 4.0 * w.S * w.S * w.D * w.H
+        self.stream = torch.cuda.current_stream()
+        torch.cuda.synchronize()
+
+    def plan(self, C, flags):
+        w, H = self.w, self.H
+        return H.hcms_plan(w.S, w.H, w.D, w.P, C, H.HCMS_DTYPE_BF16, flags | H.HCMS_FLAG_PROFILE)
+
+    def time_plan(self, plan, steps, warmup=1):
+        """-> (ms per call, mean per-chunk [scatter, attention, gather] ms over the timed calls)."""
+        torch, H = self.torch, self.H
+        fn = lambda: H.hcms_attention_forward(plan, self.q, self.k, self.v, self.out, self.w.scale)
+        for _ in range(warmup):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(self.stream)
+        for _ in range(steps):
+            fn()
+        e1.record(self.stream)
+        e1.synchronize()
+        n = min(steps, H.HCMS_PROFILE_RING)
+        kt = sum(np.asarray(H.hcms_plan_timings(plan, b)) for b in range(n)) / n
+        return e0.elapsed_time(e1) / steps, kt
+
+
+def run_c_sweep(args):
+    """Table 7 / Table 12 analogue: layer time for every C, Eq. 10 fit of beta, C* predicted vs measured."""
+    ss = Session(args)
+    H, w = ss.H, ss.w
+    Hl = w.H // w.P
+    steps = max(3, min(args.steps, 10))
+    rows = []
+    for C in range(1, Hl + 1):
+        with ss.plan(C, 0) as pl:
+            ms, _ = ss.time_plan(pl, steps)
+            _, h_c = H.hcms_chunk_table(pl)
+        with ss.plan(C, H.HCMS_FLAG_SERIAL) as pl:
+            ms_ser, kt = ss.time_plan(pl, steps)
+        rows.append({"C": C, "chunks": h_c, "hcms_ms": round(ms, 4), "serial_ms": round(ms_ser, 4),
+                     "copy_solo_ms": round(float(kt[0].sum() + kt[2].sum()), 4),
+                     "attn_solo_ms": round(float(kt[1].sum()), 4), "tflops": round(ss.flop / ms / 1e9, 1)})
+    t_comm = rows[0]["copy_solo_ms"]
+    # Eq. 10 with the measured T_comm: T(C) - T_comm/C = a + beta*C  (least squares over C = 1..Hl)
+    Cs = np.array([r["C"] for r in rows], dtype=np.float64)
+    y = np.array([r["hcms_ms"] for r in rows]) - t_comm / Cs
+    beta, a = (np.polyfit(Cs, y, 1) if len(rows) > 1 else (0.0, y[0]))
+    best = min(rows, key=lambda r: r["hcms_ms"])
+    auto_C, auto_ms = H.hcms_autotune_chunks(w.S, w.H, w.D, w.P, H.HCMS_DTYPE_BF16, 0, ss.q, ss.k, ss.v, ss.out,
+                                             w.scale, Hl, 3)
+    print(json.dumps({
+        "mode": "c-sweep", "config": {"workload": w.name, "S": w.S, "H": w.H, "D": w.D, "P": w.P, "heads_per_rank": Hl},
+        "steps": steps, "rows": rows, "t_comm_ms": t_comm, "rho": round(t_comm / rows[0]["serial_ms"], 4),
+        "fit": {"model": "Eq. 10: T(C) = a + T_comm/C + beta*C", "a_ms": round(float(a), 4), "beta_ms": round(float(beta), 5),
+                "c_star": (round(H.hcms_model_c_star(t_comm, float(beta)), 2) if beta > 0 else None),
+                "choose_chunks": H.hcms_model_choose_chunks(Hl, t_comm, float(beta))},
+        "measured_best_C": best["C"], "autotune": {"best_C": auto_C, "ms": [round(m, 4) for m in auto_ms]},
+        "speedup_best_vs_serial_C1": round(rows[0]["serial_ms"] / best["hcms_ms"], 4),
+        "s_max_bound": round(H.hcms_model_s_max(t_comm / rows[0]["serial_ms"]), 4)}), flush=True)
+
+
+def run_rho_sweep(args):
+    """Table 13 analogue: route 0..4 of the chunk tensors through pinned host memory (the emulated wire of
+    BASELINE.json configs[4]) and compare the measured speedup with Theorem 2's 1/(1-rho) and Eq. 11."""
+    ss = Session(args)
+    H, w = ss.H, ss.w
+    C = args.chunks or w.C
+    steps = max(2, min(args.steps, 5))
+    Q, K, V, O = H.HCMS_FLAG_HOST_ROUTE_Q, H.HCMS_FLAG_HOST_ROUTE_K, H.HCMS_FLAG_HOST_ROUTE_V, H.HCMS_FLAG_HOST_ROUTE_O
+    rows = []
+    for name, mask in [("none", 0), ("O", O), ("Q,O", Q | O), ("Q,K,O", Q | K | O), ("Q,K,V,O", Q | K | V | O)]:
+        with ss.plan(C, mask | H.HCMS_FLAG_SERIAL) as pl:
+            ser, kt = ss.time_plan(pl, steps)
+        t_comm = float(kt[0].sum() + kt[2].sum())
+        with ss.plan(C, mask) as pl:
+            one, _ = ss.time_plan(pl, steps)
+        with ss.plan(C, mask | H.HCMS_FLAG_SPLIT_COMM) as pl:
+            split, _ = ss.time_plan(pl, steps)
+        rho = t_comm / ser
+        rows.append({"host_routed": name, "serial_ms": round(ser, 3), "t_comm_ms": round(t_comm, 3),
+                     "t_attn_ms": round(float(kt[1].sum()), 3), "rho": round(rho, 4),
+                     "hcms_ms": round(one, 3), "speedup": round(ser / one, 4),
+                     "hcms_split_comm_ms": round(split, 3), "speedup_split_comm": round(ser / split, 4),
+                     "eq11_beta0": round(H.hcms_model_speedup(C, rho, 0.0, ser), 4),
+                     "s_max_1_over_1_minus_rho": round(H.hcms_model_s_max(rho), 4),
+                     "exposed_bound_ms": round(float(kt[1].sum() + kt[0][0] + kt[2][-1]), 3)})
+    print(json.dumps({"mode": "rho-sweep", "C": C, "steps": steps,
+                      "config": {"workload": w.name, "S": w.S, "H": w.H, "D": w.D, "P": w.P},
+                      "note": "rho = T_comm/T_serial with T_comm = sum of scatter+gather incl. D2H+H2D hops (Eq. 1); "
+                              "exposed_bound = T_attn + scatter_0 + gather_{C-1}, the floor of any C-chunk pipeline",
+                      "rows": rows}), flush=True)
+
+
+def run_timeline(args):
+    """Fig. 2 analogue: begin/end of every scatter, attention and gather of one HCMS call, from the CUDA
+    events HCMS_FLAG_PROFILE records on the streams the steps run on (nsys is not installed)."""
+    ss = Session(args)
+    H, w = ss.H, ss.w
+    C = args.chunks or w.C
+    flags = (H.HCMS_FLAG_SINGLE_COMP if args.single_comp else 0)
+    with ss.plan(C, flags) as pl:
+        ms, _ = ss.time_plan(pl, 3, warmup=2)
+        b, e = H.hcms_plan_timeline(pl, 0)
+    names = ["scatter", "attention", "gather"]
+    ops = [{"op": names[kind], "chunk": c, "stream": ("S_comm" if kind != 1 else ("S_comp" if args.single_comp or c % 2 == 0 else "S_comp'")),
+            "begin_ms": round(b[kind][c], 4), "end_ms": round(e[kind][c], 4)} for kind in range(3) for c in range(C)]
+    ops.sort(key=lambda o: o["begin_ms"])
+    span = max(o["end_ms"] for o in ops)
+    width = 100
+    for o in ops:
+        x0, x1 = int(o["begin_ms"] / span * width), max(int(o["end_ms"] / span * width), int(o["begin_ms"] / span * width) + 1)
+        print(f'{o["op"]:>9s}[{o["chunk"]}] {o["stream"]:<7s} |' + " " * x0 + "#" * (x1 - x0) + " " * (width - x1) +
+              f'| {o["begin_ms"]:8.3f} -> {o["end_ms"]:8.3f} ms', file=sys.stderr)
+    comm_busy = sum(o["end_ms"] - o["begin_ms"] for o in ops if o["op"] != "attention")
+    hidden = sum(max(0.0, min(o["end_ms"], a["end_ms"]) - max(o["begin_ms"], a["begin_ms"]))
+                 for o in ops if o["op"] != "attention" for a in ops if a["op"] == "attention")
+    print(json.dumps({"mode": "timeline", "C": C, "ms_per_call": round(ms, 4), "span_ms": round(span, 4),
+                      "config": {"workload": w.name, "S": w.S, "H": w.H, "D": w.D, "P": w.P},
+                      "comm_ms": round(comm_busy, 4), "comm_ms_overlapped_with_attention": round(min(hidden, comm_busy), 4),
+                      "ops": ops}), flush=True)
+
+
 # dram__bytes_read.sum + dram__bytes_write.sum per attention launch summed over one step, from the
 # ncu --set full capture committed under profiles/ (bytes; None until captured for that config)
 ATTN_TRAFFIC = {}
@@ -427,6 +575,12 @@ def main(argv=None):
     args = parse_args(argv)
     if args.impl == "reference":
         run_reference(args)
+    elif args.mode == "c-sweep":
+        run_c_sweep(args)
+    elif args.mode == "rho-sweep":
+        run_rho_sweep(args)
+    elif args.mode == "timeline":
+        run_timeline(args)
     else:
         run_hcms(args)
 

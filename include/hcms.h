@@ -113,6 +113,15 @@ double hcms_model_t_hcms(int C, double t0, double t_comm, double t_attn, double 
 double hcms_model_c_star(double t_comm, double beta);
 double hcms_model_speedup(int C, double rho, double beta, double t_total);
 double hcms_model_s_max(double rho);
+/*
+ * Integer chunk count from the model (adaptive C, the paper's future work L346, via Theorem 1):
+ * the C in [1, heads_per_rank] that minimises Eq. 10's C-dependent part  t_comm/C + C*beta.  That
+ * function is convex in C, so the minimiser is floor(C*) or ceil(C*), C* = sqrt(t_comm/beta), clamped
+ * to the range; ties go to the smaller C (fewer launches).  beta <= 0 (no per-chunk overhead) returns
+ * heads_per_rank; t_comm <= 0 returns 1.  Returns 0 if heads_per_rank <= 0 or an argument is NaN.
+ * Worked pin: Table 12 row 1 (L440): t_comm = 0.396*73.3 ms, beta = 1.41 ms, 5 heads per rank -> 5.
+ */
+int hcms_model_choose_chunks(int heads_per_rank, double t_comm, double beta);
 
 /* ---- plan ------------------------------------------------------------------------------ */
 /*
@@ -221,6 +230,28 @@ int hcms_plan_timings(hcms_plan_t* plan, int calls_back, float* scatter_ms, floa
  * Errors: as hcms_plan_timings, plus INVALID_ARG for step outside 0..2 or NULL span_ms.
  */
 int hcms_plan_step_span(hcms_plan_t* plan, int calls_back, int step, float* span_ms);
+/*
+ * Same events, read as a timeline (the measured counterpart of Fig. 2): begin_ms[k*C + c] and
+ * end_ms[k*C + c] are the begin / end of step kind k (0 = scatter, 1 = attention, 2 = gather) of chunk c,
+ * in milliseconds after the begin event of chunk 0's scatter.  Host arrays of 3*C floats each.
+ * SYNCHRONISES the host with those events.  Errors: as hcms_plan_timings, plus INVALID_ARG for NULL arrays.
+ */
+int hcms_plan_timeline(hcms_plan_t* plan, int calls_back, float* begin_ms, float* end_ms);
+
+/* ---- adaptive chunk count (the paper's future work, L346) ------------------- */
+/*
+ * Measure hcms_attention_forward for every C in [1, min(max_C, H/P)] on the caller's tensors and
+ * report the fastest: for each C a temporary plan (flags = `flags` without SERIAL/PROFILE) runs one
+ * warm-up and `reps` timed calls between two CUDA events on `stream`; ms_per_call[C-1] = mean time
+ * of a call (host array of max_C floats, may be NULL; entries beyond H/P are set to -1), *best_C = the
+ * argmin (ties to the smaller C).  q,k,v,out as for hcms_attention_forward; `out` holds the result of
+ * the last measured call (identical bits for every C).  SYNCHRONISES the host; allocates and frees one
+ * workspace per C.  Errors: INVALID_ARG (NULL, max_C < 1, reps < 1), those of hcms_plan and of
+ * hcms_attention_forward.
+ */
+int hcms_autotune_chunks(int64_t S, int H, int D, int P, int dtype, uint32_t flags, const void* q, const void* k,
+                         const void* v, void* out, float scale, void* stream, int max_C, int reps, int* best_C,
+                         float* ms_per_call);
 
 #ifdef __cplusplus
 }

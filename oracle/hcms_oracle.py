@@ -232,3 +232,15 @@ def speedup(C: int, rho: float, beta: float, t_total: float) -> float:
 def s_max(rho: float) -> float:
     """Theorem 2 (L158, L429): ``S_max = 1 / (1 - rho)``."""
     return 1.0 / (1.0 - rho)
+
+
+def choose_chunks(heads_per_rank: int, t_comm: float, beta: float) -> int:
+    """Adaptive C (future work L346) by brute force over Eq. 10: the integer ``C`` in
+    ``[1, heads_per_rank]`` with the smallest ``T_hcms(C)`` (T_0, T_attn do not depend on C),
+    ties to the smaller C.  Theorem 1 says this is a neighbour of ``sqrt(T_comm/beta)``."""
+    best, best_t = 1, None
+    for C in range(1, heads_per_rank + 1):
+        t = t_hcms(C, 0.0, t_comm, 0.0, beta)
+        if best_t is None or t < best_t:
+            best, best_t = C, t
+    return best

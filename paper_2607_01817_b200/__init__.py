@@ -52,6 +52,7 @@ _SIGNATURES = {
     "hcms_model_c_star": (c_double, [c_double, c_double]),
     "hcms_model_speedup": (c_double, [c_int, c_double, c_double, c_double]),
     "hcms_model_s_max": (c_double, [c_double]),
+    "hcms_model_choose_chunks": (c_int, [c_int, c_double, c_double]),
     "hcms_plan": (c_int, [POINTER(c_void_p), c_int64, c_int, c_int, c_int, c_int, c_int, c_uint32]),
     "hcms_plan_destroy": (c_int, [c_void_p]),
     "hcms_plan_workspace_bytes": (c_size_t, [c_void_p]),
@@ -67,6 +68,9 @@ _SIGNATURES = {
     "hcms_plan_last_launch_count": (c_int, [c_void_p]),
     "hcms_plan_timings": (c_int, [c_void_p, c_int, POINTER(c_float), POINTER(c_float), POINTER(c_float)]),
     "hcms_plan_step_span": (c_int, [c_void_p, c_int, c_int, POINTER(c_float)]),
+    "hcms_plan_timeline": (c_int, [c_void_p, c_int, POINTER(c_float), POINTER(c_float)]),
+    "hcms_autotune_chunks": (c_int, [c_int64, c_int, c_int, c_int, c_int, c_uint32] + [c_void_p] * 4 +
+                             [c_float, c_void_p, c_int, c_int, POINTER(c_int), POINTER(c_float)]),
 }
 
 
@@ -176,6 +180,10 @@ def hcms_model_s_max(rho) -> float:
     return lib.hcms_model_s_max(rho)
 
 
+def hcms_model_choose_chunks(heads_per_rank: int, t_comm: float, beta: float) -> int:
+    return lib.hcms_model_choose_chunks(heads_per_rank, t_comm, beta)
+
+
 # ---- plan ------------------------------------------------------------------------------------
 
 class Plan:
@@ -258,6 +266,24 @@ def hcms_plan_step_span(plan: Plan, calls_back: int = 0, step: int = 1) -> float
     ms = c_float()
     _check(lib.hcms_plan_step_span(plan.handle, calls_back, step, ctypes.byref(ms)), "hcms_plan_step_span")
     return float(ms.value)
+
+
+def hcms_plan_timeline(plan: Plan, calls_back: int = 0):
+    """-> (begin_ms, end_ms), each [3][C] (scatter, attention, gather) in ms after chunk 0's scatter began."""
+    n = 3 * plan.C
+    b, e = (c_float * n)(), (c_float * n)()
+    _check(lib.hcms_plan_timeline(plan.handle, calls_back, b, e), "hcms_plan_timeline")
+    cut = lambda a: [list(a)[k * plan.C:(k + 1) * plan.C] for k in range(3)]
+    return cut(b), cut(e)
+
+
+def hcms_autotune_chunks(S, H, D, P, dtype, flags, q, k, v, out, scale: float, max_C: int, reps: int = 3, stream=None):
+    """Measure every C in [1, min(max_C, H/P)] on the caller's tensors -> (best_C, [ms per call for C = 1..max_C])."""
+    best = c_int()
+    ms = (c_float * max(int(max_C), 1))()
+    _check(lib.hcms_autotune_chunks(S, H, D, P, dtype, flags, _ptr(q), _ptr(k), _ptr(v), _ptr(out), scale,
+                                    _stream(stream), max_C, reps, ctypes.byref(best), ms), "hcms_autotune_chunks")
+    return int(best.value), list(ms)
 
 
 # ---- the hot path ------------------------------------------------------------------------------

@@ -155,6 +155,16 @@ double hcms_model_s_max(double rho) {
   if (!(rho < 1)) return NAN;
   return 1.0 / (1.0 - rho);  // Theorem 2 (L158, L429)
 }
+int hcms_model_choose_chunks(int heads_per_rank, double t_comm, double beta) {
+  if (heads_per_rank <= 0 || std::isnan(t_comm) || std::isnan(beta)) return 0;
+  if (!(t_comm > 0)) return 1;
+  if (!(beta > 0)) return heads_per_rank;
+  const double c_star = std::sqrt(t_comm / beta);  // Theorem 1; t_comm/C + C*beta is convex in C
+  auto clamp = [&](double c) { return c < 1 ? 1 : (c > heads_per_rank ? heads_per_rank : static_cast<int>(c)); };
+  const int lo = clamp(std::floor(c_star)), hi = clamp(std::ceil(c_star));
+  const double f_lo = t_comm / lo + lo * beta, f_hi = t_comm / hi + hi * beta;
+  return f_hi < f_lo ? hi : lo;
+}
 
 int hcms_plan(hcms_plan_t** out, int64_t S, int H, int D, int P, int C, int dtype, uint32_t flags) {
   if (!out) return fail(HCMS_ERR_INVALID_ARG, "plan output pointer is NULL");
@@ -539,6 +549,76 @@ int hcms_plan_step_span(hcms_plan_t* plan, int calls_back, int step, float* span
   }
   *span_ms = best;
   return HCMS_OK;
+}
+
+int hcms_plan_timeline(hcms_plan_t* plan, int calls_back, float* begin_ms, float* end_ms) {
+  if (!plan || !begin_ms || !end_ms) return fail(HCMS_ERR_INVALID_ARG, "plan, begin_ms or end_ms is NULL");
+  if (!(plan->flags & HCMS_FLAG_PROFILE)) return fail(HCMS_ERR_INVALID_ARG, "plan was made without HCMS_FLAG_PROFILE");
+  if (calls_back < 0 || calls_back >= HCMS_PROFILE_RING || calls_back >= plan->prof_calls)
+    return fail(HCMS_ERR_INVALID_ARG, "calls_back=%d: %lld profiled calls so far, ring keeps %d", calls_back,
+                plan->prof_calls, HCMS_PROFILE_RING);
+  const int C = plan->sh.C;
+  const size_t base = static_cast<size_t>((plan->prof_calls - 1 - calls_back) % HCMS_PROFILE_RING) * C;
+  for (int step = 0; step < 3; ++step)
+    for (int c = 0; c < C; ++c) HCMS_CUDA(cudaEventSynchronize(plan->prof[step][1][base + c]));
+  cudaEvent_t origin = plan->prof[0][0][base];  // chunk 0's scatter begins first (Alg. 1 order on S_comm)
+  for (int step = 0; step < 3; ++step)
+    for (int c = 0; c < C; ++c) {
+      HCMS_CUDA(cudaEventElapsedTime(&begin_ms[step * C + c], origin, plan->prof[step][0][base + c]));
+      HCMS_CUDA(cudaEventElapsedTime(&end_ms[step * C + c], origin, plan->prof[step][1][base + c]));
+    }
+  return HCMS_OK;
+}
+
+int hcms_autotune_chunks(int64_t S, int H, int D, int P, int dtype, uint32_t flags, const void* q, const void* k,
+                         const void* v, void* out, float scale, void* stream, int max_C, int reps, int* best_C,
+                         float* ms_per_call) {
+  if (!q || !k || !v || !out || !best_C) return fail(HCMS_ERR_INVALID_ARG, "NULL argument");
+  if (max_C < 1 || reps < 1) return fail(HCMS_ERR_INVALID_ARG, "max_C=%d and reps=%d must be >= 1", max_C, reps);
+  if (P <= 0 || H <= 0 || H % P) return fail(HCMS_ERR_UNSUPPORTED_SHAPE, "H=%d is not divisible by P=%d", H, P);
+  const int Hl = H / P;
+  const int top = max_C < Hl ? max_C : Hl;
+  cudaStream_t caller = static_cast<cudaStream_t>(stream);
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  HCMS_CUDA(cudaEventCreate(&e0));
+  cudaError_t ce = cudaEventCreate(&e1);
+  if (ce != cudaSuccess) {
+    cudaEventDestroy(e0);
+    return fail_cuda(ce, "cudaEventCreate");
+  }
+  int status = HCMS_OK;
+  float best_ms = 0.f;
+  *best_C = 0;
+  if (ms_per_call)
+    for (int i = 0; i < max_C; ++i) ms_per_call[i] = -1.f;
+  for (int C = 1; C <= top && status == HCMS_OK; ++C) {
+    hcms_plan_t* plan = nullptr;
+    status = hcms_plan(&plan, S, H, D, P, C, dtype, flags & ~(HCMS_FLAG_SERIAL | HCMS_FLAG_PROFILE));
+    if (status != HCMS_OK) break;
+    status = hcms_attention_forward(plan, q, k, v, out, S, H, D, P, C, scale, stream);  // warm-up
+    if (status == HCMS_OK) {
+      ce = cudaEventRecord(e0, caller);
+      for (int r = 0; r < reps && status == HCMS_OK && ce == cudaSuccess; ++r)
+        status = hcms_attention_forward(plan, q, k, v, out, S, H, D, P, C, scale, stream);
+      if (ce == cudaSuccess) ce = cudaEventRecord(e1, caller);
+      if (ce == cudaSuccess) ce = cudaEventSynchronize(e1);
+      float ms = 0.f;
+      if (ce == cudaSuccess) ce = cudaEventElapsedTime(&ms, e0, e1);
+      if (ce != cudaSuccess && status == HCMS_OK) status = fail_cuda(ce, "autotune timing");
+      if (status == HCMS_OK) {
+        ms /= reps;
+        if (ms_per_call) ms_per_call[C - 1] = ms;
+        if (*best_C == 0 || ms < best_ms) {
+          best_ms = ms;
+          *best_C = C;
+        }
+      }
+    }
+    plan_free(plan);
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  return status;
 }
 
 int hcms_attention_forward_host(hcms_plan_t* plan, const void* q, const void* k, const void* v, void* out, int64_t S,

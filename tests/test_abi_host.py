@@ -102,6 +102,18 @@ def test_time_model(golden_rows):
     assert math.isnan(H.hcms_model_t_hcms(0, 1, 1, 1, 1)) and math.isnan(H.hcms_model_speedup(0, .1, .1, 1))
 
 
+def test_choose_chunks_matches_brute_force_over_eq10(golden_rows):
+    from oracle import hcms_oracle as O
+    rho, beta, t_total, c_pred = (float(x) for x in golden_rows("table12_cstar.txt")[0][:4])
+    assert H.hcms_model_choose_chunks(5, rho / 100 * t_total, beta) == int(c_pred)      # Table 12 row 1
+    for Hl in (1, 2, 3, 5, 10, 24):
+        for tc in (0.05, 0.5, 4.6, 29.0, 63.7, 300.0):
+            for b in (1e-3, 0.02, 0.3, 1.41, 6.83, 50.0):
+                assert H.hcms_model_choose_chunks(Hl, tc, b) == O.choose_chunks(Hl, tc, b), (Hl, tc, b)
+    assert H.hcms_model_choose_chunks(7, 10.0, 0.0) == 7 and H.hcms_model_choose_chunks(7, 0.0, 1.0) == 1
+    assert H.hcms_model_choose_chunks(0, 1.0, 1.0) == 0 and H.hcms_model_choose_chunks(4, float("nan"), 1.0) == 0
+
+
 def test_plan_argument_validation_precedes_device_use():
     bf16 = H.HCMS_DTYPE_BF16
     cases = [

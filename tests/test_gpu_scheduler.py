@@ -1,0 +1,115 @@
+"""-m gpu: the dual-stream chunk scheduler of hcms_attention_forward (section 3.4-3.6,
+Algorithm 1) observed through the C ABI: event ordering (Eq. 6-7), the host-routed emulated
+wire (BASELINE.json configs[4]), the adaptive chunk count (future work L346), and a negative test that
+shows the E_c^comm wait is what keeps attention behind its all-to-all.
+
+Every variant must produce the SAME BITS as the plain call (the schedule changes, the function does
+not: L31, Table 14); the plain call itself is checked against the oracle in
+test_gpu_attention.py.
+"""
+import numpy as np
+import pytest
+import torch
+
+import hcms_inputs as I
+import paper_2607_01817_b200 as H
+from gpu_util import DEV, nan_fill_, to_dev, to_host
+
+pytestmark = pytest.mark.gpu
+
+
+def _inputs(S, Hh, D, seed=11):
+    w = I.Workload("sched", S, Hh, D, 1, 1, seed, "bf16", 1.0)
+    return tuple(to_dev(t) for t in I.make_qkv(w)), float(D) ** -0.5
+
+
+def _forward(qkv, S, Hh, D, P, C, scale, flags=0, poison_ws=True):
+    q, k, v = qkv
+    out = nan_fill_(torch.empty_like(q))
+    with H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, flags) as plan:
+        if poison_ws:
+            n = H.hcms_plan_workspace_bytes(plan)
+            ws = nan_fill_(torch.empty((n + 1) // 2, dtype=torch.int16, device=DEV))
+            H.hcms_plan_set_workspace(plan, ws, n)
+        H.hcms_attention_forward(plan, q, k, v, out, scale)
+        torch.cuda.synchronize()
+    return to_host(out)
+
+
+def test_timeline_obeys_eq6_eq7_and_alg1_order():
+    S, Hh, D, P, C = 4096, 12, 128, 2, 3
+    qkv, scale = _inputs(S, Hh, D)
+    out = torch.empty_like(qkv[0])
+    for flags in (0, H.HCMS_FLAG_SINGLE_COMP, H.HCMS_FLAG_SPLIT_COMM):
+        with H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, flags | H.HCMS_FLAG_PROFILE) as plan:
+            for _ in range(3):
+                H.hcms_attention_forward(plan, *qkv, out, scale)
+            b, e = H.hcms_plan_timeline(plan, 0)
+            dur = H.hcms_plan_timings(plan, 0)
+        (sb, ab, gb), (se, ae, ge) = b, e
+        assert sb[0] == 0.0
+        for c in range(C):
+            assert se[c] <= ab[c] + 1e-3, "Attn_c <- wait(E_c^comm)  (Eq. 6)"
+            assert ae[c] <= gb[c] + 1e-3, "A_c^out <- wait(E_c^comp)  (Eq. 7)"
+            assert se[c] > sb[c] and ae[c] > ab[c] and ge[c] > gb[c]
+            for kind, (bb, ee) in enumerate(((sb, se), (ab, ae), (gb, ge))):
+                assert abs((ee[c] - bb[c]) - dur[kind][c]) < 2e-3
+            if c:
+                assert sb[c] >= se[c - 1] - 1e-3, "S_comm issues the input all-to-alls in chunk order (Alg. 1 lines 6-11)"
+                assert gb[c] >= ge[c - 1] - 1e-3
+                if flags & H.HCMS_FLAG_SINGLE_COMP:
+                    assert ab[c] >= ae[c - 1] - 1e-3, "one S_comp runs the chunks in order"
+        if not flags & H.HCMS_FLAG_SPLIT_COMM:
+            assert gb[0] >= se[C - 1] - 1e-3, "single S_comm: output all-to-alls follow all input all-to-alls (R-8)"
+        # the overlap the method exists for: chunk 1's scatter is under way or done before chunk 0's attention ends
+        assert sb[1] < ae[0]
+
+
+def test_timeline_errors():
+    with H.hcms_plan(1024, 4, 64, 2, 2) as plan:
+        with pytest.raises(H.HcmsError) as ei:
+            H.hcms_plan_timeline(plan, 0)
+        assert ei.value.status == H.HCMS_ERR_INVALID_ARG
+    with H.hcms_plan(1024, 4, 64, 2, 2, H.HCMS_DTYPE_BF16, H.HCMS_FLAG_PROFILE) as plan:
+        with pytest.raises(H.HcmsError):
+            H.hcms_plan_timeline(plan, 0)          # no call recorded yet
+
+
+def test_host_routed_wire_keeps_the_bits():
+    S, Hh, D, P, C = 2048, 8, 64, 2, 2
+    qkv, scale = _inputs(S, Hh, D, seed=5)
+    ref = _forward(qkv, S, Hh, D, P, C, scale)
+    Q, K, V, O = H.HCMS_FLAG_HOST_ROUTE_Q, H.HCMS_FLAG_HOST_ROUTE_K, H.HCMS_FLAG_HOST_ROUTE_V, H.HCMS_FLAG_HOST_ROUTE_O
+    for mask in (O, Q | O, Q | K | V | O):
+        for extra in (0, H.HCMS_FLAG_SERIAL, H.HCMS_FLAG_SPLIT_COMM):
+            got = _forward(qkv, S, Hh, D, P, C, scale, mask | extra)
+            assert np.array_equal(got, ref), (hex(mask), hex(extra))
+
+
+def test_autotune_chunks_measures_every_C_and_keeps_the_bits():
+    S, Hh, D, P = 2048, 8, 128, 2
+    qkv, scale = _inputs(S, Hh, D, seed=3)
+    ref = _forward(qkv, S, Hh, D, P, 1, scale)
+    out = nan_fill_(torch.empty_like(qkv[0]))
+    best, ms = H.hcms_autotune_chunks(S, Hh, D, P, H.HCMS_DTYPE_BF16, 0, *qkv, out, scale, 6, 2)
+    torch.cuda.synchronize()
+    assert 1 <= best <= 4 and len(ms) == 6
+    assert all(m > 0 for m in ms[:4]) and ms[4] == -1 and ms[5] == -1       # H/P = 4 caps the sweep
+    assert ms[best - 1] == min(ms[:4])
+    assert np.array_equal(to_host(out), ref)
+    with pytest.raises(H.HcmsError) as ei:
+        H.hcms_autotune_chunks(S, Hh, D, P, H.HCMS_DTYPE_BF16, 0, *qkv, out, scale, 0, 2)
+    assert ei.value.status == H.HCMS_ERR_INVALID_ARG
+
+
+def test_dropping_the_comm_wait_lets_attention_read_unscattered_chunks():
+    """Negative test: with HCMS_FLAG_DEBUG_NO_COMM_WAIT the compute stream no longer
+    waits on E_c^comm, so on a shape whose scatter takes far longer than a launch, attention reads the
+    NaN-poisoned workspace.  The same shape with the wait in place is clean (checked first)."""
+    S, Hh, D, P, C = 16384, 32, 128, 4, 2
+    qkv, scale = _inputs(S, Hh, D, seed=9)
+    good = _forward(qkv, S, Hh, D, P, C, scale)
+    is_nan = lambda bits: ((bits & 0x7F80) == 0x7F80) & ((bits & 0x007F) != 0)
+    assert not is_nan(good).any()
+    bad = _forward(qkv, S, Hh, D, P, C, scale, H.HCMS_FLAG_DEBUG_NO_COMM_WAIT)
+    assert is_nan(bad).any(), "the race did not show: the negative test has lost its teeth"

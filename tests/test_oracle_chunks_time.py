@@ -80,3 +80,15 @@ def test_time_model_limits_and_optimum():
     eps = 1e-4
     f = lambda C: O.t_hcms(C, t0, tc, ta, beta)
     assert f(cs) <= f(cs - eps) and f(cs) <= f(cs + eps)
+
+
+def test_choose_chunks_brute_force_agrees_with_theorem1(golden_rows):
+    # Table 12 row 1 (L440): 40 heads on 8 GPUs = 5 per rank, C* = 4.54 -> the paper prints 5
+    for rho, beta, t_total, pred in golden_rows("table12_cstar.txt"):
+        assert O.choose_chunks(5, float(rho) / 100 * float(t_total), float(beta)) == int(pred)
+    # unconstrained, the integer optimum is a neighbour of Theorem 1's C*; constrained, it is clamped
+    for tc, beta in [(29.0, 1.41), (63.7, 6.83), (0.5, 0.004), (100.0, 0.01), (1.0, 5.0)]:
+        cs = O.c_star(tc, beta)
+        assert O.choose_chunks(10**4, tc, beta) in (max(1, math.floor(cs)), math.ceil(cs))
+        assert O.choose_chunks(3, tc, beta) == min(3, O.choose_chunks(10**4, tc, beta))
+    assert O.choose_chunks(7, 10.0, 0.0) == 7          # no per-chunk overhead: as many chunks as heads
