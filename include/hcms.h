@@ -70,10 +70,10 @@ enum {
                                           128-bit ld/st variant (same bits out) */
 #define HCMS_FLAG_SPLIT_COMM 0x4u      /* separate streams for input and output all-to-all (Eq. 8
                                           "all three in parallel"); default is Alg. 1's single S_comm */
-#define HCMS_FLAG_HOST_ROUTE_Q 0x10u   /* config 5: route this tensor's chunk buffer through pinned host */
-#define HCMS_FLAG_HOST_ROUTE_K 0x20u   /* memory (cudaMemcpyAsync D2H then H2D) after the scatter kernel */
-#define HCMS_FLAG_HOST_ROUTE_V 0x40u   /* (Q,K,V) or before the gather kernel (O) to raise the          */
-#define HCMS_FLAG_HOST_ROUTE_O 0x80u   /* communication ratio rho (section 3.7)                    */
+#define HCMS_FLAG_HOST_ROUTE_Q 0x10u   /* config 5: this tensor's chunk crosses an emulated wire through pinned  */
+#define HCMS_FLAG_HOST_ROUTE_K 0x20u   /* host memory: scatter -> device send buffer -> D2H -> H2D -> Q'_c/K'_c/ */
+#define HCMS_FLAG_HOST_ROUTE_V 0x40u   /* V'_c, and O'_c -> D2H -> H2D -> device receive buffer -> gather, to    */
+#define HCMS_FLAG_HOST_ROUTE_O 0x80u   /* raise the communication ratio rho (section 3.7).  Same bits.     */
 #define HCMS_FLAG_DEBUG_NO_COMM_WAIT 0x100u /* TEST ONLY: drop the compute stream's wait on E_c^comm
                                           (Eq. 6) so a negative test can observe the race */
 

@@ -533,8 +533,8 @@ int poly_setting() {
   static int v = -1;
   if (v < 0) {
     const char* e = std::getenv("HCMS_ATTN_POLY");
-    v = e ? std::atoi(e) : 3;
-    if (v < 0 || v > 8) v = 3;
+    v = e ? std::atoi(e) : 2;
+    if (v < 0 || v > 8) v = 2;
   }
   return v;
 }
@@ -544,12 +544,12 @@ KernelFn pick_kernel(int poly) {
   switch (poly) {
     case 0: return attention_fwd_kernel<D, 0>;
     case 1: return attention_fwd_kernel<D, 1>;
-    case 2: return attention_fwd_kernel<D, 2>;
+    case 3: return attention_fwd_kernel<D, 3>;
     case 4: return attention_fwd_kernel<D, 4>;
     case 5: return attention_fwd_kernel<D, 5>;
     case 6: return attention_fwd_kernel<D, 6>;
     case 8: return attention_fwd_kernel<D, 8>;
-    default: return attention_fwd_kernel<D, 3>;
+    default: return attention_fwd_kernel<D, 2>;
   }
 }
 

@@ -64,8 +64,10 @@ struct hcms_plan {
   cudaStream_t s_comm = nullptr, s_comm_out = nullptr, s_comp = nullptr, s_comp2 = nullptr;
   cudaEvent_t e_main = nullptr, e_fin_comm = nullptr, e_fin_comp = nullptr, e_fin_comp2 = nullptr, e_fin_in = nullptr;
   std::vector<cudaEvent_t> e_comm, e_comp;
-  // host route (config 5)
+  // host route (config 5): per routed tensor one pinned host buffer and one device "send/receive" buffer,
+  // each as large as the largest chunk tensor
   void* pinned[4] = {nullptr, nullptr, nullptr, nullptr};
+  void* wire[4] = {nullptr, nullptr, nullptr, nullptr};
   // host-buffer entry point staging
   void* staging[4] = {nullptr, nullptr, nullptr, nullptr};
   int last_launches = 0;
@@ -98,6 +100,8 @@ static void plan_free(hcms_plan_t* p) {
   if (p->ws_owned && p->ws) cudaFree(p->ws);
   for (auto& h : p->pinned)
     if (h) cudaFreeHost(h);
+  for (auto& d : p->wire)
+    if (d) cudaFree(d);
   for (auto& d : p->staging)
     if (d) cudaFree(d);
   delete p;
@@ -259,7 +263,10 @@ int hcms_plan(hcms_plan_t** out, int64_t S, int H, int D, int P, int C, int dtyp
     size_t max_chunk = 0;
     for (auto& ck : p->chunks) max_chunk = ck.bytes > max_chunk ? ck.bytes : max_chunk;
     for (int t = 0; t < 4; ++t)
-      if (flags & (HCMS_FLAG_HOST_ROUTE_Q << t)) PLAN_CUDA(cudaMallocHost(&p->pinned[t], max_chunk));
+      if (flags & (HCMS_FLAG_HOST_ROUTE_Q << t)) {
+        PLAN_CUDA(cudaMallocHost(&p->pinned[t], max_chunk));
+        PLAN_CUDA(cudaMalloc(&p->wire[t], max_chunk));
+      }
   }
 #undef PLAN_CUDA
   *out = p;
@@ -432,11 +439,13 @@ int hcms_attention_forward(hcms_plan_t* plan, const void* q, const void* k, cons
   char* ws = static_cast<char*>(plan->ws);
   plan->last_launches = 0;
 
-  auto host_route = [&](int t, const Chunk& ck, cudaStream_t s) -> int {
-    if (!(plan->flags & (HCMS_FLAG_HOST_ROUTE_Q << t))) return HCMS_OK;
-    // the emulated wire: device -> pinned host -> device, same bits
-    HCMS_CUDA(cudaMemcpyAsync(plan->pinned[t], ws + ck.off[t], ck.bytes, cudaMemcpyDeviceToHost, s));
-    HCMS_CUDA(cudaMemcpyAsync(ws + ck.off[t], plan->pinned[t], ck.bytes, cudaMemcpyHostToDevice, s));
+  // The emulated wire of BASELINE.json configs[4]: a routed tensor's chunk is produced into the plan's
+  // device send buffer, crosses to pinned host memory and comes back into the buffer its consumer reads
+  // (scatter -> wire -> D2H -> H2D -> Q'_c/K'_c/V'_c;  O'_c -> D2H -> H2D -> wire -> gather).  Same bits.
+  auto routed = [&](int t) { return (plan->flags & (HCMS_FLAG_HOST_ROUTE_Q << t)) != 0; };
+  auto host_hop = [&](int t, const void* from, void* to, size_t bytes, cudaStream_t s) -> int {
+    HCMS_CUDA(cudaMemcpyAsync(plan->pinned[t], from, bytes, cudaMemcpyDeviceToHost, s));
+    HCMS_CUDA(cudaMemcpyAsync(to, plan->pinned[t], bytes, cudaMemcpyHostToDevice, s));
     plan->last_launches += 2;
     return HCMS_OK;
   };
@@ -458,12 +467,14 @@ int hcms_attention_forward(hcms_plan_t* plan, const void* q, const void* k, cons
   for (int c = 0; c < sh.C; ++c) {
     const Chunk& ck = plan->chunks[c];
     const void* src[3] = {q, k, v};
-    void* dst[3] = {ws + ck.off[0], ws + ck.off[1], ws + ck.off[2]};
+    void* dst[3];
+    for (int t = 0; t < 3; ++t) dst[t] = routed(t) ? plan->wire[t] : static_cast<void*>(ws + ck.off[t]);
     HCMS_CUDA(mark(0, c, 0, s_in));
     st = do_layout(plan, 3, src, dst, c, false, s_in);
     if (st) return st;
     for (int t = 0; t < 3; ++t) {
-      st = host_route(t, ck, s_in);
+      if (!routed(t)) continue;
+      st = host_hop(t, plan->wire[t], ws + ck.off[t], ck.bytes, s_in);
       if (st) return st;
     }
     HCMS_CUDA(mark(0, c, 1, s_in));
@@ -486,9 +497,11 @@ int hcms_attention_forward(hcms_plan_t* plan, const void* q, const void* k, cons
     const Chunk& ck = plan->chunks[c];
     if (!serial) HCMS_CUDA(cudaStreamWaitEvent(s_out, plan->e_comp[c], 0));
     HCMS_CUDA(mark(2, c, 0, s_out));
-    st = host_route(3, ck, s_out);
-    if (st) return st;
-    const void* src[1] = {ws + ck.off[3]};
+    if (routed(3)) {
+      st = host_hop(3, ws + ck.off[3], plan->wire[3], ck.bytes, s_out);
+      if (st) return st;
+    }
+    const void* src[1] = {routed(3) ? plan->wire[3] : static_cast<const void*>(ws + ck.off[3])};
     void* dst[1] = {out};
     st = do_layout(plan, 1, src, dst, c, true, s_out);
     if (st) return st;

@@ -9,8 +9,9 @@
 // and written once, so the roofline is HBM bandwidth (2*P*S*h_c*D*es bytes per tensor).
 //
 // Two variants, same bits out:
-//   * vec: 128-bit ld.global.nc / st.global, four independent requests per thread, one launch
-//          for Q,K,V (grid.z), destination-contiguous thread order;
+//   * vec: 256-bit ld.global.nc / st.global (LDG.256 / STG.256; 128-bit if a pointer is only 16-byte
+//          aligned), four independent requests per thread, one launch for Q,K,V (grid.z), thread order
+//          following the contiguous side; no shared memory, so its CTAs fit beside a resident attention CTA;
 //   * tma: one elected thread per CTA drives a ring of shared-memory stages: a TMA bulk-tensor
 //          load of a [rows][h_c][D] box per (rank, head-chunk) tile, then a bulk store of the
 //          now contiguous tile (scatter), or the reverse (gather).  Few registers, no LSU work.
@@ -24,81 +25,124 @@ using namespace ptx;
 // vec variant
 // ------------------------------------------------------------------------------------------
 struct LayoutVecParams {
-  const uint4* src[3];
-  uint4* dst[3];
-  uint32_t n_per_rank;       // S * run_vecs  (16-byte vectors of one rank's dense block)
-  uint32_t run_vecs;         // h_c*D*es/16   (contiguous run in the strided tensor)
-  uint32_t row_stride_vecs;  // H*D*es/16
-  uint32_t rank_stride_vecs; // Hl*D*es/16
-  uint32_t chunk_off_vecs;   // o_c*D*es/16
+  const uint8_t* src[3];
+  uint8_t* dst[3];
+  uint32_t n_per_rank;       // S * run_vecs  (vectors of one rank's dense block)
+  uint32_t run_vecs;         // h_c*D*es / vector bytes  (contiguous run in the strided tensor)
+  uint32_t row_stride_vecs;  // H*D*es / vector bytes
+  uint32_t rank_stride_vecs; // Hl*D*es / vector bytes
+  uint32_t chunk_off_vecs;   // o_c*D*es / vector bytes
+  uint32_t step_rows;        // kVecThreads / run_vecs : how far a thread's next vector lies, in rows ...
+  uint32_t step_cols;        // kVecThreads % run_vecs : ... and in vectors inside the run
 };
 
-__device__ __forceinline__ uint4 ld_stream(const uint4* p) {
-  uint4 r;
+// 128-bit and 256-bit (sm_100: LDG.256 / STG.256) streaming accesses that stay out of L1
+struct alignas(16) Vec16 {
+  uint32_t v[4];
+};
+struct alignas(32) Vec32 {
+  uint32_t v[8];
+};
+__device__ __forceinline__ void ld_stream(const uint8_t* p, Vec16& r) {
   asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
-               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+               : "=r"(r.v[0]), "=r"(r.v[1]), "=r"(r.v[2]), "=r"(r.v[3])
                : "l"(p));
-  return r;
 }
-__device__ __forceinline__ void st_stream(uint4* p, const uint4& v) {
-  asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x), "r"(v.y),
-               "r"(v.z), "r"(v.w)
+__device__ __forceinline__ void st_stream(uint8_t* p, const Vec16& r) {
+  asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(r.v[0]), "r"(r.v[1]), "r"(r.v[2]),
+               "r"(r.v[3])
+               : "memory");
+}
+__device__ __forceinline__ void ld_stream(const uint8_t* p, Vec32& r) {
+  asm volatile("ld.global.nc.L1::no_allocate.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=r"(r.v[0]), "=r"(r.v[1]), "=r"(r.v[2]), "=r"(r.v[3]), "=r"(r.v[4]), "=r"(r.v[5]), "=r"(r.v[6]),
+                 "=r"(r.v[7])
+               : "l"(p));
+}
+__device__ __forceinline__ void st_stream(uint8_t* p, const Vec32& r) {
+  asm volatile("st.global.L1::no_allocate.v8.u32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "r"(r.v[0]), "r"(r.v[1]),
+               "r"(r.v[2]), "r"(r.v[3]), "r"(r.v[4]), "r"(r.v[5]), "r"(r.v[6]), "r"(r.v[7])
                : "memory");
 }
 
 constexpr int kVecThreads = 256;
 constexpr int kVecUnroll = 4;
 
-template <bool kGather>
+// Thread order follows the dense (contiguous) side: vector i of a rank's dense block is row s = i / run_vecs,
+// column w = i % run_vecs of the run.  One division per thread; the thread's next vectors lie kVecThreads
+// further, i.e. (step_rows, step_cols) further with a carry.  All loads are issued before the first store.
+template <bool kGather, typename Vec>
 __global__ void __launch_bounds__(kVecThreads) layout_vec_kernel(const LayoutVecParams p) {
   const uint32_t rank = blockIdx.y;
-  const uint4* __restrict__ src = p.src[blockIdx.z];
-  uint4* __restrict__ dst = p.dst[blockIdx.z];
+  // selects, not p.src[blockIdx.z]: a dynamically indexed kernel parameter is copied to the stack
+  const uint32_t z = blockIdx.z;
+  const uint8_t* __restrict__ src = z == 0 ? p.src[0] : (z == 1 ? p.src[1] : p.src[2]);
+  uint8_t* __restrict__ dst = z == 0 ? p.dst[0] : (z == 1 ? p.dst[1] : p.dst[2]);
   const uint32_t i0 = blockIdx.x * (kVecThreads * kVecUnroll) + threadIdx.x;
   const size_t dense_base = static_cast<size_t>(rank) * p.n_per_rank;
   const size_t strided_base = static_cast<size_t>(rank) * p.rank_stride_vecs + p.chunk_off_vecs;
+  uint32_t s = i0 / p.run_vecs;
+  uint32_t w = i0 - s * p.run_vecs;
 
-  uint4 val[kVecUnroll];
+  Vec val[kVecUnroll];
   size_t out_idx[kVecUnroll];
 #pragma unroll
   for (int u = 0; u < kVecUnroll; ++u) {
     const uint32_t i = i0 + u * kVecThreads;
     if (i < p.n_per_rank) {
-      const uint32_t s = i / p.run_vecs;
-      const uint32_t w = i - s * p.run_vecs;
       const size_t strided = static_cast<size_t>(s) * p.row_stride_vecs + strided_base + w;
       const size_t dense = dense_base + i;
-      val[u] = ld_stream(src + (kGather ? dense : strided));
+      ld_stream(src + (kGather ? dense : strided) * sizeof(Vec), val[u]);
       out_idx[u] = kGather ? strided : dense;
+    }
+    s += p.step_rows;
+    w += p.step_cols;
+    if (w >= p.run_vecs) {
+      w -= p.run_vecs;
+      s += 1;
     }
   }
 #pragma unroll
   for (int u = 0; u < kVecUnroll; ++u) {
     const uint32_t i = i0 + u * kVecThreads;
-    if (i < p.n_per_rank) st_stream(dst + out_idx[u], val[u]);
+    if (i < p.n_per_rank) st_stream(dst + out_idx[u] * sizeof(Vec), val[u]);
   }
 }
 
 cudaError_t launch_layout_vec(const LayoutArgs& a, cudaStream_t stream) {
   LayoutVecParams p{};
   const size_t run_bytes = static_cast<size_t>(a.h_c) * a.D * a.es;
-  const size_t n_per_rank = static_cast<size_t>(a.S) * (run_bytes / 16);
-  if (run_bytes % 16 || n_per_rank >= (1ull << 31)) return cudaErrorInvalidValue;
+  // 256-bit accesses when every address is 32-byte aligned (runs are multiples of 128 B for D >= 64), else 128-bit
+  bool wide = run_bytes % 32 == 0 && (static_cast<size_t>(a.D) * a.es) % 32 == 0;
+  for (int t = 0; t < a.n_tensors; ++t)
+    wide = wide && reinterpret_cast<uintptr_t>(a.src[t]) % 32 == 0 && reinterpret_cast<uintptr_t>(a.dst[t]) % 32 == 0;
+  const size_t vb = wide ? 32 : 16;
+  const size_t n_per_rank = static_cast<size_t>(a.S) * (run_bytes / vb);
+  if (run_bytes % vb || n_per_rank >= (1ull << 31)) return cudaErrorInvalidValue;
   for (int t = 0; t < a.n_tensors; ++t) {
-    p.src[t] = static_cast<const uint4*>(a.src[t]);
-    p.dst[t] = static_cast<uint4*>(a.dst[t]);
+    p.src[t] = static_cast<const uint8_t*>(a.src[t]);
+    p.dst[t] = static_cast<uint8_t*>(a.dst[t]);
   }
   p.n_per_rank = static_cast<uint32_t>(n_per_rank);
-  p.run_vecs = static_cast<uint32_t>(run_bytes / 16);
-  p.row_stride_vecs = static_cast<uint32_t>(static_cast<size_t>(a.H) * a.D * a.es / 16);
-  p.rank_stride_vecs = static_cast<uint32_t>(static_cast<size_t>(a.Hl) * a.D * a.es / 16);
-  p.chunk_off_vecs = static_cast<uint32_t>(static_cast<size_t>(a.o_c) * a.D * a.es / 16);
+  p.run_vecs = static_cast<uint32_t>(run_bytes / vb);
+  p.row_stride_vecs = static_cast<uint32_t>(static_cast<size_t>(a.H) * a.D * a.es / vb);
+  p.rank_stride_vecs = static_cast<uint32_t>(static_cast<size_t>(a.Hl) * a.D * a.es / vb);
+  p.chunk_off_vecs = static_cast<uint32_t>(static_cast<size_t>(a.o_c) * a.D * a.es / vb);
+  p.step_rows = kVecThreads / p.run_vecs;
+  p.step_cols = kVecThreads % p.run_vecs;
   const uint32_t per_block = kVecThreads * kVecUnroll;
   dim3 grid((p.n_per_rank + per_block - 1) / per_block, a.P, a.n_tensors);
-  if (a.gather)
-    layout_vec_kernel<true><<<grid, kVecThreads, 0, stream>>>(p);
-  else
-    layout_vec_kernel<false><<<grid, kVecThreads, 0, stream>>>(p);
+  if (a.gather) {
+    if (wide)
+      layout_vec_kernel<true, Vec32><<<grid, kVecThreads, 0, stream>>>(p);
+    else
+      layout_vec_kernel<true, Vec16><<<grid, kVecThreads, 0, stream>>>(p);
+  } else {
+    if (wide)
+      layout_vec_kernel<false, Vec32><<<grid, kVecThreads, 0, stream>>>(p);
+    else
+      layout_vec_kernel<false, Vec16><<<grid, kVecThreads, 0, stream>>>(p);
+  }
   return cudaGetLastError();
 }
 

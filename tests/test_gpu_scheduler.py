@@ -103,13 +103,15 @@ def test_autotune_chunks_measures_every_C_and_keeps_the_bits():
 
 
 def test_dropping_the_comm_wait_lets_attention_read_unscattered_chunks():
-    """Negative test: with HCMS_FLAG_DEBUG_NO_COMM_WAIT the compute stream no longer
-    waits on E_c^comm, so on a shape whose scatter takes far longer than a launch, attention reads the
-    NaN-poisoned workspace.  The same shape with the wait in place is clean (checked first)."""
-    S, Hh, D, P, C = 16384, 32, 128, 4, 2
+    """Negative test: with HCMS_FLAG_DEBUG_NO_COMM_WAIT the compute stream no longer waits
+    on E_c^comm.  V takes the emulated wire through pinned host memory (milliseconds), so attention, no longer
+    held back by the event, reads the NaN-poisoned V'_c before the wire delivers it.  The same call with the
+    wait in place is clean (checked first)."""
+    S, Hh, D, P, C = 8192, 16, 128, 2, 2
     qkv, scale = _inputs(S, Hh, D, seed=9)
-    good = _forward(qkv, S, Hh, D, P, C, scale)
     is_nan = lambda bits: ((bits & 0x7F80) == 0x7F80) & ((bits & 0x007F) != 0)
+    good = _forward(qkv, S, Hh, D, P, C, scale, H.HCMS_FLAG_HOST_ROUTE_V)
     assert not is_nan(good).any()
-    bad = _forward(qkv, S, Hh, D, P, C, scale, H.HCMS_FLAG_DEBUG_NO_COMM_WAIT)
+    assert np.array_equal(good, _forward(qkv, S, Hh, D, P, C, scale))
+    bad = _forward(qkv, S, Hh, D, P, C, scale, H.HCMS_FLAG_HOST_ROUTE_V | H.HCMS_FLAG_DEBUG_NO_COMM_WAIT)
     assert is_nan(bad).any(), "the race did not show: the negative test has lost its teeth"
