@@ -23,7 +23,7 @@ import numpy as np
 
 __all__ = [
     "Workload", "WORKLOADS", "workload", "normal_f32", "f32_to_bf16_bits",
-    "bf16_bits_to_f32", "make_qkv", "index_pattern",
+    "bf16_bits_to_f32", "make_qkv", "index_pattern", "make_layer_inputs", "rope_tables",
 ]
 
 _MASK64 = np.uint64(0xFFFFFFFFFFFFFFFF)
@@ -163,3 +163,31 @@ def index_pattern(S: int, H: int, D: int, dtype) -> np.ndarray:
         return ids.reshape(S, H, D).view(dt) if dt != np.uint16 else ids.reshape(S, H, D)
     ids = (ids & np.uint64(0xFFFFFFFF)).astype(np.uint32)
     return ids.reshape(S, H, D).view(dt) if dt != np.uint32 else ids.reshape(S, H, D)
+
+
+def rope_tables(S: int, D: int, base: float = 10000.0):
+    """cos/sin tables ``[S, D/2]`` fp32 handed to the layer as INPUT data (the library and the oracle both
+    only consume tables): angle(s, i) = s * base**(-2i/D), the 1-D position scheme of RoFormer [34], computed
+    in fp64 and rounded once.  A video DiT would tabulate its 3-D grid angles the same way."""
+    i = np.arange(D // 2, dtype=np.float64)
+    ang = np.arange(S, dtype=np.float64)[:, None] * (base ** (-2.0 * i / D))[None, :]
+    return np.cos(ang).astype(np.float32), np.sin(ang).astype(np.float32)
+
+
+def make_layer_inputs(w: Workload, Dm: int | None = None, S: int | None = None, threads: int = 8):
+    """Inputs of the whole attention layer (Alg. 1 lines 2-27) for workload ``w``: activations
+    ``x [S, Dm]`` ~ N(0,1) (tensor id 3), ``w_qkv [3*H*D, Dm]`` ~ N(0, 1/Dm) (id 4), ``w_o [Dm, H*D]`` ~
+    N(0, 1/(H*D)) (id 5), all rounded to bf16 bit patterns, plus :func:`rope_tables`.  ``Dm`` defaults to
+    ``H*D`` (Table 3: 5120 = 40 x 128).  Random-init weights stand in for the model's: the paper's
+    checkpoints are not available here.  With these variances q, k, v come out ~ N(0,1), the distribution of
+    :func:`make_qkv`; ``k_scale`` (config 3) multiplies the K rows of ``w_qkv``."""
+    S = w.S if S is None else int(S)
+    hd = w.H * w.D
+    Dm = hd if Dm is None else int(Dm)
+    x = f32_to_bf16_bits(normal_f32(w.seed, 3, S * Dm, threads=threads).reshape(S, Dm))
+    wq = normal_f32(w.seed, 4, 3 * hd * Dm, threads=threads).reshape(3 * hd, Dm) * np.float32(1.0 / np.sqrt(Dm))
+    if w.k_scale != 1.0:
+        wq[hd:2 * hd] *= np.float32(w.k_scale)
+    wo = normal_f32(w.seed, 5, Dm * hd, threads=threads).reshape(Dm, hd) * np.float32(1.0 / np.sqrt(hd))
+    cos, sin = rope_tables(S, w.D)
+    return x, f32_to_bf16_bits(wq), f32_to_bf16_bits(wo), cos, sin

@@ -40,7 +40,7 @@
 extern "C" {
 #endif
 
-#define HCMS_VERSION 100 /* major*10000 + minor*100 + patch */
+#define HCMS_VERSION 200 /* major*10000 + minor*100 + patch */
 
 /* ---- status codes ------------------------------------------------------------------- */
 enum {
@@ -252,6 +252,57 @@ int hcms_plan_timeline(hcms_plan_t* plan, int calls_back, float* begin_ms, float
 int hcms_autotune_chunks(int64_t S, int H, int D, int P, int dtype, uint32_t flags, const void* q, const void* k,
                          const void* v, void* out, float scale, void* stream, int max_C, int reps, int* best_C,
                          float* ms_per_call);
+
+/* ---- the attention layer around the hot path --------------------------------- */
+/*
+ * Section 3.1 (L59): "QKV projection -> RoPE positional encoding -> input all-to-all -> attention
+ * computation -> output all-to-all -> output projection"; Algorithm 1 (L170) lines 2, 3 and 27.  These are
+ * the T_other of Eq. 1 (L61).  Both projections are torch.nn.Linear-style maps without bias (the paper
+ * names none):  C[M,N] = A[M,K] * B[N,K]^T, bf16 operands, fp32 accumulation, bf16 result (RNE).
+ *
+ * hcms_gemm_bf16_nt: the bare contraction.  a: device [M,K] bf16, b: device [N,K] bf16, c: device [M,N]
+ * bf16, all row-major, 16-byte aligned, c not overlapping a or b.  K % 8 == 0, N % 128 == 0.
+ * Asynchronous on `stream`.  Errors: INVALID_ARG, UNSUPPORTED_SHAPE, MISALIGNED, ALIAS,
+ * UNSUPPORTED_DEVICE, CUDA.
+ */
+int hcms_gemm_bf16_nt(const void* a, const void* b, void* c, int64_t M, int N, int K, void* stream);
+/*
+ * Alg. 1 lines 2-3 in one kernel: [q|k|v] = x * w_qkv^T, then the rotary embedding on q and k.
+ *   x: device [S, Dm] bf16 (the P ranks' token shards in rank order); w_qkv: device [3*H*D, Dm] bf16, row n =
+ *   output feature n, features ordered q heads, k heads, v heads, D consecutive features per head;
+ *   q,k,v: device [S,H,D] bf16 (the layout hcms_attention_forward takes).
+ *   rope_cos, rope_sin: device [S, D/2] fp32 tables, or both NULL for no rotation.  For token s and pair
+ *   i < D/2 of every head:  (x[2i], x[2i+1]) <- (x[2i]*c - x[2i+1]*s, x[2i]*s + x[2i+1]*c), c = cos[s][i],
+ *   s = sin[s][i]  (adjacent-pair convention of RoFormer [34]; the caller's table fixes the position scheme,
+ *   1-D or the 3-D grid of a video DiT).  The rotation is applied to the fp32 accumulators, then rounded once.
+ * S,H,D are the plan's; Dm % 128 == 0 and H*D % 128 == 0.  Asynchronous on `stream`.
+ * Errors: INVALID_ARG (NULL, only one table NULL, Dm <= 0), UNSUPPORTED_SHAPE, UNSUPPORTED_DTYPE (plan not
+ * bf16), MISALIGNED, CUDA.
+ */
+int hcms_qkv_projection_rope(hcms_plan_t* plan, const void* x, const void* w_qkv, const void* rope_cos,
+                             const void* rope_sin, void* q, void* k, void* v, int Dm, void* stream);
+/* Alg. 1 line 27: y[S,Dm] = o[S,H*D] * w_o^T; o: device [S,H,D] bf16 (the Concat of line 26), w_o: device
+ * [Dm, H*D] bf16, y: device [S,Dm] bf16.  Same rules and errors as above. */
+int hcms_output_projection(hcms_plan_t* plan, const void* o, const void* w_o, void* y, int Dm, void* stream);
+/*
+ * Algorithm 1 lines 2-27 for one layer: hcms_qkv_projection_rope on `stream` (main stream), then
+ * hcms_attention_forward (lines 4-26: E_main, S_comm / S_comp, events) on the plan-owned q,k,v,o buffers
+ * (4*S*H*D*2 bytes, allocated on first use), then hcms_output_projection on `stream`.
+ * x: device [S,Dm] bf16; y: device [S,Dm] bf16, not overlapping x; weights and tables as above.
+ * S,H,D,P,C must equal the plan's.  Asynchronous: y is valid once the caller synchronises `stream`.
+ * With HCMS_FLAG_PROFILE the three parts are bracketed by events (hcms_plan_layer_timings).
+ * Errors: those of the three calls it makes.
+ */
+int hcms_layer_forward(hcms_plan_t* plan, const void* x, const void* w_qkv, const void* w_o, const void* rope_cos,
+                       const void* rope_sin, void* y, int64_t S, int Dm, int H, int D, int P, int C, float scale,
+                       void* stream);
+/* Device address of the plan-owned layer buffer `which` (0 = q, 1 = k, 2 = v after RoPE, 3 = o) of
+ * hcms_layer_forward, each [S,H,D] bf16; NULL before the first call.  For tests. */
+void* hcms_plan_layer_buffer(const hcms_plan_t* plan, int which);
+/* Device milliseconds of the last hcms_layer_forward on a HCMS_FLAG_PROFILE plan: QKV projection + RoPE,
+ * lines 4-26 (all-to-alls and attention), output projection.  Any pointer may be NULL.  SYNCHRONISES the
+ * host with those events.  Errors: INVALID_ARG (no profiled layer call yet), CUDA. */
+int hcms_plan_layer_timings(hcms_plan_t* plan, float* qkv_ms, float* hcms_ms, float* out_ms);
 
 #ifdef __cplusplus
 }

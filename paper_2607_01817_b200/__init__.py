@@ -71,6 +71,12 @@ _SIGNATURES = {
     "hcms_plan_timeline": (c_int, [c_void_p, c_int, POINTER(c_float), POINTER(c_float)]),
     "hcms_autotune_chunks": (c_int, [c_int64, c_int, c_int, c_int, c_int, c_uint32] + [c_void_p] * 4 +
                              [c_float, c_void_p, c_int, c_int, POINTER(c_int), POINTER(c_float)]),
+    "hcms_gemm_bf16_nt": (c_int, [c_void_p] * 3 + [c_int64, c_int, c_int, c_void_p]),
+    "hcms_qkv_projection_rope": (c_int, [c_void_p] * 8 + [c_int, c_void_p]),
+    "hcms_output_projection": (c_int, [c_void_p] * 4 + [c_int, c_void_p]),
+    "hcms_layer_forward": (c_int, [c_void_p] * 7 + [c_int64, c_int, c_int, c_int, c_int, c_int, c_float, c_void_p]),
+    "hcms_plan_layer_buffer": (c_void_p, [c_void_p, c_int]),
+    "hcms_plan_layer_timings": (c_int, [c_void_p, POINTER(c_float), POINTER(c_float), POINTER(c_float)]),
 }
 
 
@@ -317,3 +323,40 @@ def hcms_a2a_gather(plan: Plan, src, dst, c: int, stream=None) -> None:
 def hcms_attention_chunk(plan: Plan, qc, kc, vc, oc, c: int, scale: float, stream=None) -> None:
     _check(lib.hcms_attention_chunk(plan.handle, _ptr(qc), _ptr(kc), _ptr(vc), _ptr(oc), c, scale, _stream(stream)),
            "hcms_attention_chunk")
+
+
+# ---- the attention layer around the hot path (Alg. 1 lines 2-3, 27) ------------------------------
+
+def hcms_gemm_bf16_nt(a, b, c, M: int, N: int, K: int, stream=None) -> None:
+    """c[M,N] = a[M,K] @ b[N,K]^T on device bf16 tensors; asynchronous on ``stream``."""
+    _check(lib.hcms_gemm_bf16_nt(_ptr(a), _ptr(b), _ptr(c), M, N, K, _stream(stream)), "hcms_gemm_bf16_nt")
+
+
+def hcms_qkv_projection_rope(plan: Plan, x, w_qkv, rope_cos, rope_sin, q, k, v, Dm: int, stream=None) -> None:
+    """Alg. 1 lines 2-3: x[S,Dm] @ w_qkv[3HD,Dm]^T -> q,k,v [S,H,D], RoPE on q,k (tables [S,D/2] fp32 or None)."""
+    _check(lib.hcms_qkv_projection_rope(plan.handle, _ptr(x), _ptr(w_qkv), _ptr(rope_cos), _ptr(rope_sin), _ptr(q),
+                                        _ptr(k), _ptr(v), Dm, _stream(stream)), "hcms_qkv_projection_rope")
+
+
+def hcms_output_projection(plan: Plan, o, w_o, y, Dm: int, stream=None) -> None:
+    """Alg. 1 line 27: y[S,Dm] = o[S,H*D] @ w_o[Dm,H*D]^T."""
+    _check(lib.hcms_output_projection(plan.handle, _ptr(o), _ptr(w_o), _ptr(y), Dm, _stream(stream)),
+           "hcms_output_projection")
+
+
+def hcms_layer_forward(plan: Plan, x, w_qkv, w_o, rope_cos, rope_sin, y, Dm: int, scale: float, stream=None) -> None:
+    """Alg. 1 lines 2-27 on device tensors; asynchronous on ``stream``."""
+    _check(lib.hcms_layer_forward(plan.handle, _ptr(x), _ptr(w_qkv), _ptr(w_o), _ptr(rope_cos), _ptr(rope_sin), _ptr(y),
+                                  plan.S, Dm, plan.H, plan.D, plan.P, plan.C, scale, _stream(stream)),
+           "hcms_layer_forward")
+
+
+def hcms_plan_layer_buffer(plan: Plan, which: int) -> int:
+    return lib.hcms_plan_layer_buffer(plan.handle, which) or 0
+
+
+def hcms_plan_layer_timings(plan: Plan):
+    """-> (qkv_ms, hcms_ms, out_ms) of the last hcms_layer_forward (HCMS_FLAG_PROFILE plans)."""
+    vals = [c_float() for _ in range(3)]
+    _check(lib.hcms_plan_layer_timings(plan.handle, *[ctypes.byref(v) for v in vals]), "hcms_plan_layer_timings")
+    return tuple(float(v.value) for v in vals)

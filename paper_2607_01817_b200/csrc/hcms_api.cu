@@ -71,6 +71,10 @@ struct hcms_plan {
   // host-buffer entry point staging
   void* staging[4] = {nullptr, nullptr, nullptr, nullptr};
   int last_launches = 0;
+  // hcms_layer_forward: q,k,v,o [S,H,D] (allocated on first use) and, under HCMS_FLAG_PROFILE, 4 events
+  void* layer_buf[4] = {nullptr, nullptr, nullptr, nullptr};
+  cudaEvent_t e_layer[4] = {nullptr, nullptr, nullptr, nullptr};
+  bool layer_timed = false;
   // HCMS_FLAG_PROFILE: [step 0=scatter,1=attention,2=gather][begin,end][ring slot * C + chunk]
   std::vector<cudaEvent_t> prof[3][2];
   long long prof_calls = 0;   // forward calls that recorded a full set of events
@@ -104,6 +108,10 @@ static void plan_free(hcms_plan_t* p) {
     if (d) cudaFree(d);
   for (auto& d : p->staging)
     if (d) cudaFree(d);
+  for (auto& d : p->layer_buf)
+    if (d) cudaFree(d);
+  for (auto& e : p->e_layer)
+    if (e) cudaEventDestroy(e);
   delete p;
 }
 
@@ -256,6 +264,8 @@ int hcms_plan(hcms_plan_t** out, int64_t S, int H, int D, int P, int C, int dtyp
         side.assign(static_cast<size_t>(C) * HCMS_PROFILE_RING, nullptr);
         for (auto& e : side) PLAN_CUDA(cudaEventCreate(&e));
       }
+  if (flags & HCMS_FLAG_PROFILE)
+    for (auto& e : p->e_layer) PLAN_CUDA(cudaEventCreate(&e));
   PLAN_CUDA(cudaMalloc(&p->ws, p->ws_bytes));
   p->ws_owned = true;
   if (dtype == HCMS_DTYPE_BF16) PLAN_CUDA(attention_init());
@@ -652,6 +662,180 @@ int hcms_attention_forward_host(hcms_plan_t* plan, const void* q, const void* k,
   if (st) return st;
   HCMS_CUDA(cudaMemcpyAsync(out, plan->staging[3], bytes, cudaMemcpyDeviceToHost, caller));
   HCMS_CUDA(cudaStreamSynchronize(caller));
+  return HCMS_OK;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------
+// the attention layer around the hot path (Alg. 1 lines 2-3 and 27)
+// ------------------------------------------------------------------------------------------
+static bool overlaps(const void* a, size_t na, const void* b, size_t nb) {
+  const char* x = static_cast<const char*>(a);
+  const char* y = static_cast<const char*>(b);
+  return x < y + nb && y < x + na;
+}
+
+static int device_sms(int* sms) {
+  static int cached = 0;
+  if (cached == 0) {
+    int dev = 0, n = 0;
+    cudaError_t ce = cudaGetDeviceCount(&n);
+    if (ce != cudaSuccess || n == 0) {
+      cudaGetLastError();
+      return fail(HCMS_ERR_UNSUPPORTED_DEVICE, "no CUDA device; libhcms has no CPU fallback");
+    }
+    HCMS_CUDA(cudaGetDevice(&dev));
+    int major = 0, count = 0;
+    HCMS_CUDA(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    HCMS_CUDA(cudaDeviceGetAttribute(&count, cudaDevAttrMultiProcessorCount, dev));
+    if (major != 10) return fail(HCMS_ERR_UNSUPPORTED_DEVICE, "device %d is sm_%dx; libhcms is built for sm_100a only", dev, major);
+    cached = count;
+  }
+  *sms = cached;
+  return HCMS_OK;
+}
+
+static int run_gemm(const GemmArgs& g, cudaStream_t st, const char* what) {
+  cudaError_t e = launch_gemm(g, st);
+  if (e != cudaSuccess) return fail_cuda(e, what);
+  return HCMS_OK;
+}
+
+extern "C" {
+
+int hcms_gemm_bf16_nt(const void* a, const void* b, void* c, int64_t M, int N, int K, void* stream) {
+  if (!a || !b || !c) return fail(HCMS_ERR_INVALID_ARG, "NULL argument");
+  if (M <= 0 || N <= 0 || K <= 0) return fail(HCMS_ERR_INVALID_ARG, "M=%lld N=%d K=%d must be positive", static_cast<long long>(M), N, K);
+  if (M > (1ll << 30)) return fail(HCMS_ERR_UNSUPPORTED_SHAPE, "M=%lld too large", static_cast<long long>(M));
+  if (K % 8 || N % 128) return fail(HCMS_ERR_UNSUPPORTED_SHAPE, "need K %% 8 == 0 and N %% 128 == 0 (K=%d, N=%d)", K, N);
+  if (!aligned16(a) || !aligned16(b) || !aligned16(c)) return fail(HCMS_ERR_MISALIGNED, "a, b and c must be 16-byte aligned");
+  const size_t nc = static_cast<size_t>(M) * N * 2;
+  if (overlaps(c, nc, a, static_cast<size_t>(M) * K * 2) || overlaps(c, nc, b, static_cast<size_t>(N) * K * 2))
+    return fail(HCMS_ERR_ALIAS, "c overlaps an operand");
+  int sms = 0;
+  int st = device_sms(&sms);
+  if (st) return st;
+  GemmArgs g{};
+  g.a = a;
+  g.b = b;
+  g.out[0] = c;
+  g.M = M;
+  g.N = N;
+  g.K = K;
+  g.n_per_out = N;
+  g.rope_outs = 0;
+  g.D = 128;
+  g.num_sms = sms;
+  return run_gemm(g, static_cast<cudaStream_t>(stream), "gemm launch");
+}
+
+static int check_layer_shape(const hcms_plan_t* plan, int Dm) {
+  if (plan->dtype != HCMS_DTYPE_BF16) return fail(HCMS_ERR_UNSUPPORTED_DTYPE, "the projections need a bf16 plan");
+  if (Dm <= 0) return fail(HCMS_ERR_INVALID_ARG, "Dm=%d must be positive", Dm);
+  if (Dm % 128) return fail(HCMS_ERR_UNSUPPORTED_SHAPE, "Dm=%d must be a multiple of 128", Dm);
+  if ((plan->sh.H * plan->sh.D) % 128) return fail(HCMS_ERR_UNSUPPORTED_SHAPE, "H*D=%d must be a multiple of 128", plan->sh.H * plan->sh.D);
+  return HCMS_OK;
+}
+
+int hcms_qkv_projection_rope(hcms_plan_t* plan, const void* x, const void* w_qkv, const void* rope_cos,
+                             const void* rope_sin, void* q, void* k, void* v, int Dm, void* stream) {
+  if (!plan || !x || !w_qkv || !q || !k || !v) return fail(HCMS_ERR_INVALID_ARG, "NULL argument");
+  if ((rope_cos == nullptr) != (rope_sin == nullptr)) return fail(HCMS_ERR_INVALID_ARG, "pass both RoPE tables or neither");
+  int st = check_layer_shape(plan, Dm);
+  if (st) return st;
+  for (const void* ptr : {x, w_qkv, rope_cos, rope_sin, static_cast<const void*>(q), static_cast<const void*>(k), static_cast<const void*>(v)})
+    if (!aligned16(ptr)) return fail(HCMS_ERR_MISALIGNED, "every pointer must be 16-byte aligned");
+  const Shape& sh = plan->sh;
+  GemmArgs g{};
+  g.a = x;
+  g.b = w_qkv;
+  g.out[0] = q;
+  g.out[1] = k;
+  g.out[2] = v;
+  g.M = sh.S;
+  g.N = 3 * sh.H * sh.D;
+  g.K = Dm;
+  g.n_per_out = sh.H * sh.D;
+  g.rope_outs = rope_cos ? 2 : 0;
+  g.D = sh.D;
+  g.cos = static_cast<const float*>(rope_cos);
+  g.sin = static_cast<const float*>(rope_sin);
+  g.num_sms = plan->num_sms;
+  return run_gemm(g, static_cast<cudaStream_t>(stream), "QKV projection launch");
+}
+
+int hcms_output_projection(hcms_plan_t* plan, const void* o, const void* w_o, void* y, int Dm, void* stream) {
+  if (!plan || !o || !w_o || !y) return fail(HCMS_ERR_INVALID_ARG, "NULL argument");
+  int st = check_layer_shape(plan, Dm);
+  if (st) return st;
+  if (!aligned16(o) || !aligned16(w_o) || !aligned16(y)) return fail(HCMS_ERR_MISALIGNED, "every pointer must be 16-byte aligned");
+  const Shape& sh = plan->sh;
+  GemmArgs g{};
+  g.a = o;
+  g.b = w_o;
+  g.out[0] = y;
+  g.M = sh.S;
+  g.N = Dm;
+  g.K = sh.H * sh.D;
+  g.n_per_out = Dm;
+  g.rope_outs = 0;
+  g.D = sh.D;
+  g.num_sms = plan->num_sms;
+  return run_gemm(g, static_cast<cudaStream_t>(stream), "output projection launch");
+}
+
+int hcms_layer_forward(hcms_plan_t* plan, const void* x, const void* w_qkv, const void* w_o, const void* rope_cos,
+                       const void* rope_sin, void* y, int64_t S, int Dm, int H, int D, int P, int C, float scale,
+                       void* stream) {
+  if (!plan || !x || !w_qkv || !w_o || !y) return fail(HCMS_ERR_INVALID_ARG, "NULL argument");
+  const Shape& sh = plan->sh;
+  if (S != sh.S || H != sh.H || D != sh.D || P != sh.P || C != sh.C)
+    return fail(HCMS_ERR_PLAN_MISMATCH, "call shape differs from the plan's");
+  int st = check_layer_shape(plan, Dm);
+  if (st) return st;
+  const size_t xy_bytes = static_cast<size_t>(S) * Dm * 2;
+  if (overlaps(x, xy_bytes, y, xy_bytes)) return fail(HCMS_ERR_ALIAS, "y overlaps x");
+  const size_t bytes = static_cast<size_t>(S) * H * D * sh.es;
+  for (auto& b : plan->layer_buf)
+    if (!b) HCMS_CUDA(cudaMalloc(&b, bytes));
+  cudaStream_t caller = static_cast<cudaStream_t>(stream);
+  const bool profile = plan->flags & HCMS_FLAG_PROFILE;
+  if (profile) HCMS_CUDA(cudaEventRecord(plan->e_layer[0], caller));
+  st = hcms_qkv_projection_rope(plan, x, w_qkv, rope_cos, rope_sin, plan->layer_buf[0], plan->layer_buf[1],
+                                plan->layer_buf[2], Dm, stream);                        // lines 2-3
+  if (st) return st;
+  if (profile) HCMS_CUDA(cudaEventRecord(plan->e_layer[1], caller));
+  st = hcms_attention_forward(plan, plan->layer_buf[0], plan->layer_buf[1], plan->layer_buf[2], plan->layer_buf[3], S, H,
+                              D, P, C, scale, stream);                                  // lines 4-26
+  if (st) return st;
+  const int hot_launches = plan->last_launches;
+  if (profile) HCMS_CUDA(cudaEventRecord(plan->e_layer[2], caller));
+  st = hcms_output_projection(plan, plan->layer_buf[3], w_o, y, Dm, stream);            // line 27
+  if (st) return st;
+  if (profile) {
+    HCMS_CUDA(cudaEventRecord(plan->e_layer[3], caller));
+    plan->layer_timed = true;
+  }
+  plan->last_launches = hot_launches + 2;
+  return HCMS_OK;
+}
+
+void* hcms_plan_layer_buffer(const hcms_plan_t* plan, int which) {
+  return (plan && which >= 0 && which < 4) ? plan->layer_buf[which] : nullptr;
+}
+
+int hcms_plan_layer_timings(hcms_plan_t* plan, float* qkv_ms, float* hcms_ms, float* out_ms) {
+  if (!plan) return fail(HCMS_ERR_INVALID_ARG, "plan is NULL");
+  if (!(plan->flags & HCMS_FLAG_PROFILE) || !plan->layer_timed)
+    return fail(HCMS_ERR_INVALID_ARG, "no hcms_layer_forward has run on this plan under HCMS_FLAG_PROFILE");
+  HCMS_CUDA(cudaEventSynchronize(plan->e_layer[3]));
+  float* outs[3] = {qkv_ms, hcms_ms, out_ms};
+  for (int i = 0; i < 3; ++i) {
+    float ms = 0.f;
+    HCMS_CUDA(cudaEventElapsedTime(&ms, plan->e_layer[i], plan->e_layer[i + 1]));
+    if (outs[i]) *outs[i] = ms;
+  }
   return HCMS_OK;
 }
 

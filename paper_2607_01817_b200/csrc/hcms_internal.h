@@ -64,6 +64,23 @@ struct AttnArgs {
 cudaError_t launch_attention(const AttnArgs& a, cudaStream_t stream);
 cudaError_t attention_init();  // sets kernel attributes once; resolves cuTensorMapEncodeTiled
 
+// ---- projection GEMMs (gemm_bf16.cu): C[M,N] = A[M,K] * B[N,K]^T, bf16 -> fp32 -> bf16 -------
+struct GemmArgs {
+  const void* a;       // [M, K] bf16, row-major
+  const void* b;       // [N, K] bf16, row-major (torch.nn.Linear weight)
+  void* out[3];        // N / n_per_out output tensors, each [M, n_per_out] bf16 row-major
+  int64_t M;
+  int N, K;
+  int n_per_out;       // multiple of 128; N for a plain GEMM, H*D for the QKV projection
+  int rope_outs;       // RoPE on the first rope_outs outputs (0 = none)
+  int D;               // head dimension (RoPE only): 64 or 128
+  const float* cos;    // [M, D/2] fp32 (RoPE only)
+  const float* sin;
+  int num_sms;
+};
+cudaError_t launch_gemm(const GemmArgs& a, cudaStream_t stream);
+cudaError_t gemm_init();
+
 // ---- driver entry point for tensor maps (tma_desc.cu) ------------------------------------
 // dims/strides innermost first; strides[0] is implied (element size). Returns cudaSuccess or an error.
 cudaError_t encode_tensor_map(CUtensorMap* out, CUtensorMapDataType dt, int rank, const void* base,
