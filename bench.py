@@ -61,6 +61,7 @@ def parse_args(argv=None):
     ap.add_argument("--single-comp", action="store_true", help="HCMS_FLAG_SINGLE_COMP: one compute stream, as Alg. 1")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-layer", action="store_true", help="skip the whole-layer (Alg. 1 lines 2-27) measurement")
     ap.add_argument("--cpu-rows", type=int, default=512, help="query rows per head in the cpu_baseline sample")
     ap.add_argument("--ref-rows", type=int, default=96, help="query rows per head per step for --impl reference")
     return ap.parse_args(argv)
@@ -212,6 +213,48 @@ def time_oracle_sample(w, q, k, v, rows) -> float:
 # ---------------------------------------------------------------------------------------------
 
 L2_BYTES = 126 * 1024 * 1024
+
+
+def measure_layer(args, H, torch, dev, w, C, base_flags, timed, pk, threads):
+    """hcms_layer_forward on seeded activations / random-init weights of the workload's shape (Dm = H*D, Table 3
+    L210-215): layer ms, the three parts from the events HCMS_FLAG_PROFILE records on the caller's stream, and
+    the projection kernels' TFLOP/s against the measured sustained bf16 peak."""
+    S, Hh, D, P = w.S, w.H, w.D, w.P
+    Dm = Hh * D
+    arrs = I.make_layer_inputs(w, threads=threads)
+    x, wq, wo = (torch.from_numpy(t.view(np.int16)).to(dev) for t in arrs[:3])
+    cos, sin = (torch.from_numpy(t).to(dev) for t in arrs[3:])
+    y = torch.empty((S, Dm), dtype=torch.int16, device=dev)
+    plan = H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, base_flags)
+    step = lambda: H.hcms_layer_forward(plan, x, wq, wo, cos, sin, y, Dm, w.scale)
+    n = max(3, min(args.steps, 10))
+    for _ in range(3):
+        step()
+    torch.cuda.synchronize()
+    parts = np.zeros(3)
+    total = 0.0
+    for _ in range(n):                       # per-call events: the part timings belong to the call just made
+        total += timed(plan, 1, step)
+        parts += np.asarray(H.hcms_plan_layer_timings(plan))
+    ms, parts = total / n, parts / n
+    launches = H.hcms_plan_last_launch_count(plan)
+    plan.close()
+    qkv_flop, out_flop, attn_flop = 2.0 * S * Dm * 3 * Hh * D, 2.0 * S * Hh * D * Dm, 4.0 * S * S * D * Hh
+    gemm_tf = (qkv_flop + out_flop) / ((parts[0] + parts[2]) * 1e-3) / 1e12
+    return {
+        "what": "hcms_layer_forward: QKV projection + RoPE -> HCMS chunk pipeline -> output projection (Alg. 1 lines 2-27)",
+        "Dm": Dm, "ms_per_layer": round(ms, 4), "steps": n, "launches_per_layer": launches,
+        "qkv_rope_ms": round(float(parts[0]), 4), "hcms_ms": round(float(parts[1]), 4), "out_proj_ms": round(float(parts[2]), 4),
+        "qkv_rope_tflops": round(qkv_flop / (parts[0] * 1e-3) / 1e12, 1),
+        "out_proj_tflops": round(out_flop / (parts[2] * 1e-3) / 1e12, 1),
+        "layer_tflops": round((qkv_flop + out_flop + attn_flop) / (ms * 1e-3) / 1e12, 1),
+        "gemm_roofline": {"kernel": "gemm_bf16_nt_kernel<256>", "bound": "tensor", "achieved": round(gemm_tf, 1),
+                          "peak": pk["bf16_tflops_sustained"], "unit": "TFLOP/s",
+                          "frac": round(gemm_tf / pk["bf16_tflops_sustained"], 4),
+                          "frac_of_nominal": round(gemm_tf / NOMINAL_BF16_TFLOPS, 4)},
+        "t_other_share": round(float(parts[0] + parts[2]) / ms, 4),
+        "weights": "random init N(0, 1/fan_in) -> bf16, RoPE tables s*10000^(-2i/D) (hcms_inputs.make_layer_inputs)",
+    }
 
 
 def run_hcms(args):
@@ -372,6 +415,10 @@ def run_hcms(args):
         same = bool(torch.equal(host_out.to(dev), out))
         result["e2e"]["bitwise_equal_to_device_path"] = same
         plan_e.close()
+
+    # ---- the whole attention layer, Alg. 1 lines 2-27: projections + RoPE around the hot path ----
+    if not args.no_layer:
+        result["layer_full"] = measure_layer(args, H, torch, dev, w, C, base_flags, timed, pk, threads)
 
     # ---- the oracle on the host cores (rank 0, N = 1 only) -----------------------------------
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
