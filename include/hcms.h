@@ -40,7 +40,7 @@
 extern "C" {
 #endif
 
-#define HCMS_VERSION 200 /* major*10000 + minor*100 + patch */
+#define HCMS_VERSION 300 /* major*10000 + minor*100 + patch */
 
 /* ---- status codes ------------------------------------------------------------------- */
 enum {
@@ -86,6 +86,12 @@ enum {
                                           alternate by chunk parity, so that chunk c+1's thread blocks fill
                                           the SMs vacated by the last (partial) wave of chunk c; the event
                                           dependencies of Eq. 6-7 are unchanged and so are the bits. */
+
+#define HCMS_FLAG_TRAINING 0x800u      /* the plan also serves the backward pass (L304, Table 15): its
+                                          workspace doubles (dO'_c, dQ'_c, dK'_c, dV'_c per chunk), and
+                                          hcms_attention_forward saves the row statistic lse_i = log sum_k
+                                          exp(scale q_i.k_k) of every head (H*S floats) and keeps Q'_c, K'_c,
+                                          V'_c, O'_c for hcms_attention_backward */
 
 typedef struct hcms_plan hcms_plan_t;
 
@@ -303,6 +309,43 @@ void* hcms_plan_layer_buffer(const hcms_plan_t* plan, int which);
  * lines 4-26 (all-to-alls and attention), output projection.  Any pointer may be NULL.  SYNCHRONISES the
  * host with those events.  Errors: INVALID_ARG (no profiled layer call yet), CUDA. */
 int hcms_plan_layer_timings(hcms_plan_t* plan, float* qkv_ms, float* hcms_ms, float* out_ms);
+
+/* ---- backward of the hot path ----------------------------------------------- */
+/*
+ * "HCMS is compatible with PyTorch autograd ... forward+backward combined execution" (L304; Table 15
+ * L479-483; future work L346).  Autograd differentiates Alg. 1; the all-to-alls are permutations, so the
+ * backward of lines 4-26 is the same pipeline run on the gradients: per head chunk c
+ *     input all-to-all of dO (scatter)  ->  attention backward on every rank's heads  ->  output all-to-all
+ *     of dQ'_c, dK'_c, dV'_c (one gather launch for the three),
+ * with chunk c+1's all-to-all on S_comm overlapping chunk c's attention backward on S_comp, ordered by the
+ * same events E_main, E_c^comm, E_c^comp (Eq. 6-7).  Per head, with P = softmax(scale Q K^T):
+ *     dV = P^T dO,  dP = dO V^T,  dS = P o (dP - rowsum(dO o O)),  dQ = scale dS K,  dK = scale dS^T Q.
+ * P is recomputed from the saved lse; two deterministic tcgen05 passes (dK/dV, then dQ) without atomics, so
+ * the gradients are bitwise independent of P and C.  bf16 operands (P, dS rounded to bf16 for the MMAs), fp32
+ * accumulation, bf16 gradients.
+ *
+ * hcms_attention_backward: `plan` must carry HCMS_FLAG_TRAINING and the last hcms_attention_forward on it must
+ * be the forward being differentiated (its Q'_c, K'_c, V'_c, O'_c and lse are read from the workspace; `scale`
+ * must be the same).  dout: device [S,H,D] bf16 = dL/d(out); dq, dk, dv: device [S,H,D] bf16, distinct, not
+ * overlapping dout.  Asynchronous on `stream` like the forward.  HCMS_FLAG_SERIAL runs it on `stream` alone.
+ * Errors: INVALID_ARG (NULL, plan without TRAINING, no forward yet), PLAN_MISMATCH, MISALIGNED, ALIAS, CUDA.
+ */
+int hcms_attention_backward(hcms_plan_t* plan, const void* dout, void* dq, void* dk, void* dv, int64_t S, int H,
+                            int D, int P, int C, float scale, void* stream);
+/*
+ * Single steps on caller-supplied chunk buffers ([P][S][h_c][D] bf16 unless stated; chunk c of the plan):
+ * hcms_attention_chunk_lse = hcms_attention_chunk that also writes lse: device [P*h_c][S] fp32, natural log.
+ * hcms_attention_backward_chunk: qc,kc,vc,oc,doc and lse in, dqc,dkc,dvc out (3 launches: delta/lse packing,
+ * dK/dV pass, dQ pass); works on any bf16 plan (scratch for the packed statistics is allocated on first use).
+ */
+int hcms_attention_chunk_lse(hcms_plan_t* plan, const void* qc, const void* kc, const void* vc, void* oc, void* lse,
+                             int c, float scale, void* stream);
+int hcms_attention_backward_chunk(hcms_plan_t* plan, const void* qc, const void* kc, const void* vc, const void* oc,
+                                  const void* doc, const void* lse, void* dqc, void* dkc, void* dvc, int c,
+                                  float scale, void* stream);
+/* Device address of the lse the last forward saved on a TRAINING plan: [H][S] fp32 in the order chunk 0's
+ * P*h_0 heads (p-major), chunk 1's, ...; NULL otherwise.  For tests. */
+void* hcms_plan_lse(const hcms_plan_t* plan);
 
 #ifdef __cplusplus
 }

@@ -41,6 +41,7 @@ HCMS_FLAG_HOST_ROUTE_O = 0x80
 HCMS_FLAG_DEBUG_NO_COMM_WAIT = 0x100
 HCMS_FLAG_PROFILE = 0x200
 HCMS_FLAG_SINGLE_COMP = 0x400
+HCMS_FLAG_TRAINING = 0x800
 
 # every symbol include/hcms.h declares: name -> (restype, argtypes)
 _SIGNATURES = {
@@ -77,6 +78,10 @@ _SIGNATURES = {
     "hcms_layer_forward": (c_int, [c_void_p] * 7 + [c_int64, c_int, c_int, c_int, c_int, c_int, c_float, c_void_p]),
     "hcms_plan_layer_buffer": (c_void_p, [c_void_p, c_int]),
     "hcms_plan_layer_timings": (c_int, [c_void_p, POINTER(c_float), POINTER(c_float), POINTER(c_float)]),
+    "hcms_attention_backward": (c_int, [c_void_p] * 5 + [c_int64, c_int, c_int, c_int, c_int, c_float, c_void_p]),
+    "hcms_attention_chunk_lse": (c_int, [c_void_p] * 6 + [c_int, c_float, c_void_p]),
+    "hcms_attention_backward_chunk": (c_int, [c_void_p] * 10 + [c_int, c_float, c_void_p]),
+    "hcms_plan_lse": (c_void_p, [c_void_p]),
 }
 
 
@@ -360,3 +365,27 @@ def hcms_plan_layer_timings(plan: Plan):
     vals = [c_float() for _ in range(3)]
     _check(lib.hcms_plan_layer_timings(plan.handle, *[ctypes.byref(v) for v in vals]), "hcms_plan_layer_timings")
     return tuple(float(v.value) for v in vals)
+
+
+# ---- backward of the hot path -----------------------------------------------------
+
+def hcms_attention_backward(plan: Plan, dout, dq, dk, dv, scale: float, stream=None) -> None:
+    """Gradients of the last hcms_attention_forward on a HCMS_FLAG_TRAINING plan; device [S,H,D] bf16 tensors."""
+    _check(lib.hcms_attention_backward(plan.handle, _ptr(dout), _ptr(dq), _ptr(dk), _ptr(dv), plan.S, plan.H, plan.D,
+                                       plan.P, plan.C, scale, _stream(stream)), "hcms_attention_backward")
+
+
+def hcms_attention_chunk_lse(plan: Plan, qc, kc, vc, oc, lse, c: int, scale: float, stream=None) -> None:
+    _check(lib.hcms_attention_chunk_lse(plan.handle, _ptr(qc), _ptr(kc), _ptr(vc), _ptr(oc), _ptr(lse), c, scale,
+                                        _stream(stream)), "hcms_attention_chunk_lse")
+
+
+def hcms_attention_backward_chunk(plan: Plan, qc, kc, vc, oc, doc, lse, dqc, dkc, dvc, c: int, scale: float,
+                                  stream=None) -> None:
+    _check(lib.hcms_attention_backward_chunk(plan.handle, _ptr(qc), _ptr(kc), _ptr(vc), _ptr(oc), _ptr(doc), _ptr(lse),
+                                             _ptr(dqc), _ptr(dkc), _ptr(dvc), c, scale, _stream(stream)),
+           "hcms_attention_backward_chunk")
+
+
+def hcms_plan_lse(plan: Plan) -> int:
+    return lib.hcms_plan_lse(plan.handle) or 0

@@ -93,6 +93,7 @@ struct AttnParams {
   int n_kv;          // ceil(S/128)
   int h_c;
   float scale_log2;  // scale * log2(e)
+  float* lse;        // optional [P*h_c][S]: log sum_k exp(scale q.k) per query row (natural log), for the backward
 };
 
 // ---- packed fp32x2 arithmetic (FFMA2 / FADD2 on sm_100) and helpers ----------------------------------
@@ -471,7 +472,11 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
     float la, lb, lc, ld;
     unpack2(l2, la, lb);
     unpack2(l2b, lc, ld);
-    const float inv_l = 1.0f / ((la + lb) + (lc + ld));
+    const float l_sum = (la + lb) + (lc + ld);
+    const float inv_l = 1.0f / l_sum;
+    if (prm.lse != nullptr && q_row0 + t * kBM + row < prm.S)      // sum_k exp(s_k) = l * exp(m): lse = m*scale + log l
+      prm.lse[static_cast<size_t>(head) * prm.S + q_row0 + t * kBM + row] =
+          (m_run * scale_log2 + log2f(l_sum)) * 0.6931471805599453f;
     const uint32_t o_smem = p_smem + t * kPTileBytes;     // PV_t(n_kv-1) has finished reading it
 #pragma unroll
     for (int c4 = 0; c4 < D / 32; ++c4) {
@@ -577,6 +582,7 @@ cudaError_t launch_attention(const AttnArgs& a, cudaStream_t stream) {
   // scale == 0 is legal (uniform softmax); a tiny positive factor keeps (-inf)*scale_log2 = -inf for
   // masked tail keys while exp2(s*1e-30) is exactly 1 in fp32.
   prm.scale_log2 = fmaxf(a.scale * 1.4426950408889634f, 1e-30f);
+  prm.lse = a.lse;
   dim3 grid(static_cast<unsigned>((a.S + kQTiles * kBM - 1) / (kQTiles * kBM)), static_cast<unsigned>(a.P * a.h_c));
   const int poly = poly_setting();
   if (a.D == 128)

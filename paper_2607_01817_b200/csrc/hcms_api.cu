@@ -75,6 +75,11 @@ struct hcms_plan {
   void* layer_buf[4] = {nullptr, nullptr, nullptr, nullptr};
   cudaEvent_t e_layer[4] = {nullptr, nullptr, nullptr, nullptr};
   bool layer_timed = false;
+  // HCMS_FLAG_TRAINING: gradient chunk buffers dO'_c, dQ'_c, dK'_c, dV'_c (same offsets as the forward's), lse [H][S]
+  void* train_ws = nullptr;
+  float* lse = nullptr;
+  void* stats = nullptr;      // packed {lse*log2e, delta}: [H][s_pad] float2 (lazily allocated)
+  bool forward_done = false;
   // HCMS_FLAG_PROFILE: [step 0=scatter,1=attention,2=gather][begin,end][ring slot * C + chunk]
   std::vector<cudaEvent_t> prof[3][2];
   long long prof_calls = 0;   // forward calls that recorded a full set of events
@@ -110,6 +115,9 @@ static void plan_free(hcms_plan_t* p) {
     if (d) cudaFree(d);
   for (auto& d : p->layer_buf)
     if (d) cudaFree(d);
+  if (p->train_ws) cudaFree(p->train_ws);
+  if (p->lse) cudaFree(p->lse);
+  if (p->stats) cudaFree(p->stats);
   for (auto& e : p->e_layer)
     if (e) cudaEventDestroy(e);
   delete p;
@@ -269,6 +277,12 @@ int hcms_plan(hcms_plan_t** out, int64_t S, int H, int D, int P, int C, int dtyp
   PLAN_CUDA(cudaMalloc(&p->ws, p->ws_bytes));
   p->ws_owned = true;
   if (dtype == HCMS_DTYPE_BF16) PLAN_CUDA(attention_init());
+  if (dtype == HCMS_DTYPE_BF16) PLAN_CUDA(attention_bwd_init());
+  if (flags & HCMS_FLAG_TRAINING) {
+    if (dtype != HCMS_DTYPE_BF16) return bail(fail(HCMS_ERR_UNSUPPORTED_DTYPE, "HCMS_FLAG_TRAINING needs a bf16 plan"));
+    PLAN_CUDA(cudaMalloc(&p->train_ws, p->ws_bytes));
+    PLAN_CUDA(cudaMalloc(reinterpret_cast<void**>(&p->lse), static_cast<size_t>(H) * S * sizeof(float)));
+  }
   if (flags & (HCMS_FLAG_HOST_ROUTE_Q | HCMS_FLAG_HOST_ROUTE_K | HCMS_FLAG_HOST_ROUTE_V | HCMS_FLAG_HOST_ROUTE_O)) {
     size_t max_chunk = 0;
     for (auto& ck : p->chunks) max_chunk = ck.bytes > max_chunk ? ck.bytes : max_chunk;
@@ -364,9 +378,10 @@ static int do_layout(hcms_plan_t* p, int n, const void* const* src, void* const*
 }
 
 static int do_attention(hcms_plan_t* p, const void* qc, const void* kc, const void* vc, void* oc, int c, float scale,
-                        cudaStream_t st) {
+                        cudaStream_t st, float* lse = nullptr) {
   const Chunk& ck = p->chunks[c];
   AttnArgs a{qc, kc, vc, oc, p->sh.S, p->sh.D, p->sh.P, ck.h, scale};
+  a.lse = lse;
   cudaError_t e = launch_attention(a, st);
   if (e != cudaSuccess) return fail_cuda(e, "attention launch");
   p->last_launches += 1;
@@ -497,7 +512,8 @@ int hcms_attention_forward(hcms_plan_t* plan, const void* q, const void* k, cons
     if (!serial && !(plan->flags & HCMS_FLAG_DEBUG_NO_COMM_WAIT))
       HCMS_CUDA(cudaStreamWaitEvent(s_comp, plan->e_comm[c], 0));
     HCMS_CUDA(mark(1, c, 0, s_comp));
-    st = do_attention(plan, ws + ck.off[0], ws + ck.off[1], ws + ck.off[2], ws + ck.off[3], c, scale, s_comp);
+    float* lse_c = plan->lse ? plan->lse + static_cast<size_t>(sh.P) * sh.S * ck.o : nullptr;   // chunk c: [P*h_c][S]
+    st = do_attention(plan, ws + ck.off[0], ws + ck.off[1], ws + ck.off[2], ws + ck.off[3], c, scale, s_comp, lse_c);
     if (st) return st;
     HCMS_CUDA(mark(1, c, 1, s_comp));
     if (!serial) HCMS_CUDA(cudaEventRecord(plan->e_comp[c], s_comp));  // E_c^comp
@@ -518,6 +534,7 @@ int hcms_attention_forward(hcms_plan_t* plan, const void* q, const void* k, cons
     HCMS_CUDA(mark(2, c, 1, s_out));
   }
   if (profile) plan->prof_calls += 1;
+  plan->forward_done = true;
   if (!serial) {
     // line 25: Synchronize(S_comm, S_comp) -- expressed as stream waits, the host is not blocked
     HCMS_CUDA(cudaEventRecord(plan->e_fin_comm, s_out));
@@ -835,6 +852,161 @@ int hcms_plan_layer_timings(hcms_plan_t* plan, float* qkv_ms, float* hcms_ms, fl
     float ms = 0.f;
     HCMS_CUDA(cudaEventElapsedTime(&ms, plan->e_layer[i], plan->e_layer[i + 1]));
     if (outs[i]) *outs[i] = ms;
+  }
+  return HCMS_OK;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------
+// backward of the hot path: the same chunk pipeline on the gradients
+// ------------------------------------------------------------------------------------------
+static int ensure_stats(hcms_plan_t* p) {
+  if (!p->stats) HCMS_CUDA(cudaMalloc(&p->stats, attention_bwd_stats_bytes(p->sh.S, p->sh.H)));
+  return HCMS_OK;
+}
+
+// chunk c's slice of the packed statistics: heads are laid out chunk by chunk like the lse
+static void* stats_of_chunk(hcms_plan_t* p, int c) {
+  const size_t per_head = attention_bwd_stats_bytes(p->sh.S, 1);
+  return static_cast<char*>(p->stats) + per_head * p->sh.P * p->chunks[c].o;
+}
+
+static int do_attention_bwd(hcms_plan_t* p, const void* qc, const void* kc, const void* vc, const void* oc,
+                            const void* doc, const float* lse, void* dqc, void* dkc, void* dvc, int c, float scale,
+                            cudaStream_t st) {
+  AttnBwdArgs a{};
+  a.q = qc;
+  a.k = kc;
+  a.v = vc;
+  a.o = oc;
+  a.d_o = doc;
+  a.lse = lse;
+  a.dq = dqc;
+  a.dk = dkc;
+  a.dv = dvc;
+  a.stats = stats_of_chunk(p, c);
+  a.S = p->sh.S;
+  a.D = p->sh.D;
+  a.P = p->sh.P;
+  a.h_c = p->chunks[c].h;
+  a.scale = scale;
+  cudaError_t e = launch_attention_bwd(a, st);
+  if (e != cudaSuccess) return fail_cuda(e, "attention backward launch");
+  p->last_launches += 3;
+  return HCMS_OK;
+}
+
+extern "C" {
+
+void* hcms_plan_lse(const hcms_plan_t* plan) { return plan ? plan->lse : nullptr; }
+
+int hcms_attention_chunk_lse(hcms_plan_t* plan, const void* qc, const void* kc, const void* vc, void* oc, void* lse,
+                             int c, float scale, void* stream) {
+  if (!plan || !qc || !kc || !vc || !oc || !lse) return fail(HCMS_ERR_INVALID_ARG, "NULL argument");
+  if (plan->dtype != HCMS_DTYPE_BF16) return fail(HCMS_ERR_UNSUPPORTED_DTYPE, "attention needs a bf16 plan");
+  if (c < 0 || c >= plan->sh.C) return fail(HCMS_ERR_PLAN_MISMATCH, "chunk %d outside [0,%d)", c, plan->sh.C);
+  if (!aligned16(qc) || !aligned16(kc) || !aligned16(vc) || !aligned16(oc) || !aligned16(lse))
+    return fail(HCMS_ERR_MISALIGNED, "pointer is not 16-byte aligned");
+  int st = check_scale(scale);
+  if (st) return st;
+  plan->last_launches = 0;
+  return do_attention(plan, qc, kc, vc, oc, c, scale, static_cast<cudaStream_t>(stream), static_cast<float*>(lse));
+}
+
+int hcms_attention_backward_chunk(hcms_plan_t* plan, const void* qc, const void* kc, const void* vc, const void* oc,
+                                  const void* doc, const void* lse, void* dqc, void* dkc, void* dvc, int c,
+                                  float scale, void* stream) {
+  if (!plan || !qc || !kc || !vc || !oc || !doc || !lse || !dqc || !dkc || !dvc)
+    return fail(HCMS_ERR_INVALID_ARG, "NULL argument");
+  if (plan->dtype != HCMS_DTYPE_BF16) return fail(HCMS_ERR_UNSUPPORTED_DTYPE, "attention needs a bf16 plan");
+  if (c < 0 || c >= plan->sh.C) return fail(HCMS_ERR_PLAN_MISMATCH, "chunk %d outside [0,%d)", c, plan->sh.C);
+  for (const void* ptr : {qc, kc, vc, oc, doc, lse, static_cast<const void*>(dqc), static_cast<const void*>(dkc),
+                          static_cast<const void*>(dvc)})
+    if (!aligned16(ptr)) return fail(HCMS_ERR_MISALIGNED, "pointer is not 16-byte aligned");
+  int st = check_scale(scale);
+  if (st) return st;
+  st = ensure_stats(plan);
+  if (st) return st;
+  plan->last_launches = 0;
+  return do_attention_bwd(plan, qc, kc, vc, oc, doc, static_cast<const float*>(lse), dqc, dkc, dvc, c, scale,
+                          static_cast<cudaStream_t>(stream));
+}
+
+int hcms_attention_backward(hcms_plan_t* plan, const void* dout, void* dq, void* dk, void* dv, int64_t S, int H, int D,
+                            int P, int C, float scale, void* stream) {
+  if (!plan || !dout || !dq || !dk || !dv) return fail(HCMS_ERR_INVALID_ARG, "NULL argument");
+  const Shape& sh = plan->sh;
+  if (S != sh.S || H != sh.H || D != sh.D || P != sh.P || C != sh.C)
+    return fail(HCMS_ERR_PLAN_MISMATCH, "call shape differs from the plan's");
+  if (!(plan->flags & HCMS_FLAG_TRAINING) || !plan->train_ws || !plan->lse)
+    return fail(HCMS_ERR_INVALID_ARG, "the plan was made without HCMS_FLAG_TRAINING");
+  if (!plan->forward_done) return fail(HCMS_ERR_INVALID_ARG, "no hcms_attention_forward has run on this plan");
+  int st = check_scale(scale);
+  if (st) return st;
+  if (!aligned16(dout) || !aligned16(dq) || !aligned16(dk) || !aligned16(dv))
+    return fail(HCMS_ERR_MISALIGNED, "dout, dq, dk and dv must be 16-byte aligned");
+  const size_t bytes = static_cast<size_t>(S) * H * D * sh.es;
+  const void* all[4] = {dout, dq, dk, dv};
+  for (int i = 0; i < 4; ++i)
+    for (int j = i + 1; j < 4; ++j)
+      if (overlaps(all[i], bytes, all[j], bytes)) return fail(HCMS_ERR_ALIAS, "dout, dq, dk, dv must not overlap");
+  if (!plan->ws) return fail(HCMS_ERR_WORKSPACE_TOO_SMALL, "plan has no workspace");
+  st = ensure_stats(plan);
+  if (st) return st;
+
+  cudaStream_t caller = static_cast<cudaStream_t>(stream);
+  const bool serial = plan->flags & HCMS_FLAG_SERIAL;
+  cudaStream_t s_comm = serial ? caller : plan->s_comm;
+  const bool dual_comp = !serial && !(plan->flags & HCMS_FLAG_SINGLE_COMP) && sh.C > 1;
+  auto comp_stream = [&](int c) { return serial ? caller : ((dual_comp && (c & 1)) ? plan->s_comp2 : plan->s_comp); };
+  char* ws = static_cast<char*>(plan->ws);          // Q'_c, K'_c, V'_c, O'_c saved by the forward
+  char* gw = static_cast<char*>(plan->train_ws);    // dO'_c at off[3], dQ'_c, dK'_c, dV'_c at off[0..2]
+  plan->last_launches = 0;
+  if (!serial) {
+    HCMS_CUDA(cudaEventRecord(plan->e_main, caller));
+    HCMS_CUDA(cudaStreamWaitEvent(s_comm, plan->e_main, 0));
+    HCMS_CUDA(cudaStreamWaitEvent(plan->s_comp, plan->e_main, 0));
+    if (dual_comp) HCMS_CUDA(cudaStreamWaitEvent(plan->s_comp2, plan->e_main, 0));
+  }
+  // input all-to-all of the incoming gradient, every chunk, on S_comm
+  for (int c = 0; c < sh.C; ++c) {
+    const Chunk& ck = plan->chunks[c];
+    const void* src[1] = {dout};
+    void* dst[1] = {gw + ck.off[3]};
+    st = do_layout(plan, 1, src, dst, c, false, s_comm);
+    if (st) return st;
+    if (!serial) HCMS_CUDA(cudaEventRecord(plan->e_comm[c], s_comm));
+  }
+  // attention backward per chunk on S_comp
+  for (int c = 0; c < sh.C; ++c) {
+    const Chunk& ck = plan->chunks[c];
+    cudaStream_t s_comp = comp_stream(c);
+    if (!serial) HCMS_CUDA(cudaStreamWaitEvent(s_comp, plan->e_comm[c], 0));
+    const float* lse_c = plan->lse + static_cast<size_t>(sh.P) * sh.S * ck.o;
+    st = do_attention_bwd(plan, ws + ck.off[0], ws + ck.off[1], ws + ck.off[2], ws + ck.off[3], gw + ck.off[3], lse_c,
+                          gw + ck.off[0], gw + ck.off[1], gw + ck.off[2], c, scale, s_comp);
+    if (st) return st;
+    if (!serial) HCMS_CUDA(cudaEventRecord(plan->e_comp[c], s_comp));
+  }
+  // output all-to-all of dQ'_c, dK'_c, dV'_c (one launch for the three) on S_comm
+  for (int c = 0; c < sh.C; ++c) {
+    const Chunk& ck = plan->chunks[c];
+    if (!serial) HCMS_CUDA(cudaStreamWaitEvent(s_comm, plan->e_comp[c], 0));
+    const void* src[3] = {gw + ck.off[0], gw + ck.off[1], gw + ck.off[2]};
+    void* dst[3] = {dq, dk, dv};
+    st = do_layout(plan, 3, src, dst, c, true, s_comm);
+    if (st) return st;
+  }
+  if (!serial) {
+    HCMS_CUDA(cudaEventRecord(plan->e_fin_comm, s_comm));
+    HCMS_CUDA(cudaEventRecord(plan->e_fin_comp, plan->s_comp));
+    HCMS_CUDA(cudaStreamWaitEvent(caller, plan->e_fin_comm, 0));
+    HCMS_CUDA(cudaStreamWaitEvent(caller, plan->e_fin_comp, 0));
+    if (dual_comp) {
+      HCMS_CUDA(cudaEventRecord(plan->e_fin_comp2, plan->s_comp2));
+      HCMS_CUDA(cudaStreamWaitEvent(caller, plan->e_fin_comp2, 0));
+    }
   }
   return HCMS_OK;
 }

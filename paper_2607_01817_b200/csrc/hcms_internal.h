@@ -60,9 +60,30 @@ struct AttnArgs {
   int64_t S;
   int D, P, h_c;
   float scale;
+  float* lse = nullptr;   // optional [P*h_c][S] fp32: log sum_k exp(scale q.k) per row (saved for the backward)
 };
 cudaError_t launch_attention(const AttnArgs& a, cudaStream_t stream);
 cudaError_t attention_init();  // sets kernel attributes once; resolves cuTensorMapEncodeTiled
+
+// ---- attention backward (attention_bwd.cu) -------------------------------------------------
+struct AttnBwdArgs {
+  const void* q;       // [P][S][h_c][D] bf16, the chunk buffers the forward read
+  const void* k;
+  const void* v;
+  const void* o;       // the forward's output chunk
+  const void* d_o;     // dL/dO', same layout
+  const float* lse;    // [P*h_c][S] fp32, natural log, as the forward wrote it
+  void* dq;            // outputs, same layout as q
+  void* dk;
+  void* dv;
+  void* stats;         // scratch, attention_bwd_stats_bytes(S, P*h_c) bytes
+  int64_t S;
+  int D, P, h_c;
+  float scale;
+};
+cudaError_t launch_attention_bwd(const AttnBwdArgs& a, cudaStream_t stream);   // 3 launches
+cudaError_t attention_bwd_init();
+size_t attention_bwd_stats_bytes(int64_t S, int heads);
 
 // ---- projection GEMMs (gemm_bf16.cu): C[M,N] = A[M,K] * B[N,K]^T, bf16 -> fp32 -> bf16 -------
 struct GemmArgs {
