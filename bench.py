@@ -581,7 +581,7 @@ def run_timeline(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per attention launch summed over one step, from the
 # ncu --set full capture committed under profiles/ (bytes; None until captured for that config)
-ATTN_TRAFFIC = {}
+ATTN_TRAFFIC = {3: 1294.0e6}   # profiles/r1e_ncu_summary.md: 389.8 + 390.1 + 257.5 + 256.7 MB
 
 
 # ---------------------------------------------------------------------------------------------
