@@ -62,6 +62,7 @@ def parse_args(argv=None):
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-layer", action="store_true", help="skip the whole-layer (Alg. 1 lines 2-27) measurement")
+    ap.add_argument("--no-backward", action="store_true", help="skip the forward+backward (Table 15 analogue) measurement")
     ap.add_argument("--cpu-rows", type=int, default=512, help="query rows per head in the cpu_baseline sample")
     ap.add_argument("--ref-rows", type=int, default=96, help="query rows per head per step for --impl reference")
     return ap.parse_args(argv)
@@ -257,6 +258,42 @@ def measure_layer(args, H, torch, dev, w, C, base_flags, timed, pk, threads):
     }
 
 
+def measure_backward(args, H, torch, w, C, base_flags, timed, pk, qd, kd, vd, out):
+    """hcms_attention_forward + hcms_attention_backward on a HCMS_FLAG_TRAINING plan, dual-stream and serial
+    (the paper's Table 15 compares exactly these two for forward+backward).  The backward's algorithmic work is
+    5 contractions of 2*S^2*D flop per head (dV, dP, dQ, dK and the recomputed S); the two-pass design executes 7."""
+    S, Hh, D, P = w.S, w.H, w.D, w.P
+    dout = torch.from_numpy(I.f32_to_bf16_bits(I.normal_f32(w.seed, 6, S * Hh * D).reshape(S, Hh, D)).view(np.int16)).to(qd.device)
+    dq, dk, dv = (torch.empty_like(qd) for _ in range(3))
+    n = max(2, min(args.steps, 5))
+    res = {}
+    for name, extra in (("hcms", 0), ("serial", H.HCMS_FLAG_SERIAL)):
+        plan = H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, (base_flags & ~H.HCMS_FLAG_PROFILE) | H.HCMS_FLAG_TRAINING | extra)
+        fwd = lambda: H.hcms_attention_forward(plan, qd, kd, vd, out, w.scale)
+        bwd = lambda: H.hcms_attention_backward(plan, dout, dq, dk, dv, w.scale)
+        fwd(); bwd(); fwd(); bwd()
+        torch.cuda.synchronize()
+        t_f = t_b = 0.0
+        for _ in range(n):
+            t_f += timed(plan, 1, fwd)
+            t_b += timed(plan, 1, bwd)
+        res[name] = (t_f / n, t_b / n, H.hcms_plan_last_launch_count(plan))
+        plan.close()
+    f_ms, b_ms, launches = res["hcms"]
+    alg = 10.0 * S * S * D * Hh
+    return {
+        "what": "hcms_attention_forward + hcms_attention_backward (scatter dO -> dK/dV pass + dQ pass -> gather dQ,dK,dV per chunk)",
+        "steps": n, "fwd_ms": round(f_ms, 4), "bwd_ms": round(b_ms, 4), "fwd_bwd_ms": round(f_ms + b_ms, 4),
+        "serial_fwd_bwd_ms": round(res["serial"][0] + res["serial"][1], 4),
+        "speedup_vs_serial": round((res["serial"][0] + res["serial"][1]) / (f_ms + b_ms), 4),
+        "bwd_launches": launches,
+        "bwd_tflops_algorithmic": round(alg / (b_ms * 1e-3) / 1e12, 1),
+        "bwd_tflops_executed": round(1.4 * alg / (b_ms * 1e-3) / 1e12, 1),
+        "bwd_frac_of_sustained_peak": round(alg / (b_ms * 1e-3) / 1e12 / pk["bf16_tflops_sustained"], 4),
+        "fwd_bwd_tflops_algorithmic": round(3.5 * 4.0 * S * S * D * Hh / ((f_ms + b_ms) * 1e-3) / 1e12, 1),
+    }
+
+
 def run_hcms(args):
     import torch
     import paper_2607_01817_b200 as H   # raises if libhcms.so is missing: there is no fallback
@@ -419,6 +456,10 @@ def run_hcms(args):
     # ---- the whole attention layer, Alg. 1 lines 2-27: projections + RoPE around the hot path ----
     if not args.no_layer:
         result["layer_full"] = measure_layer(args, H, torch, dev, w, C, base_flags, timed, pk, threads)
+
+    # ---- forward + backward through the chunk pipeline (Table 15 L479-483 analogue) ----
+    if not args.no_backward:
+        result["backward"] = measure_backward(args, H, torch, w, C, base_flags, timed, pk, qd, kd, vd, out)
 
     # ---- the oracle on the host cores (rank 0, N = 1 only) -----------------------------------
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
