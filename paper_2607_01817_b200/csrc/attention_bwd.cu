@@ -19,8 +19,10 @@
 //
 // One CTA = 384 threads: warp 0 TMA producer, warp 1 MMA issuer, warp 2 TMEM allocator, warps 4-7 / 8-11 two
 // softmax warpgroups that take the streamed tiles alternately (tile t -> warpgroup t & 1), each with its own
-// T1/T2 columns in TMEM and its own P / dS staging in shared memory, so the tensor core works on tile t+1
-// while a warpgroup turns tile t into P and dS.  TMEM: T1[2] 0..127, T2[2] 128..255, accumulators from 256.
+// T1/T2 columns in TMEM.  P and dS are written back INTO those columns as packed bf16 and feed the accumulating
+// MMAs as TMEM A operands (tcgen05.mma with A in TMEM): the kernel is bound by shared-memory operand traffic
+// (ncu: tensor queue always full at 52 % pipe activity with P/dS staged in shared memory), and this removes the
+// P/dS stores and their re-reads from it.  TMEM: T1[2] 0..127, T2[2] 128..255, accumulators from 256.
 #include <cuda_bf16.h>
 
 #include "hcms_internal.h"
@@ -35,7 +37,6 @@ constexpr int kRows = 128;        // resident rows per CTA (UMMA M)
 constexpr int kCols = 64;         // streamed rows per iteration (UMMA N of T1/T2, K extent of the accumulating GEMMs)
 constexpr int kThreads = 384;
 constexpr int kTmemCols = 512;
-constexpr int kPdBytes = kRows * 128;          // P or dS staging: 128 rows x 64 bf16, one 128-byte-swizzle panel
 
 template <int D>
 struct Cfg {
@@ -44,8 +45,8 @@ struct Cfg {
   static constexpr int kStrPanelBytes = kCols * 128;           // one 64-row panel of a streamed tile
   static constexpr int kStrBytes = kPanels * kStrPanelBytes;   // one streamed tile
   static constexpr int kStageBytes = 2 * kStrBytes;            // X_t and Y_t
-  static constexpr int kStages = D == 128 ? 3 : 4;
-  static constexpr int kSmemBytes = 2 * kResBytes + kStages * kStageBytes + 4 * kPdBytes + 1024 + 256;
+  static constexpr int kStages = D == 128 ? 5 : 8;
+  static constexpr int kSmemBytes = 2 * kResBytes + kStages * kStageBytes + 1024 + 256;
   static constexpr int kTmemT1 = 0, kTmemT2 = 128, kTmemAcc = 256;
 };
 
@@ -84,15 +85,13 @@ attention_bwd_kernel(const __grid_constant__ BwdMaps maps, const BwdParams prm) 
   const uint32_t r1_smem = smem_base;
   const uint32_t r2_smem = r1_smem + C::kResBytes;
   const uint32_t ring = r2_smem + C::kResBytes;                      // kStages x (X_t, Y_t)
-  const uint32_t pd_smem = ring + kStages * C::kStageBytes;          // [warpgroup][P, dS]
-  const uint32_t bar_base = pd_smem + 4 * kPdBytes;
+  const uint32_t bar_base = ring + kStages * C::kStageBytes;
   const uint32_t bar_r_full = bar_base;                      // TMA -> MMA: resident tiles
   const uint32_t bar_x_full = bar_r_full + 8;                // [kStages] TMA -> MMA
   const uint32_t bar_x_empty = bar_x_full + 8 * kStages;     // [kStages] MMA -> TMA
   const uint32_t bar_t_full = bar_x_empty + 8 * kStages;     // [2] MMA -> warpgroup: T1, T2 of its tile are in TMEM
-  const uint32_t bar_pd_full = bar_t_full + 16;              // [2] warpgroup -> MMA: P / dS stored, T1/T2 consumed
-  const uint32_t bar_pd_free = bar_pd_full + 16;             // [2] MMA -> warpgroup: its P / dS have been read
-  const uint32_t bar_done = bar_pd_free + 16;                // MMA -> all: every accumulation has completed
+  const uint32_t bar_pd_full = bar_t_full + 16;              // [2] warpgroup -> MMA: P / dS of its tile are in TMEM
+  const uint32_t bar_done = bar_pd_full + 16;                // MMA -> all: every accumulation has completed
   const uint32_t tmem_slot = bar_done + 8;
 
   const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
@@ -113,7 +112,6 @@ attention_bwd_kernel(const __grid_constant__ BwdMaps maps, const BwdParams prm) 
     for (int g = 0; g < 2; ++g) {
       mbar_init(bar_t_full + 8 * g, 1);
       mbar_init(bar_pd_full + 8 * g, 4);    // one elected lane per warp of the warpgroup
-      mbar_init(bar_pd_free + 8 * g, 1);
     }
     fence_mbar_init();
     fence_proxy_async_smem();
@@ -189,14 +187,15 @@ attention_bwd_kernel(const __grid_constant__ BwdMaps maps, const BwdParams prm) 
           mma_ss_lohi(tmem_base + C::kTmemT2 + b * kCols, r2_lo + r_off, y_lo + s_off, hi, hi, idesc_t, ks > 0 ? 1u : 0u);
         }
       };
-      // acc[128 x D] += PD[128 x 64] * B[64 x D]: A K-major (one panel), B MN-major: 64-wide D panels
-      // kStrPanelBytes apart (LBO), 8-row groups 1024 B apart (SBO), 16 rows (one K step) = 2048 B
-      auto issue_acc = [&](uint32_t d_tmem, uint32_t pd_addr, uint32_t b_tile, bool accumulate) {
-        const uint32_t a_lo = umma_desc_lo(pd_addr, 16);
-        const uint32_t b_lo = umma_desc_lo(b_tile, C::kStrPanelBytes);
+      // acc[128 x D] += PD[128 x 64] * B[64 x D]: A = P or dS as packed bf16 in TMEM (8 columns per K step of 16),
+      // B MN-major in shared memory: 64-wide D panels kStrPanelBytes apart (LBO), 8-row groups 1024 B apart (SBO),
+      // 16 rows (one K step) = 2048 B
+      auto issue_acc = [&](uint32_t d_tmem, uint32_t a_tmem, uint32_t b_tile, bool accumulate) {
 #pragma unroll
-        for (int ks = 0; ks < kCols / 16; ++ks)
-          mma_ss_lohi(d_tmem, a_lo + ks * 2, b_lo + ks * (2048 >> 4), hi, hi, idesc_acc, (accumulate || ks > 0) ? 1u : 0u);
+        for (int ks = 0; ks < kCols / 16; ++ks) {
+          const uint64_t b_desc = (static_cast<uint64_t>(hi) << 32) | (umma_desc_lo(b_tile, C::kStrPanelBytes) + ks * (2048 >> 4));
+          mma_ts(d_tmem, a_tmem + ks * 8, b_desc, idesc_acc, (accumulate || ks > 0) ? 1u : 0u);
+        }
       };
       mbar_wait(bar_r_full, 0);
       tc_fence_after();
@@ -218,21 +217,22 @@ attention_bwd_kernel(const __grid_constant__ BwdMaps maps, const BwdParams prm) 
       for (int t = 0; t < n_iter; ++t) {
         const int b = t & 1;
         const uint32_t addr = ring + (t % kStages) * C::kStageBytes;
-        mbar_wait(bar_pd_full + 8 * b, (t >> 1) & 1);     // P / dS of tile t stored; T1/T2[b] are in registers
+        mbar_wait(bar_pd_full + 8 * b, (t >> 1) & 1);     // P / dS of tile t sit in the columns of T1/T2[b]
         tc_fence_after();
         if (leader) {
-          const uint32_t pd = pd_smem + b * 2 * kPdBytes;
+          const uint32_t p_tmem = tmem_base + C::kTmemT1 + b * kCols, ds_tmem = tmem_base + C::kTmemT2 + b * kCols;
           if (kDQ) {
-            issue_acc(tmem_base + C::kTmemAcc, pd + kPdBytes, addr, t > 0);                 // dQ += dS K_t
+            issue_acc(tmem_base + C::kTmemAcc, ds_tmem, addr, t > 0);                        // dQ += dS K_t
           } else {
-            issue_acc(tmem_base + C::kTmemAcc, pd, addr + C::kStrBytes, t > 0);             // dV += P^T dO_t
-            issue_acc(tmem_base + C::kTmemAcc + D, pd + kPdBytes, addr, t > 0);             // dK += dS^T Q_t
+            issue_acc(tmem_base + C::kTmemAcc, p_tmem, addr + C::kStrBytes, t > 0);          // dV += P^T dO_t
+            issue_acc(tmem_base + C::kTmemAcc + D, ds_tmem, addr, t > 0);                    // dK += dS^T Q_t
           }
           tc_commit(bar_x_empty + 8 * (t % kStages));
-          tc_commit(bar_pd_free + 8 * b);
           if (t == n_iter - 1) tc_commit(bar_done);
         }
         __syncwarp();
+        // T1/T2 of tile t+2 overwrite buffer b: issued after the accumulations that read P / dS from it (the
+        // tensor pipe executes one thread's MMAs in issue order)
         if (t + 2 < n_iter) {
           const uint32_t next = wait_tile(t + 2);
           if (leader) {
@@ -252,8 +252,6 @@ attention_bwd_kernel(const __grid_constant__ BwdMaps maps, const BwdParams prm) 
     const uint32_t lane_addr = static_cast<uint32_t>((warp & 3) * 32) << 16;
     const uint32_t t1_tmem = tmem_base + lane_addr + C::kTmemT1 + g * kCols;
     const uint32_t t2_tmem = tmem_base + lane_addr + C::kTmemT2 + g * kCols;
-    const uint32_t p_row = pd_smem + g * 2 * kPdBytes + row * 128;
-    const uint32_t ds_row = p_row + kPdBytes;
     const uint32_t swz = static_cast<uint32_t>(row & 7);
     const float scale_log2 = prm.scale_log2;
     const float2* stats = prm.stats + static_cast<size_t>(head) * prm.s_pad;
@@ -274,12 +272,12 @@ attention_bwd_kernel(const __grid_constant__ BwdMaps maps, const BwdParams prm) 
       tmem_ld32(t2_tmem, &dp[0]);
       tmem_ld32(t2_tmem + 32, &dp[32]);
       tmem_wait_ld();
-      tc_fence_before();
-      if (k > 0) mbar_wait(bar_pd_free + 8 * g, (k - 1) & 1);     // the accumulations of tile t-2 have read P / dS
       const int valid = prm.S - t * kCols;                        // streamed rows of this tile that exist (dQ pass mask)
+      // P and dS go back into the first 32 columns of T1 / T2 as packed bf16 (element 2c in the low half): the
+      // accumulating MMAs read their A operand from TMEM, so neither costs shared-memory bandwidth
+      uint32_t pw[kCols / 2], dw[kCols / 2];
 #pragma unroll
       for (int ch = 0; ch < kCols / 8; ++ch) {
-        uint32_t pw[4], dw[4];
 #pragma unroll
         for (int pr = 0; pr < 4; ++pr) {
           const int c = ch * 8 + pr * 2;
@@ -299,14 +297,14 @@ attention_bwd_kernel(const __grid_constant__ BwdMaps maps, const BwdParams prm) 
           }
           const float e0 = p0 * (__uint_as_float(dp[c]) - d0);
           const float e1 = p1 * (__uint_as_float(dp[c + 1]) - d1);
-          pw[pr] = pack_bf16(p0, p1);
-          dw[pr] = pack_bf16(e0, e1);
+          if (!kDQ) pw[ch * 4 + pr] = pack_bf16(p0, p1);
+          dw[ch * 4 + pr] = pack_bf16(e0, e1);
         }
-        const uint32_t off = (static_cast<uint32_t>(ch) ^ swz) << 4;
-        if (!kDQ) st_shared_v4(p_row + off, pw[0], pw[1], pw[2], pw[3]);
-        st_shared_v4(ds_row + off, dw[0], dw[1], dw[2], dw[3]);
       }
-      fence_proxy_async_smem();
+      if (!kDQ) tmem_st32(t1_tmem, pw);
+      tmem_st32(t2_tmem, dw);
+      tmem_wait_st();
+      tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(bar_pd_full + 8 * g);
     }
