@@ -48,6 +48,7 @@ struct Cfg {
   static constexpr int kStages = D == 128 ? 5 : 8;
   static constexpr int kSmemBytes = 2 * kResBytes + kStages * kStageBytes + 1024 + 256;
   static constexpr int kTmemT1 = 0, kTmemT2 = 128, kTmemAcc = 256;
+  static constexpr int kTmemR1 = 384, kTmemR2 = 448;   // dQ pass only: Q_i, dO_i as packed bf16 (D/2 columns each)
 };
 
 struct alignas(64) BwdMaps {
@@ -68,6 +69,9 @@ struct BwdParams {
 
 __device__ __forceinline__ void st_shared_v4(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
   asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
+__device__ __forceinline__ void ld_shared_v4(uint32_t addr, uint32_t& a, uint32_t& b, uint32_t& c, uint32_t& d) {
+  asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(a), "=r"(b), "=r"(c), "=r"(d) : "r"(addr) : "memory");
 }
 __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
   uint32_t r;
@@ -92,7 +96,8 @@ attention_bwd_kernel(const __grid_constant__ BwdMaps maps, const BwdParams prm) 
   const uint32_t bar_t_full = bar_x_empty + 8 * kStages;     // [2] MMA -> warpgroup: T1, T2 of its tile are in TMEM
   const uint32_t bar_pd_full = bar_t_full + 16;              // [2] warpgroup -> MMA: P / dS of its tile are in TMEM
   const uint32_t bar_done = bar_pd_full + 16;                // MMA -> all: every accumulation has completed
-  const uint32_t tmem_slot = bar_done + 8;
+  const uint32_t bar_rt_full = bar_done + 8;                 // dQ pass: warpgroups -> MMA: Q_i, dO_i copied into TMEM
+  const uint32_t tmem_slot = bar_rt_full + 8;
 
   const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
   const int lane = threadIdx.x & 31;
@@ -105,6 +110,7 @@ attention_bwd_kernel(const __grid_constant__ BwdMaps maps, const BwdParams prm) 
   if (threadIdx.x == 0) {
     mbar_init(bar_r_full, 1);
     mbar_init(bar_done, 1);
+    mbar_init(bar_rt_full, 8);            // one elected lane per softmax warp
     for (int s = 0; s < kStages; ++s) {
       mbar_init(bar_x_full + 8 * s, 1);
       mbar_init(bar_x_empty + 8 * s, 1);
@@ -178,13 +184,21 @@ attention_bwd_kernel(const __grid_constant__ BwdMaps maps, const BwdParams prm) 
         for (int ks = 0; ks < D / 16; ++ks) {
           const uint32_t r_off = ((ks >> 2) * (kRows * 128) + (ks & 3) * 32) >> 4;
           const uint32_t s_off = ((ks >> 2) * C::kStrPanelBytes + (ks & 3) * 32) >> 4;
-          mma_ss_lohi(tmem_base + C::kTmemT1 + b * kCols, r1_lo + r_off, x_lo + s_off, hi, hi, idesc_t, ks > 0 ? 1u : 0u);
+          if (kDQ)   // A = Q_i from TMEM: the resident operand costs no shared-memory bandwidth
+            mma_ts(tmem_base + C::kTmemT1 + b * kCols, tmem_base + C::kTmemR1 + ks * 8,
+                   (static_cast<uint64_t>(hi) << 32) | (x_lo + s_off), idesc_t, ks > 0 ? 1u : 0u);
+          else
+            mma_ss_lohi(tmem_base + C::kTmemT1 + b * kCols, r1_lo + r_off, x_lo + s_off, hi, hi, idesc_t, ks > 0 ? 1u : 0u);
         }
 #pragma unroll
         for (int ks = 0; ks < D / 16; ++ks) {
           const uint32_t r_off = ((ks >> 2) * (kRows * 128) + (ks & 3) * 32) >> 4;
           const uint32_t s_off = ((ks >> 2) * C::kStrPanelBytes + (ks & 3) * 32) >> 4;
-          mma_ss_lohi(tmem_base + C::kTmemT2 + b * kCols, r2_lo + r_off, y_lo + s_off, hi, hi, idesc_t, ks > 0 ? 1u : 0u);
+          if (kDQ)
+            mma_ts(tmem_base + C::kTmemT2 + b * kCols, tmem_base + C::kTmemR2 + ks * 8,
+                   (static_cast<uint64_t>(hi) << 32) | (y_lo + s_off), idesc_t, ks > 0 ? 1u : 0u);
+          else
+            mma_ss_lohi(tmem_base + C::kTmemT2 + b * kCols, r2_lo + r_off, y_lo + s_off, hi, hi, idesc_t, ks > 0 ? 1u : 0u);
         }
       };
       // acc[128 x D] += PD[128 x 64] * B[64 x D]: A = P or dS as packed bf16 in TMEM (8 columns per K step of 16),
@@ -198,6 +212,7 @@ attention_bwd_kernel(const __grid_constant__ BwdMaps maps, const BwdParams prm) 
         }
       };
       mbar_wait(bar_r_full, 0);
+      if (kDQ) mbar_wait(bar_rt_full, 0);
       tc_fence_after();
       // ring bookkeeping: tile t lives in stage t % kStages, its full-barrier phase is (t / kStages) & 1
       auto wait_tile = [&](int t) -> uint32_t {
@@ -261,6 +276,27 @@ attention_bwd_kernel(const __grid_constant__ BwdMaps maps, const BwdParams prm) 
       const float2 st = __ldg(stats + r);                // rows >= S: {+inf, 0} -> P = 0 (never stored anyway)
       row_lse2 = st.x;
       row_delta = st.y;
+    }
+
+    if (kDQ) {
+      // warpgroup 0 copies Q_i, warpgroup 1 dO_i from the swizzled shared-memory tile into TMEM (row = lane, column c
+      // = elements 2c, 2c+1): the A operand of every T1 / T2 MMA of this CTA
+      mbar_wait(bar_r_full, 0);
+      const uint32_t src = (g == 0 ? r1_smem : r2_smem) + row * 128;
+      const uint32_t dst = tmem_base + lane_addr + (g == 0 ? C::kTmemR1 : C::kTmemR2);
+#pragma unroll
+      for (int pn = 0; pn < C::kPanels; ++pn) {
+        uint32_t w[32];
+#pragma unroll
+        for (int ch = 0; ch < 8; ++ch)
+          ld_shared_v4(src + pn * (kRows * 128) + ((static_cast<uint32_t>(ch) ^ swz) << 4), w[ch * 4], w[ch * 4 + 1],
+                       w[ch * 4 + 2], w[ch * 4 + 3]);
+        tmem_st32(dst + pn * 32, w);
+      }
+      tmem_wait_st();
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar_rt_full);
     }
 
     for (int t = g, k = 0; t < n_iter; t += 2, ++k) {
