@@ -19,6 +19,7 @@
 // panels through L2.
 #include <cuda_bf16.h>
 
+#include <cstdlib>
 #include <mutex>
 
 #include "hcms_internal.h"
@@ -32,7 +33,6 @@ namespace {
 constexpr int kBM = 128;          // UMMA M
 constexpr int kBK = 64;           // one 128-byte swizzle panel of bf16 along K
 constexpr int kThreads = 256;
-constexpr int kGroupM = 16;       // m-tiles per band
 constexpr int kABytes = kBM * kBK * 2;
 constexpr int kEpiPanelBytes = kBM * 128;     // 128 rows x 64 bf16
 
@@ -60,16 +60,17 @@ struct GemmParams {
   const float* cos;     // [M, D/2]
   const float* sin;
   int m_tiles, n_tiles;
+  int group_m;          // m-tiles per band of the tile walk
 };
 
 __device__ __forceinline__ void tile_coords(int tile, const GemmParams& p, int& m0, int& n0) {
-  const int per_band = kGroupM * p.n_tiles;
+  const int per_band = p.group_m * p.n_tiles;
   const int band = tile / per_band;
   const int r = tile - band * per_band;
-  const int left = p.m_tiles - band * kGroupM;
-  const int rows = left < kGroupM ? left : kGroupM;
+  const int left = p.m_tiles - band * p.group_m;
+  const int rows = left < p.group_m ? left : p.group_m;
   const int n = r / rows;
-  m0 = (band * kGroupM + (r - n * rows)) * kBM;
+  m0 = (band * p.group_m + (r - n * rows)) * kBM;
   n0 = n;  // caller multiplies by BN
 }
 
@@ -276,6 +277,18 @@ cudaError_t map2d(CUtensorMap* m, const void* base, uint64_t inner, uint64_t out
   return encode_tensor_map(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, base, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B);
 }
 
+// m-tiles per band: the ~148 tiles in flight cover group_m x (148 / group_m) tiles, and the whole B matrix is streamed
+// from HBM once per band.  HCMS_GEMM_GROUP_M overrides the default for tuning runs (read once).
+int group_m_setting() {
+  static int v = 0;
+  if (v == 0) {
+    const char* e = std::getenv("HCMS_GEMM_GROUP_M");
+    v = e ? std::atoi(e) : 16;
+    if (v < 1 || v > 4096) v = 16;
+  }
+  return v;
+}
+
 template <int BN>
 cudaError_t launch(const GemmArgs& a, cudaStream_t stream) {
   GemmMaps maps;
@@ -302,6 +315,7 @@ cudaError_t launch(const GemmArgs& a, cudaStream_t stream) {
   p.sin = a.sin;
   p.m_tiles = static_cast<int>((a.M + kBM - 1) / kBM);
   p.n_tiles = a.N / BN;
+  p.group_m = group_m_setting();
   const int total = p.m_tiles * p.n_tiles;
   const int grid = total < a.num_sms ? total : a.num_sms;
   gemm_bf16_nt_kernel<BN><<<grid, kThreads, Cfg<BN>::kSmemBytes, stream>>>(maps, p);
