@@ -93,6 +93,14 @@ enum {
                                           exp(scale q_i.k_k) of every head (H*S floats) and keeps Q'_c, K'_c,
                                           V'_c, O'_c for hcms_attention_backward */
 
+#define HCMS_FLAG_FUSE_A2A 0x1000u     /* hcms_layer_forward only: the QKV-projection epilogue stores q, k, v
+                                          straight into the head-sharded chunk buffers Q'_c, K'_c, V'_c (the input
+                                          all-to-all is the epilogue's TMA store; on P real GPUs it would be a store to
+                                          peer memory) and the output projection loads its A operand straight from the
+                                          O'_c chunk buffers (output all-to-all + Concat in the producer's TMA load):
+                                          2 + C launches per layer, no scatter / gather kernels, no [S,H,D]
+                                          intermediates.  Same bits as the unfused layer.  Needs C <= 16, H/P <= 64. */
+
 typedef struct hcms_plan hcms_plan_t;
 
 /* ---- introspection (host only, no GPU needed) ---------------------------------------- */

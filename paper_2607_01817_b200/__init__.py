@@ -42,6 +42,7 @@ HCMS_FLAG_DEBUG_NO_COMM_WAIT = 0x100
 HCMS_FLAG_PROFILE = 0x200
 HCMS_FLAG_SINGLE_COMP = 0x400
 HCMS_FLAG_TRAINING = 0x800
+HCMS_FLAG_FUSE_A2A = 0x1000
 
 # every symbol include/hcms.h declares: name -> (restype, argtypes)
 _SIGNATURES = {

@@ -51,8 +51,20 @@ struct alignas(64) GemmMaps {
   CUtensorMap out[3];   // {n_per_out, M}, box {64, 128}
 };
 
+// Fused all-to-all (SURVEY 8(f3) "scatter fused into the QKV epilogue"): one rank-4 map {D, h_c, S, P}, box
+// {64, 1, 128, 1}, per (tensor, head chunk) over the head-sharded chunk buffers [P][S][h_c][D] of the plan.
+constexpr int kMaxChunks = 16;
+constexpr int kMaxLocalHeads = 64;
+struct alignas(64) ChunkMaps {
+  CUtensorMap m[3 * kMaxChunks];   // [tensor * C + chunk]
+};
+enum { kPlain = 0, kFusedOut = 1, kFusedA = 2 };
+
 struct GemmParams {
   int M, N, K;
+  // fused modes: heads -> (logical rank, chunk, index in chunk); D = 1 << d_shift
+  int d_shift, Hl, C;
+  uint8_t chunk_of[kMaxLocalHeads], j_of[kMaxLocalHeads];
   int n_per_out;        // output features per output tensor (N for a plain GEMM, H*D for the QKV projection)
   int rope_outs;        // the first rope_outs output tensors get the rotary embedding (2 = q and k; 0 = none)
   int half_d;           // D/2 = pairs per head
@@ -83,9 +95,13 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
   return r;
 }
 
-template <int BN>
+// kMode: kPlain = A [M,K] in, outputs [M, n_per_out] out; kFusedOut = output column n belongs to head n / D of its
+// tensor and is stored straight into that head's chunk buffer (the input all-to-all happens in the epilogue's TMA
+// store); kFusedA = A's k-block kb is columns of head kb*64 / D and is loaded straight from that head's chunk buffer
+// (the output all-to-all + Concat happen in the producer's TMA load).
+template <int BN, int kMode>
 __global__ void __launch_bounds__(kThreads, 1)
-gemm_bf16_nt_kernel(const __grid_constant__ GemmMaps maps, const GemmParams prm) {
+gemm_bf16_nt_kernel(const __grid_constant__ GemmMaps maps, const __grid_constant__ ChunkMaps cmaps, const GemmParams prm) {
   using C = Cfg<BN>;
   constexpr int kStages = C::kStages;
   extern __shared__ uint8_t smem_raw[];
@@ -144,7 +160,12 @@ gemm_bf16_nt_kernel(const __grid_constant__ GemmMaps maps, const GemmParams prm)
         if (leader) {
           const uint32_t dst = ring + stage * C::kStageBytes;
           mbar_expect_tx(bar_full + 8 * stage, C::kStageBytes);
-          tma_load_2d(dst, &maps.a, bar_full + 8 * stage, kb * kBK, m0);
+          if (kMode == kFusedA) {
+            const int head = (kb * kBK) >> prm.d_shift, rank = head / prm.Hl, lh = head - rank * prm.Hl;
+            tma_load_4d(dst, &cmaps.m[prm.chunk_of[lh]], bar_full + 8 * stage, (kb * kBK) & prm.d_mask, prm.j_of[lh], m0, rank);
+          } else {
+            tma_load_2d(dst, &maps.a, bar_full + 8 * stage, kb * kBK, m0);
+          }
           tma_load_2d(dst + kABytes, &maps.b, bar_full + 8 * stage, kb * kBK, n0);
         }
         __syncwarp();
@@ -249,7 +270,13 @@ gemm_bf16_nt_kernel(const __grid_constant__ GemmMaps maps, const GemmParams prm)
         fence_proxy_async_smem();
         named_bar_sync(1, 128);
         if (issuer) {
-          tma_store_2d(&maps.out[t_out], buf, col0 + ch * 64, m0);
+          if (kMode == kFusedOut) {
+            const int within = col0 + ch * 64;
+            const int head = within >> prm.d_shift, rank = head / prm.Hl, lh = head - rank * prm.Hl;
+            tma_store_4d(&cmaps.m[t_out * prm.C + prm.chunk_of[lh]], buf, within & prm.d_mask, prm.j_of[lh], m0, rank);
+          } else {
+            tma_store_2d(&maps.out[t_out], buf, col0 + ch * 64, m0);
+          }
           bulk_commit();
         }
       }
@@ -289,21 +316,58 @@ int group_m_setting() {
   return v;
 }
 
-template <int BN>
+template <int BN, int kMode>
 cudaError_t launch(const GemmArgs& a, cudaStream_t stream) {
   GemmMaps maps;
-  cudaError_t e = map2d(&maps.a, a.a, static_cast<uint64_t>(a.K), static_cast<uint64_t>(a.M), kBK, kBM);
+  ChunkMaps cmaps;
+  cudaError_t e = map2d(&maps.b, a.b, static_cast<uint64_t>(a.K), static_cast<uint64_t>(a.N), kBK, BN);
   if (e != cudaSuccess) return e;
-  e = map2d(&maps.b, a.b, static_cast<uint64_t>(a.K), static_cast<uint64_t>(a.N), kBK, BN);
-  if (e != cudaSuccess) return e;
+  GemmParams p{};
   const int n_out = a.N / a.n_per_out;
-  for (int t = 0; t < 3; ++t) {
-    // unused slots repeat slot 0 so that the struct holds valid descriptors only
-    void* base = a.out[t < n_out ? t : 0];
-    e = map2d(&maps.out[t], base, static_cast<uint64_t>(a.n_per_out), static_cast<uint64_t>(a.M), 64, kBM);
+  if (kMode == kPlain) {
+    e = map2d(&maps.a, a.a, static_cast<uint64_t>(a.K), static_cast<uint64_t>(a.M), kBK, kBM);
     if (e != cudaSuccess) return e;
+    for (int t = 0; t < 3; ++t) {
+      // unused slots repeat slot 0 so that the struct holds valid descriptors only
+      void* base = a.out[t < n_out ? t : 0];
+      e = map2d(&maps.out[t], base, static_cast<uint64_t>(a.n_per_out), static_cast<uint64_t>(a.M), 64, kBM);
+      if (e != cudaSuccess) return e;
+    }
+    for (auto& m : cmaps.m) m = maps.b;
+  } else {
+    const GemmChunks& ck = *a.chunks;
+    if (ck.C > kMaxChunks || ck.Hl > kMaxLocalHeads) return cudaErrorInvalidValue;
+    if (kMode == kFusedOut) {
+      e = map2d(&maps.a, a.a, static_cast<uint64_t>(a.K), static_cast<uint64_t>(a.M), kBK, kBM);
+    } else {
+      maps.a = maps.b;
+      e = map2d(&maps.out[0], a.out[0], static_cast<uint64_t>(a.n_per_out), static_cast<uint64_t>(a.M), 64, kBM);
+    }
+    if (e != cudaSuccess) return e;
+    for (int t = 0; t < 3; ++t)
+      if (kMode == kFusedOut || t > 0) maps.out[t] = kMode == kFusedOut ? maps.a : maps.out[0];
+    const int n_tensors = kMode == kFusedOut ? n_out : 1;
+    for (auto& m : cmaps.m) m = maps.b;
+    for (int t = 0; t < n_tensors; ++t)
+      for (int c = 0; c < ck.C; ++c) {
+        const uint64_t dims[4] = {static_cast<uint64_t>(a.D), static_cast<uint64_t>(ck.h[c]), static_cast<uint64_t>(a.M),
+                                  static_cast<uint64_t>(ck.P)};
+        const uint64_t strides[3] = {static_cast<uint64_t>(a.D) * 2, static_cast<uint64_t>(ck.h[c]) * a.D * 2,
+                                     static_cast<uint64_t>(a.M) * ck.h[c] * a.D * 2};
+        const uint32_t box[4] = {64, 1, kBM, 1};
+        e = encode_tensor_map(&cmaps.m[t * ck.C + c], CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, ck.base[t][c], dims, strides, box,
+                              CU_TENSOR_MAP_SWIZZLE_128B);
+        if (e != cudaSuccess) return e;
+      }
+    p.Hl = ck.Hl;
+    p.C = ck.C;
+    for (int c = 0; c < ck.C; ++c)
+      for (int j = 0; j < ck.h[c]; ++j) {
+        p.chunk_of[ck.o[c] + j] = static_cast<uint8_t>(c);
+        p.j_of[ck.o[c] + j] = static_cast<uint8_t>(j);
+      }
   }
-  GemmParams p;
+  p.d_shift = a.D == 128 ? 7 : 6;
   p.M = static_cast<int>(a.M);
   p.N = a.N;
   p.K = a.K;
@@ -318,7 +382,7 @@ cudaError_t launch(const GemmArgs& a, cudaStream_t stream) {
   p.group_m = group_m_setting();
   const int total = p.m_tiles * p.n_tiles;
   const int grid = total < a.num_sms ? total : a.num_sms;
-  gemm_bf16_nt_kernel<BN><<<grid, kThreads, Cfg<BN>::kSmemBytes, stream>>>(maps, p);
+  gemm_bf16_nt_kernel<BN, kMode><<<grid, kThreads, Cfg<BN>::kSmemBytes, stream>>>(maps, cmaps, p);
   return cudaGetLastError();
 }
 
@@ -328,21 +392,28 @@ cudaError_t gemm_init() {
   static std::once_flag once;
   static cudaError_t status = cudaSuccess;
   std::call_once(once, [] {
-    status = cudaFuncSetAttribute(gemm_bf16_nt_kernel<256>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  Cfg<256>::kSmemBytes);
-    if (status == cudaSuccess)
-      status = cudaFuncSetAttribute(gemm_bf16_nt_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    Cfg<128>::kSmemBytes);
+    auto set = [](auto fn, int bytes) {
+      if (status == cudaSuccess) status = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    };
+    set(gemm_bf16_nt_kernel<256, kPlain>, Cfg<256>::kSmemBytes);
+    set(gemm_bf16_nt_kernel<128, kPlain>, Cfg<128>::kSmemBytes);
+    set(gemm_bf16_nt_kernel<256, kFusedOut>, Cfg<256>::kSmemBytes);
+    set(gemm_bf16_nt_kernel<128, kFusedOut>, Cfg<128>::kSmemBytes);
+    set(gemm_bf16_nt_kernel<256, kFusedA>, Cfg<256>::kSmemBytes);
+    set(gemm_bf16_nt_kernel<128, kFusedA>, Cfg<128>::kSmemBytes);
   });
   return status;
 }
 
 // Shape rules (checked by the callers in hcms_api.cu): K % 8 == 0 (16-byte row pitch), n_per_out % 128 == 0,
-// N % n_per_out == 0, N / n_per_out <= 3, and with RoPE D in {64, 128}.
+// N % n_per_out == 0, N / n_per_out <= 3, and with RoPE or a fused mode D in {64, 128}; fused modes: C <= 16, H/P <= 64.
 cudaError_t launch_gemm(const GemmArgs& a, cudaStream_t stream) {
   cudaError_t e = gemm_init();
   if (e != cudaSuccess) return e;
-  return (a.n_per_out % 256 == 0) ? launch<256>(a, stream) : launch<128>(a, stream);
+  const bool wide = a.n_per_out % 256 == 0;
+  if (a.fuse == 1) return wide ? launch<256, kFusedOut>(a, stream) : launch<128, kFusedOut>(a, stream);
+  if (a.fuse == 2) return wide ? launch<256, kFusedA>(a, stream) : launch<128, kFusedA>(a, stream);
+  return wide ? launch<256, kPlain>(a, stream) : launch<128, kPlain>(a, stream);
 }
 
 }  // namespace hcms

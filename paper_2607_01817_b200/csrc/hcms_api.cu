@@ -719,6 +719,102 @@ static int run_gemm(const GemmArgs& g, cudaStream_t st, const char* what) {
   return HCMS_OK;
 }
 
+// hcms_layer_forward under HCMS_FLAG_FUSE_A2A: projection epilogue -> chunk buffers -> attention per chunk -> output
+// projection reading the O'_c chunk buffers.  Attention launches alternate between the two compute streams as in
+// hcms_attention_forward (tail-wave backfill); there is no communication stream because no copy is left.
+static int layer_forward_fused(hcms_plan_t* plan, const void* x, const void* w_qkv, const void* w_o, const void* rope_cos,
+                               const void* rope_sin, void* y, int Dm, float scale, cudaStream_t caller) {
+  const Shape& sh = plan->sh;
+  if ((rope_cos == nullptr) != (rope_sin == nullptr)) return fail(HCMS_ERR_INVALID_ARG, "pass both RoPE tables or neither");
+  if (sh.C > 16 || sh.Hl > 64)
+    return fail(HCMS_ERR_UNSUPPORTED_SHAPE, "HCMS_FLAG_FUSE_A2A needs C <= 16 and H/P <= 64 (C=%d, H/P=%d)", sh.C, sh.Hl);
+  for (const void* ptr : {x, w_qkv, w_o, rope_cos, rope_sin, static_cast<const void*>(y)})
+    if (!aligned16(ptr)) return fail(HCMS_ERR_MISALIGNED, "every pointer must be 16-byte aligned");
+  int st = check_scale(scale);
+  if (st) return st;
+  if (!plan->ws) return fail(HCMS_ERR_WORKSPACE_TOO_SMALL, "plan has no workspace");
+  char* ws = static_cast<char*>(plan->ws);
+  GemmChunks ck{};
+  ck.C = sh.C;
+  ck.Hl = sh.Hl;
+  ck.P = sh.P;
+  for (int c = 0; c < sh.C; ++c) {
+    ck.o[c] = plan->chunks[c].o;
+    ck.h[c] = plan->chunks[c].h;
+  }
+  const bool profile = plan->flags & HCMS_FLAG_PROFILE;
+  const bool serial = plan->flags & HCMS_FLAG_SERIAL;
+  const bool dual_comp = !serial && !(plan->flags & HCMS_FLAG_SINGLE_COMP) && sh.C > 1;
+  plan->last_launches = 0;
+  if (profile) HCMS_CUDA(cudaEventRecord(plan->e_layer[0], caller));
+  {  // lines 2-3 + input all-to-all
+    for (int c = 0; c < sh.C; ++c)
+      for (int t = 0; t < 3; ++t) ck.base[t][c] = ws + plan->chunks[c].off[t];
+    GemmArgs g{};
+    g.a = x;
+    g.b = w_qkv;
+    g.M = sh.S;
+    g.N = 3 * sh.H * sh.D;
+    g.K = Dm;
+    g.n_per_out = sh.H * sh.D;
+    g.rope_outs = rope_cos ? 2 : 0;
+    g.D = sh.D;
+    g.cos = static_cast<const float*>(rope_cos);
+    g.sin = static_cast<const float*>(rope_sin);
+    g.num_sms = plan->num_sms;
+    g.fuse = 1;
+    g.chunks = &ck;
+    st = run_gemm(g, caller, "fused QKV projection launch");
+    if (st) return st;
+    plan->last_launches += 1;
+  }
+  if (profile) HCMS_CUDA(cudaEventRecord(plan->e_layer[1], caller));
+  if (!serial) {
+    HCMS_CUDA(cudaEventRecord(plan->e_main, caller));
+    HCMS_CUDA(cudaStreamWaitEvent(plan->s_comp, plan->e_main, 0));
+    if (dual_comp) HCMS_CUDA(cudaStreamWaitEvent(plan->s_comp2, plan->e_main, 0));
+  }
+  for (int c = 0; c < sh.C; ++c) {   // line 15 per chunk
+    const Chunk& k = plan->chunks[c];
+    cudaStream_t s_comp = serial ? caller : ((dual_comp && (c & 1)) ? plan->s_comp2 : plan->s_comp);
+    float* lse_c = plan->lse ? plan->lse + static_cast<size_t>(sh.P) * sh.S * k.o : nullptr;
+    st = do_attention(plan, ws + k.off[0], ws + k.off[1], ws + k.off[2], ws + k.off[3], c, scale, s_comp, lse_c);
+    if (st) return st;
+  }
+  if (!serial) {
+    HCMS_CUDA(cudaEventRecord(plan->e_fin_comp, plan->s_comp));
+    HCMS_CUDA(cudaStreamWaitEvent(caller, plan->e_fin_comp, 0));
+    if (dual_comp) {
+      HCMS_CUDA(cudaEventRecord(plan->e_fin_comp2, plan->s_comp2));
+      HCMS_CUDA(cudaStreamWaitEvent(caller, plan->e_fin_comp2, 0));
+    }
+  }
+  if (profile) HCMS_CUDA(cudaEventRecord(plan->e_layer[2], caller));
+  {  // output all-to-all + Concat + line 27
+    for (int c = 0; c < sh.C; ++c) ck.base[0][c] = ws + plan->chunks[c].off[3];
+    GemmArgs g{};
+    g.b = w_o;
+    g.out[0] = y;
+    g.M = sh.S;
+    g.N = Dm;
+    g.K = sh.H * sh.D;
+    g.n_per_out = Dm;
+    g.D = sh.D;
+    g.num_sms = plan->num_sms;
+    g.fuse = 2;
+    g.chunks = &ck;
+    st = run_gemm(g, caller, "fused output projection launch");
+    if (st) return st;
+    plan->last_launches += 1;
+  }
+  if (profile) {
+    HCMS_CUDA(cudaEventRecord(plan->e_layer[3], caller));
+    plan->layer_timed = true;
+  }
+  plan->forward_done = true;
+  return HCMS_OK;
+}
+
 extern "C" {
 
 int hcms_gemm_bf16_nt(const void* a, const void* b, void* c, int64_t M, int N, int K, void* stream) {
@@ -813,6 +909,8 @@ int hcms_layer_forward(hcms_plan_t* plan, const void* x, const void* w_qkv, cons
   if (st) return st;
   const size_t xy_bytes = static_cast<size_t>(S) * Dm * 2;
   if (overlaps(x, xy_bytes, y, xy_bytes)) return fail(HCMS_ERR_ALIAS, "y overlaps x");
+  if (plan->flags & HCMS_FLAG_FUSE_A2A)
+    return layer_forward_fused(plan, x, w_qkv, w_o, rope_cos, rope_sin, y, Dm, scale, static_cast<cudaStream_t>(stream));
   const size_t bytes = static_cast<size_t>(S) * H * D * sh.es;
   for (auto& b : plan->layer_buf)
     if (!b) HCMS_CUDA(cudaMalloc(&b, bytes));

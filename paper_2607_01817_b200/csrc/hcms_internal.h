@@ -86,6 +86,12 @@ cudaError_t attention_bwd_init();
 size_t attention_bwd_stats_bytes(int64_t S, int heads);
 
 // ---- projection GEMMs (gemm_bf16.cu): C[M,N] = A[M,K] * B[N,K]^T, bf16 -> fp32 -> bf16 -------
+// chunk buffers of a plan, for the fused all-to-all modes of the projection GEMMs
+struct GemmChunks {
+  int C, Hl, P;
+  int o[16], h[16];        // Eq. 3 chunk table
+  void* base[3][16];       // [tensor][chunk] -> [P][S][h_c][D] bf16 (fuse = 1: Q'_c, K'_c, V'_c; fuse = 2: base[0] = O'_c)
+};
 struct GemmArgs {
   const void* a;       // [M, K] bf16, row-major
   const void* b;       // [N, K] bf16, row-major (torch.nn.Linear weight)
@@ -98,6 +104,9 @@ struct GemmArgs {
   const float* cos;    // [M, D/2] fp32 (RoPE only)
   const float* sin;
   int num_sms;
+  int fuse = 0;                       // 0: plain; 1: outputs stored into the chunk buffers (`out` unused);
+                                      // 2: A loaded from the O'_c chunk buffers (`a` unused)
+  const GemmChunks* chunks = nullptr;
 };
 cudaError_t launch_gemm(const GemmArgs& a, cudaStream_t stream);
 cudaError_t gemm_init();

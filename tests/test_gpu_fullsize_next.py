@@ -91,3 +91,21 @@ def test_forward_backward_cfg3_sampled():
         rel = np.linalg.norm(g - ref) / np.linalg.norm(ref)
         assert rel <= 1e-2 and err.max() <= 2e-2 * np.abs(ref).max() + 1e-5, \
             f"{name}: rel_l2={rel:.3e} max_err={err.max():.3e} max_ref={np.abs(ref).max():.3e}"
+
+
+def test_fused_layer_cfg3_equals_unfused_bitwise():
+    """HCMS_FLAG_FUSE_A2A at the full cfg 3 shape: 6 launches instead of 14, identical y."""
+    w = W3
+    S, Hh, D = w.S, w.H, w.D
+    Dm = Hh * D
+    arrs = I.make_layer_inputs(w)
+    xd, wqd, wod, cd, sd = (to_dev(t) for t in arrs)
+    ys = []
+    for flags in (0, H.HCMS_FLAG_FUSE_A2A):
+        y = dev_out(S, Dm)
+        with H.hcms_plan(S, Hh, D, w.P, w.C, H.HCMS_DTYPE_BF16, flags) as plan:
+            H.hcms_layer_forward(plan, xd, wqd, wod, cd, sd, y, Dm, w.scale)
+            torch.cuda.synchronize()
+        ys.append(y)
+    assert not bool((ys[0] == 0x7FC0).any())
+    assert torch.equal(ys[0], ys[1])

@@ -261,3 +261,54 @@ def test_layer_timings_and_errors():
         with pytest.raises(H.HcmsError) as e:
             H.hcms_layer_forward(plan, x, w_qkv, w_o, cos, sin, y, 200, w.scale)
         assert e.value.status == H.HCMS_ERR_UNSUPPORTED_SHAPE
+
+
+# ---------------------------------------------------------------------------------------------
+# HCMS_FLAG_FUSE_A2A: all-to-alls fused into the projection GEMMs
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("S,Hh,D,Dm,P,C", [(1024, 4, 64, 256, 2, 2), (2100, 12, 128, 512, 4, 2), (777, 6, 64, 384, 1, 5),
+                                           (1500, 8, 128, 1024, 2, 3)])
+def test_fused_layer_equals_unfused_bitwise(S, Hh, D, Dm, P, C):
+    """The fused layer launches 2 + C kernels (no scatter / gather) and must reproduce the unfused layer bit for
+    bit: same projections, same attention kernel on the same chunk buffers.  Uneven chunks (3 -> 2+1, 6 -> 2+1+1+1+1,
+    4 -> 2+1+1), ragged S, both head dims, one head per 64-column panel (D=64) and two panels per head (D=128)."""
+    w = I.Workload("t", S, Hh, D, P, C, 33, "bf16", 1.0)
+    x, w_qkv, w_o, cos, sin = I.make_layer_inputs(w, Dm)
+    xd, wqd, wod, cd, sd = (to_dev(t) for t in (x, w_qkv, w_o, cos, sin))
+    scale = w.scale
+    ys = []
+    for flags in (0, H.HCMS_FLAG_FUSE_A2A, H.HCMS_FLAG_FUSE_A2A | H.HCMS_FLAG_SERIAL):
+        y = dev_out(S, Dm)
+        with H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, flags) as plan:
+            n = H.hcms_plan_workspace_bytes(plan)
+            ws = nan_fill_(torch.empty((n + 1) // 2, dtype=torch.int16, device=DEV))
+            H.hcms_plan_set_workspace(plan, ws, n)
+            H.hcms_layer_forward(plan, xd, wqd, wod, cd, sd, y, Dm, scale)
+            torch.cuda.synchronize()
+            assert H.hcms_plan_last_launch_count(plan) == (3 * C + 2 if flags == 0 else C + 2)
+        ys.append(to_host(y))
+    assert not np.isnan(bf16_bits_to_f64(ys[0])).any()
+    assert np.array_equal(ys[0], ys[1]) and np.array_equal(ys[0], ys[2])
+
+
+def test_fused_layer_vs_oracle_and_chunk_buffers():
+    """Fused layer against the fp64 oracle, and its chunk buffers against the oracle's scatter of the projected q, k, v
+    (the epilogue must place every head in the right rank / chunk / slot)."""
+    w = I.Workload("t", 900, 6, 128, 2, 2, 34, "bf16", 1.0)          # per-rank 3 heads -> chunks 2 + 1
+    Dm = 256
+    x, w_qkv, w_o, cos, sin = I.make_layer_inputs(w, Dm)
+    y = dev_out(w.S, Dm)
+    with H.hcms_plan(w.S, w.H, w.D, w.P, w.C, H.HCMS_DTYPE_BF16, H.HCMS_FLAG_FUSE_A2A) as plan:
+        H.hcms_layer_forward(plan, to_dev(x), to_dev(w_qkv), to_dev(w_o), to_dev(cos), to_dev(sin), y, Dm, w.scale)
+        torch.cuda.synchronize()
+        base = H.hcms_plan_workspace(plan)
+        ref_qkv = L.project_and_rotate(x, w_qkv, cos, sin, w.H, w.D)
+        _, h_c = H.hcms_chunk_table(plan)
+        for c in range(w.C):
+            lay = H.hcms_chunk_layout(plan, c)
+            n = w.P * w.S * h_c[c] * w.D
+            for t, key in enumerate(("q_off", "k_off", "v_off")):
+                got = to_host(_device_view(base + lay[key], n)).reshape(w.P, w.S, h_c[c], w.D)
+                check_rounded(got, O.scatter_chunk(ref_qkv[t], w.P, w.C, c), f"chunk {c} tensor {t}")
+    check_layer(to_host(y), L.layer_forward(x, w_qkv, w_o, cos, sin, w.H, w.D, w.scale), "fused layer")
