@@ -240,6 +240,24 @@ def measure_layer(args, H, torch, dev, w, C, base_flags, timed, pk, threads):
     ms, parts = total / n, parts / n
     launches = H.hcms_plan_last_launch_count(plan)
     plan.close()
+    # the same layer with the all-to-alls fused into the projection GEMMs (HCMS_FLAG_FUSE_A2A)
+    y2 = torch.empty_like(y)
+    plan_f = H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, base_flags | H.HCMS_FLAG_FUSE_A2A)
+    step_f = lambda: H.hcms_layer_forward(plan_f, x, wq, wo, cos, sin, y2, Dm, w.scale)
+    for _ in range(3):
+        step_f()
+    torch.cuda.synchronize()
+    parts_f, total_f = np.zeros(3), 0.0
+    for _ in range(n):
+        total_f += timed(plan_f, 1, step_f)
+        parts_f += np.asarray(H.hcms_plan_layer_timings(plan_f))
+    ms_f, parts_f = total_f / n, parts_f / n
+    launches_f = H.hcms_plan_last_launch_count(plan_f)
+    plan_f.close()
+    fused = {"flag": "HCMS_FLAG_FUSE_A2A", "ms_per_layer": round(ms_f, 4), "launches_per_layer": launches_f,
+             "qkv_rope_scatter_ms": round(float(parts_f[0]), 4), "attention_ms": round(float(parts_f[1]), 4),
+             "gather_out_proj_ms": round(float(parts_f[2]), 4), "speedup_vs_unfused": round(ms / ms_f, 4),
+             "bitwise_equal_to_unfused": bool(torch.equal(y, y2))}
     qkv_flop, out_flop, attn_flop = 2.0 * S * Dm * 3 * Hh * D, 2.0 * S * Hh * D * Dm, 4.0 * S * S * D * Hh
     gemm_tf = (qkv_flop + out_flop) / ((parts[0] + parts[2]) * 1e-3) / 1e12
     return {
@@ -253,7 +271,7 @@ def measure_layer(args, H, torch, dev, w, C, base_flags, timed, pk, threads):
                           "peak": pk["bf16_tflops_sustained"], "unit": "TFLOP/s",
                           "frac": round(gemm_tf / pk["bf16_tflops_sustained"], 4),
                           "frac_of_nominal": round(gemm_tf / NOMINAL_BF16_TFLOPS, 4)},
-        "t_other_share": round(float(parts[0] + parts[2]) / ms, 4),
+        "t_other_share": round(float(parts[0] + parts[2]) / ms, 4), "fused": fused,
         "weights": "random init N(0, 1/fan_in) -> bf16, RoPE tables s*10000^(-2i/D) (hcms_inputs.make_layer_inputs)",
     }
 
