@@ -101,6 +101,12 @@ enum {
                                           2 + C launches per layer, no scatter / gather kernels, no [S,H,D]
                                           intermediates.  Same bits as the unfused layer.  Needs C <= 16, H/P <= 64. */
 
+#define HCMS_FLAG_GRAPH 0x2000u        /* hcms_attention_forward captures the whole chunk pipeline (every kernel and copy
+                                          on S_comm / S_comp with the event forks and joins of Eq. 6-7) into a CUDA
+                                          graph on first use and replays it with ONE launch per call; other tensor
+                                          addresses or another scale capture again.  For launch-bound shapes
+                                          (BASELINE.json configs 1-2).  Same bits.  Excludes HCMS_FLAG_PROFILE. */
+
 typedef struct hcms_plan hcms_plan_t;
 
 /* ---- introspection (host only, no GPU needed) ---------------------------------------- */
@@ -222,6 +228,8 @@ int hcms_attention_chunk(hcms_plan_t* plan, const void* qc, const void* kc, cons
 
 /* Number of kernels + async copies the last hcms_attention_forward on this plan enqueued. */
 int hcms_plan_last_launch_count(const hcms_plan_t* plan);
+/* How many times a HCMS_FLAG_GRAPH plan has captured its pipeline (1 after any number of calls on the same tensors). */
+int hcms_plan_graph_captures(const hcms_plan_t* plan);
 
 /*
  * Device durations, in milliseconds, of the steps of a recent hcms_attention_forward on a plan made

@@ -43,6 +43,7 @@ HCMS_FLAG_PROFILE = 0x200
 HCMS_FLAG_SINGLE_COMP = 0x400
 HCMS_FLAG_TRAINING = 0x800
 HCMS_FLAG_FUSE_A2A = 0x1000
+HCMS_FLAG_GRAPH = 0x2000
 
 # every symbol include/hcms.h declares: name -> (restype, argtypes)
 _SIGNATURES = {
@@ -83,6 +84,7 @@ _SIGNATURES = {
     "hcms_attention_chunk_lse": (c_int, [c_void_p] * 6 + [c_int, c_float, c_void_p]),
     "hcms_attention_backward_chunk": (c_int, [c_void_p] * 10 + [c_int, c_float, c_void_p]),
     "hcms_plan_lse": (c_void_p, [c_void_p]),
+    "hcms_plan_graph_captures": (c_int, [c_void_p]),
 }
 
 
@@ -390,3 +392,7 @@ def hcms_attention_backward_chunk(plan: Plan, qc, kc, vc, oc, doc, lse, dqc, dkc
 
 def hcms_plan_lse(plan: Plan) -> int:
     return lib.hcms_plan_lse(plan.handle) or 0
+
+
+def hcms_plan_graph_captures(plan: Plan) -> int:
+    return lib.hcms_plan_graph_captures(plan.handle)

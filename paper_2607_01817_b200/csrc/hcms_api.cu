@@ -80,6 +80,13 @@ struct hcms_plan {
   float* lse = nullptr;
   void* stats = nullptr;      // packed {lse*log2e, delta}: [H][s_pad] float2 (lazily allocated)
   bool forward_done = false;
+  // HCMS_FLAG_GRAPH: the captured chunk pipeline of the last (q, k, v, out, scale) and the stream it was captured on
+  cudaStream_t s_cap = nullptr;
+  cudaGraphExec_t graph_exec = nullptr;
+  const void* graph_key[4] = {nullptr, nullptr, nullptr, nullptr};
+  float graph_scale = 0.f;
+  int graph_launches = 0;
+  long long graph_captures = 0;
   // HCMS_FLAG_PROFILE: [step 0=scatter,1=attention,2=gather][begin,end][ring slot * C + chunk]
   std::vector<cudaEvent_t> prof[3][2];
   long long prof_calls = 0;   // forward calls that recorded a full set of events
@@ -115,6 +122,8 @@ static void plan_free(hcms_plan_t* p) {
     if (d) cudaFree(d);
   for (auto& d : p->layer_buf)
     if (d) cudaFree(d);
+  if (p->graph_exec) cudaGraphExecDestroy(p->graph_exec);
+  if (p->s_cap) cudaStreamDestroy(p->s_cap);
   if (p->train_ws) cudaFree(p->train_ws);
   if (p->lse) cudaFree(p->lse);
   if (p->stats) cudaFree(p->stats);
@@ -200,6 +209,8 @@ int hcms_plan(hcms_plan_t** out, int64_t S, int H, int D, int P, int C, int dtyp
   if (S > (1ll << 30)) return fail(HCMS_ERR_UNSUPPORTED_SHAPE, "S=%lld too large", static_cast<long long>(S));
   const int Hl = H / P;
   if (C > Hl) return fail(HCMS_ERR_UNSUPPORTED_SHAPE, "C=%d exceeds heads per rank H/P=%d", C, Hl);
+  if ((flags & HCMS_FLAG_GRAPH) && (flags & HCMS_FLAG_PROFILE))
+    return fail(HCMS_ERR_INVALID_ARG, "HCMS_FLAG_GRAPH and HCMS_FLAG_PROFILE exclude each other (timing events cannot be read from a graph)");
 
   int dev = 0, n = 0;
   cudaError_t ce = cudaGetDeviceCount(&n);
@@ -255,6 +266,7 @@ int hcms_plan(hcms_plan_t** out, int64_t S, int H, int D, int P, int C, int dtyp
   PLAN_CUDA(cudaStreamCreateWithPriority(&p->s_comm_out, cudaStreamNonBlocking, prio_hi));
   PLAN_CUDA(cudaStreamCreateWithPriority(&p->s_comp, cudaStreamNonBlocking, prio_lo));
   PLAN_CUDA(cudaStreamCreateWithPriority(&p->s_comp2, cudaStreamNonBlocking, prio_lo));
+  if (flags & HCMS_FLAG_GRAPH) PLAN_CUDA(cudaStreamCreateWithFlags(&p->s_cap, cudaStreamNonBlocking));
   PLAN_CUDA(cudaEventCreateWithFlags(&p->e_main, cudaEventDisableTiming));
   PLAN_CUDA(cudaEventCreateWithFlags(&p->e_fin_comm, cudaEventDisableTiming));
   PLAN_CUDA(cudaEventCreateWithFlags(&p->e_fin_comp, cudaEventDisableTiming));
@@ -433,6 +445,13 @@ int hcms_attention_chunk(hcms_plan_t* plan, const void* qc, const void* kc, cons
 // ------------------------------------------------------------------------------------------
 // the dual-stream chunk scheduler (Algorithm 1 lines 4-25)
 // ------------------------------------------------------------------------------------------
+}  // extern "C"
+static int enqueue_forward(hcms_plan_t* plan, const void* q, const void* k, const void* v, void* out, float scale,
+                           cudaStream_t caller);
+static int forward_graph(hcms_plan_t* plan, const void* q, const void* k, const void* v, void* out, float scale,
+                         cudaStream_t caller);
+extern "C" {
+
 int hcms_attention_forward(hcms_plan_t* plan, const void* q, const void* k, const void* v, void* out, int64_t S, int H,
                            int D, int P, int C, float scale, void* stream) {
   if (!plan || !q || !k || !v || !out) return fail(HCMS_ERR_INVALID_ARG, "NULL argument");
@@ -452,8 +471,18 @@ int hcms_attention_forward(hcms_plan_t* plan, const void* q, const void* k, cons
     if (ob < ib + bytes && ib < ob + bytes) return fail(HCMS_ERR_ALIAS, "out overlaps an input tensor");
   }
   if (!plan->ws) return fail(HCMS_ERR_WORKSPACE_TOO_SMALL, "plan has no workspace");
-
   cudaStream_t caller = static_cast<cudaStream_t>(stream);
+  if (plan->flags & HCMS_FLAG_GRAPH) return forward_graph(plan, q, k, v, out, scale, caller);
+  return enqueue_forward(plan, q, k, v, out, scale, caller);
+}
+
+}  // extern "C"
+
+// Enqueue Alg. 1 lines 4-25 for validated arguments: kernels, copies, event records and waits; no host synchronisation.
+static int enqueue_forward(hcms_plan_t* plan, const void* q, const void* k, const void* v, void* out, float scale,
+                           cudaStream_t caller) {
+  const Shape& sh = plan->sh;
+  int st = HCMS_OK;
   const bool serial = plan->flags & HCMS_FLAG_SERIAL;
   const bool split = (plan->flags & HCMS_FLAG_SPLIT_COMM) && !serial;
   cudaStream_t s_in = serial ? caller : plan->s_comm;
@@ -552,6 +581,51 @@ int hcms_attention_forward(hcms_plan_t* plan, const void* q, const void* k, cons
   }
   return HCMS_OK;
 }
+
+// HCMS_FLAG_GRAPH: the whole chunk pipeline (kernels on S_comm / S_comp, the event forks and joins of Eq. 6-7) is
+// captured once into a CUDA graph on a plan-owned stream and replayed with one launch per call; a call with other
+// tensors or another scale captures again.  The capture runs on the plan's own stream because the caller's may be
+// the legacy default stream, which cannot be captured.
+static int forward_graph(hcms_plan_t* plan, const void* q, const void* k, const void* v, void* out, float scale,
+                         cudaStream_t caller) {
+  const void* key[4] = {q, k, v, out};
+  const bool hit = plan->graph_exec && std::memcmp(key, plan->graph_key, sizeof(key)) == 0 &&
+                   std::memcmp(&scale, &plan->graph_scale, sizeof(float)) == 0;
+  if (!hit) {
+    if (plan->graph_exec) {
+      HCMS_CUDA(cudaGraphExecDestroy(plan->graph_exec));
+      plan->graph_exec = nullptr;
+    }
+    HCMS_CUDA(cudaStreamBeginCapture(plan->s_cap, cudaStreamCaptureModeRelaxed));
+    const int st = enqueue_forward(plan, q, k, v, out, scale, plan->s_cap);
+    cudaGraph_t graph = nullptr;
+    const cudaError_t ce = cudaStreamEndCapture(plan->s_cap, &graph);   // always ends the capture, also after a failure
+    if (st != HCMS_OK) {
+      if (graph) cudaGraphDestroy(graph);
+      cudaGetLastError();
+      return st;
+    }
+    if (ce != cudaSuccess) return fail_cuda(ce, "cudaStreamEndCapture");
+    const cudaError_t ci = cudaGraphInstantiate(&plan->graph_exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (ci != cudaSuccess) {
+      plan->graph_exec = nullptr;
+      return fail_cuda(ci, "cudaGraphInstantiate");
+    }
+    std::memcpy(plan->graph_key, key, sizeof(key));
+    plan->graph_scale = scale;
+    plan->graph_launches = plan->last_launches;
+    plan->graph_captures += 1;
+  }
+  HCMS_CUDA(cudaGraphLaunch(plan->graph_exec, caller));
+  plan->last_launches = plan->graph_launches;
+  plan->forward_done = true;
+  return HCMS_OK;
+}
+
+extern "C" {
+
+int hcms_plan_graph_captures(const hcms_plan_t* plan) { return plan ? static_cast<int>(plan->graph_captures) : 0; }
 
 int hcms_plan_timings(hcms_plan_t* plan, int calls_back, float* scatter_ms, float* attn_ms, float* gather_ms) {
   if (!plan) return fail(HCMS_ERR_INVALID_ARG, "plan is NULL");

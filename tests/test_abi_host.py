@@ -131,6 +131,12 @@ def test_plan_argument_validation_precedes_device_use():
         assert ei.value.status == code, args
 
 
+def test_graph_and_profile_flags_exclude_each_other():
+    with pytest.raises(H.HcmsError) as e:
+        H.hcms_plan(1024, 4, 64, 2, 2, H.HCMS_DTYPE_BF16, H.HCMS_FLAG_GRAPH | H.HCMS_FLAG_PROFILE)
+    assert e.value.status == H.HCMS_ERR_INVALID_ARG
+
+
 def test_no_cpu_fallback_without_device():
     import torch
     if torch.cuda.is_available():

@@ -115,3 +115,57 @@ def test_dropping_the_comm_wait_lets_attention_read_unscattered_chunks():
     assert np.array_equal(good, _forward(qkv, S, Hh, D, P, C, scale))
     bad = _forward(qkv, S, Hh, D, P, C, scale, H.HCMS_FLAG_HOST_ROUTE_V | H.HCMS_FLAG_DEBUG_NO_COMM_WAIT)
     assert is_nan(bad).any(), "the race did not show: the negative test has lost its teeth"
+
+
+# ---------------------------------------------------------------------------------------------
+# HCMS_FLAG_GRAPH: the chunk pipeline captured into a CUDA graph
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("extra", [0, H.HCMS_FLAG_SERIAL, H.HCMS_FLAG_SPLIT_COMM, H.HCMS_FLAG_SINGLE_COMP,
+                                   H.HCMS_FLAG_HOST_ROUTE_K | H.HCMS_FLAG_HOST_ROUTE_O, H.HCMS_FLAG_LAYOUT_TMA])
+def test_graph_replay_same_bits(extra):
+    """One capture, many replays, the bits of the plain call; new tensors capture again; poisoned workspace and
+    output before every replay (a replay that skipped a node or broke an Eq. 6-7 edge would leave NaN)."""
+    S, Hh, D, P, C = 2048, 6, 64, 2, 3
+    qkv, scale = _inputs(S, Hh, D, seed=21)
+    want = _forward(qkv, S, Hh, D, P, C, scale, extra)
+    q, k, v = qkv
+    out, out2 = nan_fill_(torch.empty_like(q)), nan_fill_(torch.empty_like(q))
+    with H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, extra | H.HCMS_FLAG_GRAPH) as plan:
+        n = H.hcms_plan_workspace_bytes(plan)
+        ws = torch.empty((n + 1) // 2, dtype=torch.int16, device=DEV)
+        H.hcms_plan_set_workspace(plan, ws, n)
+        for _ in range(3):
+            nan_fill_(ws)
+            nan_fill_(out)
+            H.hcms_attention_forward(plan, q, k, v, out, scale)
+            torch.cuda.synchronize()
+            assert np.array_equal(to_host(out), want)
+        assert H.hcms_plan_graph_captures(plan) == 1
+        launches = H.hcms_plan_last_launch_count(plan)
+        H.hcms_attention_forward(plan, q, k, v, out2, scale)             # another output tensor -> second capture
+        torch.cuda.synchronize()
+        assert H.hcms_plan_graph_captures(plan) == 2 and np.array_equal(to_host(out2), want)
+        assert H.hcms_plan_last_launch_count(plan) == launches
+        H.hcms_attention_forward(plan, q, k, v, out2, scale * 0.5)       # another scale -> third capture
+        torch.cuda.synchronize()
+        assert H.hcms_plan_graph_captures(plan) == 3 and not np.array_equal(to_host(out2), want)
+
+
+def test_graph_on_a_side_stream_orders_with_the_caller():
+    """The replay is ordered after work already on the caller's stream and before what follows it."""
+    S, Hh, D, P, C = 1024, 4, 64, 2, 2
+    qkv, scale = _inputs(S, Hh, D, seed=22)
+    want = _forward(qkv, S, Hh, D, P, C, scale)
+    side = torch.cuda.Stream()
+    with H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, H.HCMS_FLAG_GRAPH) as plan:
+        with torch.cuda.stream(side):
+            q = torch.zeros_like(qkv[0])
+            for _ in range(3):
+                q.copy_(qkv[0], non_blocking=True)                       # producer on the caller's stream
+                out = nan_fill_(torch.empty_like(q))
+                H.hcms_attention_forward(plan, q, qkv[1], qkv[2], out, scale, stream=side)
+                res = out.clone()                                        # consumer on the caller's stream
+                q.zero_()
+        side.synchronize()
+        assert np.array_equal(to_host(res), want)
