@@ -449,6 +449,25 @@ def run_hcms(args):
         "s_max_bound": round(H.hcms_model_s_max(copy_ms / ser_ms), 4),
     }
 
+    # ---- launch overhead: plain enqueue vs the CUDA-graph replay (HCMS_FLAG_GRAPH), no profile events ----
+    n_g = max(3, min(args.steps, 20))
+    g_res = {}
+    for name, extra in (("enqueue", 0), ("graph", H.HCMS_FLAG_GRAPH)):
+        plan_g = H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, (base_flags & ~H.HCMS_FLAG_PROFILE) | extra)
+        step_g = lambda: H.hcms_attention_forward(plan_g, qd, kd, vd, out, w.scale)
+        for _ in range(3):
+            step_g()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        ms_g = timed(plan_g, n_g, step_g) / n_g
+        host_us = (time.perf_counter() - t0) * 1e6 / n_g
+        g_res[name] = (ms_g, host_us)
+        plan_g.close()
+    result["graph"] = {"enqueue_ms": round(g_res["enqueue"][0], 4), "graph_ms": round(g_res["graph"][0], 4),
+                       "speedup": round(g_res["enqueue"][0] / g_res["graph"][0], 4), "steps": n_g,
+                       "what": "hcms_attention_forward without profile events: %d launches + events enqueued per call vs one "
+                               "cudaGraphLaunch of the captured pipeline" % (launches // args.steps)}
+
     # ---- end to end through the public host-buffer call --------------------------------------
     if not args.no_e2e:
         plan_e = H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, base_flags & ~H.HCMS_FLAG_PROFILE)
