@@ -9,6 +9,8 @@
 // accumulators, before the single rounding to bf16: adjacent pairs (x[2i], x[2i+1]) of a head are
 // rotated by the angle whose cos/sin the caller tabulates per (token, i)  (reading R-23).
 //
+// Two kernels: the CTA-pair kernel below (cta_group::2, 256 x 256 tiles; default when the output width allows) and this
+// single-CTA kernel (128 x 256 or 128 x 128 tiles), which also serves as the fallback (HCMS_GEMM_2CTA=0).
 // Persistent kernel, one CTA per SM, 256 threads:
 //   warp 0     TMA producer: A tile [128 x 64] and B tile [BN x 64] per k-block into a shared-memory ring
 //   warp 1     MMA issuer (one elected lane): tcgen05.mma.cta_group::1.kind::f16, M=128, N=BN, K=16, SS
@@ -292,6 +294,219 @@ gemm_bf16_nt_kernel(const __grid_constant__ GemmMaps maps, const __grid_constant
 }  // namespace
 
 // ------------------------------------------------------------------------------------------
+// CTA-pair variant (tcgen05 cta_group::2): a cluster of two CTAs on one TPC computes a 256 x 256 tile.  Each CTA
+// loads its own 128 rows of A and HALF of the B tile (128 of the 256 weight rows); one thread of the leader CTA issues
+// M=256 MMAs that read A and B from both CTAs' shared memory and write each CTA's 128 accumulator rows into its own
+// TMEM.  Per CTA this halves the B traffic into and out of shared memory and the number of MMA instructions.
+// Barriers: `full` lives in the leader (both CTAs' TMA bytes are counted there), `empty` and `acc_full` are signalled
+// in both CTAs by multicast commits, `acc_empty` lives in the leader and collects the epilogue warps of both CTAs.
+// ------------------------------------------------------------------------------------------
+struct Cfg2 {
+  static constexpr int kBN = 256;
+  static constexpr int kBHalfBytes = (kBN / 2) * kBK * 2;
+  static constexpr int kStageBytes = kABytes + kBHalfBytes;     // per CTA
+  static constexpr int kStages = 6;
+  static constexpr int kSmemBytes = kStages * kStageBytes + 2 * kEpiPanelBytes + 1024 + 256;
+  static constexpr int kTmemCols = 2 * kBN;
+};
+
+template <int kMode>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
+gemm_bf16_nt_2cta_kernel(const __grid_constant__ GemmMaps maps, const __grid_constant__ ChunkMaps cmaps, const GemmParams prm) {
+  using C = Cfg2;
+  constexpr int BN = C::kBN;
+  constexpr int kStages = C::kStages;
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t ring = smem_base;
+  const uint32_t epi = ring + kStages * C::kStageBytes;
+  const uint32_t bar_base = epi + 2 * kEpiPanelBytes;
+  const uint32_t bar_full = bar_base;                       // [kStages] leader only: TMA of both CTAs -> MMA
+  const uint32_t bar_empty = bar_full + 8 * kStages;        // [kStages] per CTA: MMA -> TMA (multicast commit)
+  const uint32_t bar_acc_full = bar_empty + 8 * kStages;    // [2] per CTA: MMA -> epilogue (multicast commit)
+  const uint32_t bar_acc_empty = bar_acc_full + 16;         // [2] leader only: epilogue warps of both CTAs -> MMA
+  const uint32_t tmem_slot = bar_acc_empty + 16;
+
+  const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
+  const int lane = threadIdx.x & 31;
+  const uint32_t rank = cluster_ctarank();
+  const int cluster_id = blockIdx.x >> 1, n_clusters = gridDim.x >> 1;
+  const int total_tiles = prm.m_tiles * prm.n_tiles;       // m_tiles counts 256-row cluster tiles here
+  const int n_kb = (prm.K + kBK - 1) / kBK;
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < kStages; ++s) {
+      mbar_init(bar_full + 8 * s, 1);
+      mbar_init(bar_empty + 8 * s, 1);
+    }
+    for (int a = 0; a < 2; ++a) {
+      mbar_init(bar_acc_full + 8 * a, 1);
+      mbar_init(bar_acc_empty + 8 * a, 8);   // 4 epilogue warps x 2 CTAs
+    }
+    fence_mbar_init();
+    fence_proxy_async_smem();
+  }
+  if (warp == 2) {
+    tmem_alloc_2sm(tmem_slot, C::kTmemCols);
+    tmem_relinquish_2sm();
+  }
+  tc_fence_before();
+  cluster_sync();
+  tc_fence_after();
+  uint32_t tmem_base;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+
+  if (warp == 0) {
+    // ---------------- TMA producer (both CTAs) ----------------
+    const bool leader = elect_one();
+    if (leader) {
+      prefetch_tensormap(&maps.a);
+      prefetch_tensormap(&maps.b);
+    }
+    int stage = 0;
+    uint32_t phase = 0;
+    for (int tile = cluster_id; tile < total_tiles; tile += n_clusters) {
+      int m0, n0;
+      tile_coords(tile, prm, m0, n0);
+      m0 = 2 * m0 + static_cast<int>(rank) * kBM;            // tile_coords counted in units of kBM
+      n0 = n0 * BN + static_cast<int>(rank) * (BN / 2);
+      for (int kb = 0; kb < n_kb; ++kb) {
+        mbar_wait(bar_empty + 8 * stage, phase ^ 1);
+        if (leader) {
+          const uint32_t dst = ring + stage * C::kStageBytes;
+          const uint32_t full0 = mapa(bar_full + 8 * stage, 0);
+          if (rank == 0) mbar_expect_tx(bar_full + 8 * stage, 2 * C::kStageBytes);
+          if (kMode == kFusedA) {
+            const int head = (kb * kBK) >> prm.d_shift, hr = head / prm.Hl, lh = head - hr * prm.Hl;
+            tma_load_4d_2sm(dst, &cmaps.m[prm.chunk_of[lh]], full0, (kb * kBK) & prm.d_mask, prm.j_of[lh], m0, hr);
+          } else {
+            tma_load_2d_2sm(dst, &maps.a, full0, kb * kBK, m0);
+          }
+          tma_load_2d_2sm(dst + kABytes, &maps.b, full0, kb * kBK, n0);
+        }
+        __syncwarp();
+        if (++stage == kStages) {
+          stage = 0;
+          phase ^= 1;
+        }
+      }
+    }
+  } else if (warp == 1 && rank == 0) {
+    // ---------------- MMA issuer (leader CTA) ----------------
+    const bool leader = elect_one();
+    constexpr uint32_t idesc = umma_idesc_bf16(2 * kBM, BN, false, false);
+    constexpr uint32_t hi = umma_desc_hi(1024);
+    int stage = 0;
+    uint32_t phase = 0;
+    int it = 0;
+    for (int tile = cluster_id; tile < total_tiles; tile += n_clusters, ++it) {
+      const int acc = it & 1;
+      mbar_wait(bar_acc_empty + 8 * acc, ((it >> 1) & 1) ^ 1);
+      tc_fence_after();
+      const uint32_t d_tmem = tmem_base + acc * BN;
+      for (int kb = 0; kb < n_kb; ++kb) {
+        mbar_wait(bar_full + 8 * stage, phase);
+        tc_fence_after();
+        if (leader) {
+          const uint32_t a_lo = umma_desc_lo(ring + stage * C::kStageBytes, 16);
+          const uint32_t b_lo = umma_desc_lo(ring + stage * C::kStageBytes + kABytes, 16);
+#pragma unroll
+          for (int ks = 0; ks < kBK / 16; ++ks)
+            mma_ss_lohi_2sm(d_tmem, a_lo + ks * 2, b_lo + ks * 2, hi, hi, idesc, (kb > 0 || ks > 0) ? 1u : 0u);
+          tc_commit_2sm(bar_empty + 8 * stage, 3);
+          if (kb == n_kb - 1) tc_commit_2sm(bar_acc_full + 8 * acc, 3);
+        }
+        __syncwarp();
+        if (++stage == kStages) {
+          stage = 0;
+          phase ^= 1;
+        }
+      }
+    }
+  } else if (warp >= 4) {
+    // ---------------- epilogue (both CTAs, each its own 128 rows) ----------------
+    const int ew = warp & 3;
+    const int row = ew * 32 + lane;
+    const uint32_t lane_addr = static_cast<uint32_t>(ew * 32) << 16;
+    const uint32_t swz = static_cast<uint32_t>(row & 7);
+    const bool issuer = threadIdx.x == 128;
+    int it = 0;
+    for (int tile = cluster_id; tile < total_tiles; tile += n_clusters, ++it) {
+      const int acc = it & 1;
+      int m0, n0;
+      tile_coords(tile, prm, m0, n0);
+      m0 = 2 * m0 + static_cast<int>(rank) * kBM;
+      n0 *= BN;
+      const int t_out = n0 / prm.n_per_out;
+      const int col0 = n0 - t_out * prm.n_per_out;
+      const bool rope = t_out < prm.rope_outs;
+      const int grow = min(m0 + row, prm.M - 1);
+      mbar_wait(bar_acc_full + 8 * acc, (it >> 1) & 1);
+      tc_fence_after();
+#pragma unroll 1
+      for (int ch = 0; ch < BN / 64; ++ch) {
+        const uint32_t buf = epi + (ch & 1) * kEpiPanelBytes;
+        if (issuer) bulk_wait_read<1>();
+        named_bar_sync(1, 128);
+#pragma unroll
+        for (int half = 0; half < 2; ++half) {
+          uint32_t r[32];
+          tmem_ld32(tmem_base + lane_addr + acc * BN + ch * 64 + half * 32, r);
+          tmem_wait_ld();
+          if (rope) {
+            const int pair0 = (((col0 + ch * 64 + half * 32) & prm.d_mask) >> 1);
+            const float4* cp = reinterpret_cast<const float4*>(prm.cos + static_cast<size_t>(grow) * prm.half_d + pair0);
+            const float4* sp = reinterpret_cast<const float4*>(prm.sin + static_cast<size_t>(grow) * prm.half_d + pair0);
+#pragma unroll
+            for (int g = 0; g < 4; ++g) {
+              const float4 c4 = __ldg(cp + g), s4 = __ldg(sp + g);
+              const float cs[4] = {c4.x, c4.y, c4.z, c4.w}, sn[4] = {s4.x, s4.y, s4.z, s4.w};
+#pragma unroll
+              for (int e = 0; e < 4; ++e) {
+                const float a = __uint_as_float(r[g * 8 + 2 * e]), b = __uint_as_float(r[g * 8 + 2 * e + 1]);
+                r[g * 8 + 2 * e] = __float_as_uint(a * cs[e] - b * sn[e]);
+                r[g * 8 + 2 * e + 1] = __float_as_uint(a * sn[e] + b * cs[e]);
+              }
+            }
+          }
+#pragma unroll
+          for (int q4 = 0; q4 < 4; ++q4) {
+            uint32_t w[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e)
+              w[e] = pack_bf16(__uint_as_float(r[q4 * 8 + 2 * e]), __uint_as_float(r[q4 * 8 + 2 * e + 1]));
+            const uint32_t chunk = half * 4 + q4;
+            st_shared_v4(buf + row * 128 + ((chunk ^ swz) << 4), w[0], w[1], w[2], w[3]);
+          }
+        }
+        if (ch == BN / 64 - 1) {
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive_cluster(mapa(bar_acc_empty + 8 * acc, 0));
+        }
+        fence_proxy_async_smem();
+        named_bar_sync(1, 128);
+        if (issuer && m0 < prm.M) {
+          if (kMode == kFusedOut) {
+            const int within = col0 + ch * 64;
+            const int head = within >> prm.d_shift, hr = head / prm.Hl, lh = head - hr * prm.Hl;
+            tma_store_4d(&cmaps.m[t_out * prm.C + prm.chunk_of[lh]], buf, within & prm.d_mask, prm.j_of[lh], m0, hr);
+          } else {
+            tma_store_2d(&maps.out[t_out], buf, col0 + ch * 64, m0);
+          }
+        }
+        if (issuer) bulk_commit();
+      }
+    }
+    if (issuer) bulk_wait<0>();
+  }
+
+  tc_fence_before();
+  cluster_sync();
+  if (warp == 2) tmem_dealloc_2sm(tmem_base, C::kTmemCols);
+}
+
+// ------------------------------------------------------------------------------------------
 // host side
 // ------------------------------------------------------------------------------------------
 namespace {
@@ -316,11 +531,21 @@ int group_m_setting() {
   return v;
 }
 
-template <int BN, int kMode>
+// HCMS_GEMM_2CTA=0/1 selects the single-CTA or the CTA-pair kernel for shapes with n_per_out % 256 == 0 (read once).
+bool pair_setting() {
+  static int v = -1;
+  if (v < 0) {
+    const char* e = std::getenv("HCMS_GEMM_2CTA");
+    v = e ? (std::atoi(e) != 0) : 1;   // measured on B200: 1527 vs 1416 TFLOP/s on the cfg 3 QKV projection
+  }
+  return v != 0;
+}
+
+template <int BN, int kMode, bool k2Cta>
 cudaError_t launch(const GemmArgs& a, cudaStream_t stream) {
   GemmMaps maps;
   ChunkMaps cmaps;
-  cudaError_t e = map2d(&maps.b, a.b, static_cast<uint64_t>(a.K), static_cast<uint64_t>(a.N), kBK, BN);
+  cudaError_t e = map2d(&maps.b, a.b, static_cast<uint64_t>(a.K), static_cast<uint64_t>(a.N), kBK, k2Cta ? BN / 2 : BN);
   if (e != cudaSuccess) return e;
   GemmParams p{};
   const int n_out = a.N / a.n_per_out;
@@ -377,12 +602,20 @@ cudaError_t launch(const GemmArgs& a, cudaStream_t stream) {
   p.d_mask = a.D - 1;
   p.cos = a.cos;
   p.sin = a.sin;
-  p.m_tiles = static_cast<int>((a.M + kBM - 1) / kBM);
   p.n_tiles = a.N / BN;
-  p.group_m = group_m_setting();
-  const int total = p.m_tiles * p.n_tiles;
-  const int grid = total < a.num_sms ? total : a.num_sms;
-  gemm_bf16_nt_kernel<BN, kMode><<<grid, kThreads, Cfg<BN>::kSmemBytes, stream>>>(maps, cmaps, p);
+  if (k2Cta) {
+    p.m_tiles = static_cast<int>((a.M + 2 * kBM - 1) / (2 * kBM));     // 256-row tiles of a CTA pair
+    p.group_m = (group_m_setting() + 1) / 2;
+    const int total = p.m_tiles * p.n_tiles, pairs = a.num_sms / 2;
+    const int grid = 2 * (total < pairs ? total : pairs);
+    gemm_bf16_nt_2cta_kernel<kMode><<<grid, kThreads, Cfg2::kSmemBytes, stream>>>(maps, cmaps, p);
+  } else {
+    p.m_tiles = static_cast<int>((a.M + kBM - 1) / kBM);
+    p.group_m = group_m_setting();
+    const int total = p.m_tiles * p.n_tiles;
+    const int grid = total < a.num_sms ? total : a.num_sms;
+    gemm_bf16_nt_kernel<BN, kMode><<<grid, kThreads, Cfg<BN>::kSmemBytes, stream>>>(maps, cmaps, p);
+  }
   return cudaGetLastError();
 }
 
@@ -401,6 +634,9 @@ cudaError_t gemm_init() {
     set(gemm_bf16_nt_kernel<128, kFusedOut>, Cfg<128>::kSmemBytes);
     set(gemm_bf16_nt_kernel<256, kFusedA>, Cfg<256>::kSmemBytes);
     set(gemm_bf16_nt_kernel<128, kFusedA>, Cfg<128>::kSmemBytes);
+    set(gemm_bf16_nt_2cta_kernel<kPlain>, Cfg2::kSmemBytes);
+    set(gemm_bf16_nt_2cta_kernel<kFusedOut>, Cfg2::kSmemBytes);
+    set(gemm_bf16_nt_2cta_kernel<kFusedA>, Cfg2::kSmemBytes);
   });
   return status;
 }
@@ -411,9 +647,14 @@ cudaError_t launch_gemm(const GemmArgs& a, cudaStream_t stream) {
   cudaError_t e = gemm_init();
   if (e != cudaSuccess) return e;
   const bool wide = a.n_per_out % 256 == 0;
-  if (a.fuse == 1) return wide ? launch<256, kFusedOut>(a, stream) : launch<128, kFusedOut>(a, stream);
-  if (a.fuse == 2) return wide ? launch<256, kFusedA>(a, stream) : launch<128, kFusedA>(a, stream);
-  return wide ? launch<256, kPlain>(a, stream) : launch<128, kPlain>(a, stream);
+  if (wide && pair_setting()) {   // CTA pairs (cta_group::2), 256 x 256 tiles
+    if (a.fuse == 1) return launch<256, kFusedOut, true>(a, stream);
+    if (a.fuse == 2) return launch<256, kFusedA, true>(a, stream);
+    return launch<256, kPlain, true>(a, stream);
+  }
+  if (a.fuse == 1) return wide ? launch<256, kFusedOut, false>(a, stream) : launch<128, kFusedOut, false>(a, stream);
+  if (a.fuse == 2) return wide ? launch<256, kFusedA, false>(a, stream) : launch<128, kFusedA, false>(a, stream);
+  return wide ? launch<256, kPlain, false>(a, stream) : launch<128, kPlain, false>(a, stream);
 }
 
 }  // namespace hcms
