@@ -46,13 +46,18 @@ constexpr float kRescaleThreshold = 8.0f;  // log2 units: rescale O only if the 
 constexpr int kPanelBytes = 128 * 128;     // one 128-byte-swizzle panel: 128 rows x 128 B
 constexpr int kPTileBytes = 2 * kPanelBytes;  // P_t: 128 rows x 128 keys bf16
 
-template <int D>
+// kPair: the CTA-pair variant (tcgen05 cta_group::2, D = 128 only).  Two CTAs of a cluster share every K_j / V_j tile:
+// each loads HALF of it (64 of the 128 keys of K_j; 64 of the 128 head-dim columns of V_j) and the leader CTA issues
+// M = 256 MMAs over both CTAs' query tiles, so per CTA the K/V traffic into and out of shared memory and the number
+// of MMA instructions are halved.
+template <int D, bool kPair = false>
 struct Cfg {
   static constexpr int kPanels = D / 64;                    // 128-byte swizzle panels along D
   static constexpr int kTileBytes = kPanels * kPanelBytes;  // one Q / K / V tile
-  static constexpr int kStages = D == 128 ? 3 : 6;          // KV ring stages (each holds one K tile or one V tile)
+  static constexpr int kKvBytes = kPair ? kTileBytes / 2 : kTileBytes;   // what one ring stage holds
+  static constexpr int kStages = D == 128 ? (kPair ? 6 : 3) : 6;          // KV ring stages (one K or one V (half) tile each)
   static constexpr int kSmemBytes =
-      kQTiles * kTileBytes + kQTiles * kPTileBytes + kStages * kTileBytes + 1024 /*align*/ + 256 /*barriers*/;
+      kQTiles * kTileBytes + kQTiles * kPTileBytes + kStages * kKvBytes + 1024 /*align*/ + 256 /*barriers*/;
   static constexpr int kTmemS = 0;                          // S_t at kTmemS + t*128
   static constexpr int kTmemO = 256;                        // O_t at kTmemO + t*D
 };
@@ -86,6 +91,7 @@ __host__ __device__ constexpr uint32_t make_idesc(int M, int N, bool b_mn_major)
 
 struct alignas(64) AttnMaps {
   CUtensorMap q, k, v, o;   // rank-4 {D, h_c, S, P}, box {64, 1, 128, 1}, SWIZZLE_128B
+  CUtensorMap kh;           // K with box {64, 1, 64, 1}: the half tile a CTA of a pair loads
 };
 
 struct AttnParams {
@@ -171,17 +177,17 @@ __device__ __forceinline__ void st_shared_v4(uint32_t addr, uint32_t a, uint32_t
 }
 
 // kPoly: of every 8 consecutive column pairs, this many take the polynomial path (the rest MUFU).
-template <int D, int kPoly>
+template <int D, int kPoly, bool kPair>
 __global__ void __launch_bounds__(kThreads, 1)
 attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm) {
-  using C = Cfg<D>;
+  using C = Cfg<D, kPair>;
   constexpr int kStages = C::kStages;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t q_smem = smem_base;                                  // kQTiles Q tiles
   const uint32_t p_smem = q_smem + kQTiles * C::kTileBytes;           // kQTiles P tiles
   const uint32_t kv_smem = p_smem + kQTiles * kPTileBytes;            // kStages K/V tiles
-  const uint32_t bar_base = kv_smem + kStages * C::kTileBytes;        // 8-byte barriers
+  const uint32_t bar_base = kv_smem + kStages * C::kKvBytes;          // 8-byte barriers
   const uint32_t bar_q_full = bar_base;                       // [2]  TMA -> MMA
   const uint32_t bar_kv_full = bar_q_full + 16;               // [kStages] TMA -> MMA
   const uint32_t bar_kv_empty = bar_kv_full + 8 * kStages;    // [kStages] MMA -> TMA
@@ -193,6 +199,7 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
 
   const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);   // warp-uniform by construction
   const int lane = threadIdx.x & 31;
+  const uint32_t cr = kPair ? cluster_ctarank() : 0u;   // rank in the CTA pair; the leader (0) issues the MMAs
   const int head = blockIdx.y;                 // p*h_c + j
   const int rank = head / prm.h_c;
   const int hj = head - rank * prm.h_c;
@@ -203,8 +210,8 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
     for (int t = 0; t < kQTiles; ++t) {
       mbar_init(bar_q_full + 8 * t, 1);
       mbar_init(bar_s_full + 8 * t, 1);
-      mbar_init(bar_s_free + 8 * t, 4);     // one elected lane per softmax warp
-      mbar_init(bar_p_full + 8 * t, 4);
+      mbar_init(bar_s_free + 8 * t, kPair ? 8 : 4);     // one elected lane per softmax warp (of both CTAs of a pair)
+      mbar_init(bar_p_full + 8 * t, kPair ? 8 : 4);
       mbar_init(bar_pv_done + 8 * t, 1);
     }
     for (int s = 0; s < kStages; ++s) {
@@ -215,11 +222,16 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
     fence_proxy_async_smem();
   }
   if (warp == 2) {
-    tmem_alloc(tmem_slot, kTmemCols);
-    tmem_relinquish();
+    if (kPair) {
+      tmem_alloc_2sm(tmem_slot, kTmemCols);
+      tmem_relinquish_2sm();
+    } else {
+      tmem_alloc(tmem_slot, kTmemCols);
+      tmem_relinquish();
+    }
   }
   tc_fence_before();
-  __syncthreads();
+  if (kPair) cluster_sync(); else __syncthreads();
   tc_fence_after();
   uint32_t tmem_base;
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
@@ -238,37 +250,72 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
         prefetch_tensormap(&maps.k);
         prefetch_tensormap(&maps.v);
       }
+      // Pair: every byte count lives on the LEADER's barrier (both CTAs' TMA complete there); each CTA loads its own
+      // Q rows, keys [j*128 + cr*64, +64) of K_j (D/64 panels of 64 rows) and head-dim columns [cr*64, +64) of V_j.
       auto load_tile = [&](const CUtensorMap* tm, uint32_t dst, uint32_t bar, int row0) {
         if (leader) {
-          mbar_expect_tx(bar, C::kTileBytes);
+          if (kPair) {
+            if (cr == 0) mbar_expect_tx(bar, 2 * C::kTileBytes);
+            const uint32_t bar0 = mapa(bar, 0);
 #pragma unroll
-          for (int pn = 0; pn < C::kPanels; ++pn) tma_load_4d(dst + pn * kPanelBytes, tm, bar, pn * 64, hj, row0, rank);
+            for (int pn = 0; pn < C::kPanels; ++pn) tma_load_4d_2sm(dst + pn * kPanelBytes, tm, bar0, pn * 64, hj, row0, rank);
+          } else {
+            mbar_expect_tx(bar, C::kTileBytes);
+#pragma unroll
+            for (int pn = 0; pn < C::kPanels; ++pn) tma_load_4d(dst + pn * kPanelBytes, tm, bar, pn * 64, hj, row0, rank);
+          }
         }
         __syncwarp();
       };
       int stage = 0;
       uint32_t phase = 0;  // ring items are loaded in consumption order
-      auto load_kv = [&](const CUtensorMap* tm, int j) {
+      auto load_kv = [&](bool is_v, int j) {
         mbar_wait(bar_kv_empty + 8 * stage, phase ^ 1);
-        load_tile(tm, kv_smem + stage * C::kTileBytes, bar_kv_full + 8 * stage, j * kBN);
+        const uint32_t dst = kv_smem + stage * C::kKvBytes, bar = bar_kv_full + 8 * stage;
+        if (kPair) {
+          if (leader) {
+            if (cr == 0) mbar_expect_tx(bar, 2 * C::kKvBytes);
+            const uint32_t bar0 = mapa(bar, 0);
+            if (is_v) {
+              tma_load_4d_2sm(dst, &maps.v, bar0, static_cast<int>(cr) * 64, hj, j * kBN, rank);
+            } else {
+#pragma unroll
+              for (int pn = 0; pn < C::kPanels; ++pn)
+                tma_load_4d_2sm(dst + pn * (kPanelBytes / 2), &maps.kh, bar0, pn * 64, hj, j * kBN + static_cast<int>(cr) * 64, rank);
+            }
+          }
+          __syncwarp();
+        } else {
+          load_tile(is_v ? &maps.v : &maps.k, dst, bar, j * kBN);
+        }
         if (++stage == kStages) {
           stage = 0;
           phase ^= 1;
         }
       };
       load_tile(&maps.q, q_smem, bar_q_full, q_row0);
-      load_kv(&maps.k, 0);
+      load_kv(false, 0);
       load_tile(&maps.q, q_smem + C::kTileBytes, bar_q_full + 8, q_row0 + kBM);
       for (int j = 0; j < n_kv; ++j) {
-        if (j + 1 < n_kv) load_kv(&maps.k, j + 1);
-        load_kv(&maps.v, j);
+        if (j + 1 < n_kv) load_kv(false, j + 1);
+        load_kv(true, j);
       }
-    } else if (warp == 1) {
-      // ---------------- MMA issuer ----------------
+    } else if (warp == 1 && (!kPair || cr == 0)) {
+      // ---------------- MMA issuer (pair: the leader CTA issues M = 256 MMAs over both CTAs' query tiles) ----------------
       const bool leader = elect_one();
-      constexpr uint32_t idesc_qk = make_idesc(kBM, kBN, false);
-      constexpr uint32_t idesc_pv = make_idesc(kBM, D, true);
+      constexpr uint32_t idesc_qk = make_idesc(kPair ? 2 * kBM : kBM, kBN, false);
+      constexpr uint32_t idesc_pv = make_idesc(kPair ? 2 * kBM : kBM, D, true);
       constexpr uint32_t hi = desc_hi(1024);                 // SBO = 1024 B for every operand
+      auto mma = [&](uint32_t d, uint32_t a_lo, uint32_t b_lo, uint32_t idesc, uint32_t acc) {
+        if (kPair) mma_ss_lohi_2sm(d, a_lo, b_lo, hi, hi, idesc, acc); else mma_ss_lohi(d, a_lo, b_lo, hi, hi, idesc, acc);
+      };
+      auto commit = [&](uint32_t bar) {          // pair: the barrier at this offset in BOTH CTAs
+        if (kPair) tc_commit_2sm(bar, 3); else tc_commit(bar);
+      };
+      auto wait_softmax = [&](uint32_t bar, uint32_t parity) {   // pair: arrivals come from both CTAs' softmax warps
+        if (kPair) mbar_wait_cluster(bar, parity); else mbar_wait(bar, parity);
+      };
+      constexpr uint32_t kKPanel = kPair ? kPanelBytes / 2 : kPanelBytes;   // a K panel holds 64 or 128 keys
       auto issue_qk = [&](int t, uint32_t k_tile) {
         // S_t[128 x 128] = Q_t[128 x D] * K_j[128 x D]^T ; both operands K-major, 128B-swizzled panels
         const uint32_t d_tmem = tmem_base + C::kTmemS + t * kBN;
@@ -277,7 +324,8 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
 #pragma unroll
         for (int ks = 0; ks < D / 16; ++ks) {
           const uint32_t off = ((ks >> 2) * kPanelBytes + (ks & 3) * 32) >> 4;
-          mma_ss_lohi(d_tmem, q_lo + off, k_lo + off, hi, hi, idesc_qk, ks > 0 ? 1u : 0u);
+          const uint32_t k_off = ((ks >> 2) * kKPanel + (ks & 3) * 32) >> 4;
+          mma(d_tmem, q_lo + off, k_lo + k_off, idesc_qk, ks > 0 ? 1u : 0u);
         }
       };
       auto issue_pv = [&](int t, uint32_t v_tile, bool accumulate) {
@@ -289,17 +337,17 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
 #pragma unroll
         for (int ks = 0; ks < kBN / 16; ++ks) {
           const uint32_t off = ((ks >> 2) * kPanelBytes + (ks & 3) * 32) >> 4;
-          mma_ss_lohi(d_tmem, p_lo + off, v_lo + ks * (2048 >> 4), hi, hi, idesc_pv, (accumulate || ks > 0) ? 1u : 0u);
+          mma(d_tmem, p_lo + off, v_lo + ks * (2048 >> 4), idesc_pv, (accumulate || ks > 0) ? 1u : 0u);
         }
       };
       int stage = 0;
       uint32_t phase = 0;
       auto kv_wait = [&]() -> uint32_t {
         mbar_wait(bar_kv_full + 8 * stage, phase);
-        return kv_smem + stage * C::kTileBytes;
+        return kv_smem + stage * C::kKvBytes;
       };
       auto kv_release = [&]() {
-        if (leader) tc_commit(bar_kv_empty + 8 * stage);
+        if (leader) commit(bar_kv_empty + 8 * stage);
         __syncwarp();
         if (++stage == kStages) {
           stage = 0;
@@ -316,7 +364,7 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
           tc_fence_after();
           if (leader) {
             issue_qk(t, k_tile);
-            tc_commit(bar_s_full + 8 * t);
+            commit(bar_s_full + 8 * t);
           }
           __syncwarp();
         }
@@ -327,11 +375,11 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
           const uint32_t k_tile = kv_wait();
 #pragma unroll
           for (int t = 0; t < kQTiles; ++t) {
-            mbar_wait(bar_s_free + 8 * t, j & 1);     // S_t(j) sits in the softmax registers
+            wait_softmax(bar_s_free + 8 * t, j & 1);  // S_t(j) sits in the softmax registers
             tc_fence_after();
             if (leader) {
               issue_qk(t, k_tile);
-              tc_commit(bar_s_full + 8 * t);
+              commit(bar_s_full + 8 * t);
             }
             __syncwarp();
           }
@@ -340,11 +388,11 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
         const uint32_t v_tile = kv_wait();
 #pragma unroll
         for (int t = 0; t < kQTiles; ++t) {
-          mbar_wait(bar_p_full + 8 * t, j & 1);       // P_t(j) stored, O_t rescaled if needed
+          wait_softmax(bar_p_full + 8 * t, j & 1);    // P_t(j) stored, O_t rescaled if needed
           tc_fence_after();
           if (leader) {
             issue_pv(t, v_tile, j > 0);
-            tc_commit(bar_pv_done + 8 * t);
+            commit(bar_pv_done + 8 * t);
           }
           __syncwarp();
         }
@@ -379,7 +427,9 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
       tmem_wait_ld();
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(bar_s_free + 8 * t);    // QK_t(j+1) may overwrite S_t now
+      if (lane == 0) {                                   // QK_t(j+1) may overwrite S_t now
+        if (kPair) mbar_arrive_cluster(mapa(bar_s_free + 8 * t, 0)); else mbar_arrive(bar_s_free + 8 * t);
+      }
       if (j == n_kv - 1 && tail_valid < kBN) {
 #pragma unroll
         for (int c = 0; c < kBN; ++c)
@@ -463,7 +513,9 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
       }
       fence_proxy_async_smem();     // generic-proxy stores -> visible to the tensor core's async-proxy reads
       __syncwarp();
-      if (lane == 0) mbar_arrive(bar_p_full + 8 * t);
+      if (lane == 0) {
+        if (kPair) mbar_arrive_cluster(mapa(bar_p_full + 8 * t, 0)); else mbar_arrive(bar_p_full + 8 * t);
+      }
     }
 
     // ---------------- epilogue: O_t / l -> bf16 -> swizzled smem (P_t's buffer) -> TMA store ----------------
@@ -510,8 +562,13 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
   }
 
   tc_fence_before();
-  __syncthreads();
-  if (warp == 2) tmem_dealloc(tmem_base, kTmemCols);
+  if (kPair) {       // neither CTA may exit while the pair's MMAs can still read its shared memory or signal its barriers
+    cluster_sync();
+    if (warp == 2) tmem_dealloc_2sm(tmem_base, kTmemCols);
+  } else {
+    __syncthreads();
+    if (warp == 2) tmem_dealloc(tmem_base, kTmemCols);
+  }
 }
 
 cudaError_t make_maps(const AttnArgs& a, AttnMaps* m) {
@@ -527,7 +584,8 @@ cudaError_t make_maps(const AttnArgs& a, AttnMaps* m) {
                                       CU_TENSOR_MAP_SWIZZLE_128B);
     if (e != cudaSuccess) return e;
   }
-  return cudaSuccess;
+  const uint32_t box_half[4] = {64, 1, 64, 1};
+  return encode_tensor_map(&m->kh, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, a.k, dims, strides, box_half, CU_TENSOR_MAP_SWIZZLE_128B);
 }
 
 using KernelFn = void (*)(const AttnMaps, const AttnParams);
@@ -544,18 +602,28 @@ int poly_setting() {
   return v;
 }
 
-template <int D>
+template <int D, bool kPair = false>
 KernelFn pick_kernel(int poly) {
   switch (poly) {
-    case 0: return attention_fwd_kernel<D, 0>;
-    case 1: return attention_fwd_kernel<D, 1>;
-    case 3: return attention_fwd_kernel<D, 3>;
-    case 4: return attention_fwd_kernel<D, 4>;
-    case 5: return attention_fwd_kernel<D, 5>;
-    case 6: return attention_fwd_kernel<D, 6>;
-    case 8: return attention_fwd_kernel<D, 8>;
-    default: return attention_fwd_kernel<D, 2>;
+    case 0: return attention_fwd_kernel<D, 0, kPair>;
+    case 1: return attention_fwd_kernel<D, 1, kPair>;
+    case 3: return attention_fwd_kernel<D, 3, kPair>;
+    case 4: return attention_fwd_kernel<D, 4, kPair>;
+    case 5: return attention_fwd_kernel<D, 5, kPair>;
+    case 6: return attention_fwd_kernel<D, 6, kPair>;
+    case 8: return attention_fwd_kernel<D, 8, kPair>;
+    default: return attention_fwd_kernel<D, 2, kPair>;
   }
+}
+
+// HCMS_ATTN_PAIR=0/1: single-CTA kernel or the CTA-pair kernel (D = 128 only); read once.
+bool pair_setting() {
+  static int v = -1;
+  if (v < 0) {
+    const char* e = std::getenv("HCMS_ATTN_PAIR");
+    v = e ? (std::atoi(e) != 0) : 0;
+  }
+  return v != 0;
 }
 
 }  // namespace
@@ -566,6 +634,9 @@ cudaError_t attention_init() {
                                          Cfg<128>::kSmemBytes);
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(pick_kernel<64>(poly), cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg<64>::kSmemBytes);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(pick_kernel<128, true>(poly), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             Cfg<128, true>::kSmemBytes);
     if (e != cudaSuccess) return e;
   }
   return cudaSuccess;
@@ -585,6 +656,23 @@ cudaError_t launch_attention(const AttnArgs& a, cudaStream_t stream) {
   prm.lse = a.lse;
   dim3 grid(static_cast<unsigned>((a.S + kQTiles * kBM - 1) / (kQTiles * kBM)), static_cast<unsigned>(a.P * a.h_c));
   const int poly = poly_setting();
+  if (a.D == 128 && pair_setting()) {
+    // CTA pairs: a cluster of 2 consecutive CTAs (512 query rows) per launch unit; an odd block count is padded by
+    // one CTA whose query rows do not exist (its loads are zero fill, its stores are skipped)
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((grid.x + 1) / 2 * 2, grid.y);
+    cfg.blockDim = dim3(kThreads);
+    cfg.dynamicSmemBytes = Cfg<128, true>::kSmemBytes;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr{};
+    attr.id = cudaLaunchAttributeClusterDimension;
+    attr.val.clusterDim.x = 2;
+    attr.val.clusterDim.y = 1;
+    attr.val.clusterDim.z = 1;
+    cfg.attrs = &attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, pick_kernel<128, true>(poly), maps, prm);
+  }
   if (a.D == 128)
     pick_kernel<128>(poly)<<<grid, kThreads, Cfg<128>::kSmemBytes, stream>>>(maps, prm);
   else if (a.D == 64)
