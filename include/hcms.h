@@ -107,6 +107,12 @@ enum {
                                           addresses or another scale capture again.  For launch-bound shapes
                                           (BASELINE.json configs 1-2).  Same bits.  Excludes HCMS_FLAG_PROFILE. */
 
+#define HCMS_FLAG_ATTN_PAIR 0x4000u    /* D = 128 only: the attention forward runs on CTA pairs (thread-block clusters of 2,
+                                          tcgen05 cta_group::2): the two CTAs share every K_j / V_j tile (each loads
+                                          half) and the leader CTA issues M = 256 MMAs over both CTAs' query tiles.
+                                          Same bits as the single-CTA kernel.  Measured on B200 (cfg 3): -13 % power at
+                                          equal clocks, +0.5 % throughput under the power cap; off by default. */
+
 typedef struct hcms_plan hcms_plan_t;
 
 /* ---- introspection (host only, no GPU needed) ---------------------------------------- */

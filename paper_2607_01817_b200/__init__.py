@@ -44,6 +44,7 @@ HCMS_FLAG_SINGLE_COMP = 0x400
 HCMS_FLAG_TRAINING = 0x800
 HCMS_FLAG_FUSE_A2A = 0x1000
 HCMS_FLAG_GRAPH = 0x2000
+HCMS_FLAG_ATTN_PAIR = 0x4000
 
 # every symbol include/hcms.h declares: name -> (restype, argtypes)
 _SIGNATURES = {

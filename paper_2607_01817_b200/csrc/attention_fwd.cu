@@ -19,6 +19,13 @@
 // when P_t(j) has been stored.  The softmax chain (S(j) -> P(j) -> S(j+1) ...) therefore never waits for a
 // tensor-core round trip, and the tensor queue always holds the next GEMM (measured: the QK/PV instruction
 // mix runs at the full 8192 flop/clk/SM with P in shared memory, with or without concurrent P stores).
+// Pair variant: the softmax warps of the peer CTA signal the leader's barriers with RELAXED cluster-scope arrives.  A
+// release.cluster arrive costs a cluster-wide fence per warp and iteration (measured: 20.7 ms instead of 16.4 ms at
+// BASELINE config 3).  What the leader's MMAs read after the arrive is (a) S columns already pulled out of TMEM,
+// ordered by tcgen05.wait::ld + tcgen05.fence::before_thread_sync, and (b) the P tile in the arriving CTA's own
+// shared memory, which every lane has pushed through fence.proxy.async before the __syncwarp that precedes the
+// arrive; the leader waits with acquire.cluster.  tests/test_gpu_attention.py compares the pair kernel bit for bit
+// with the single-CTA kernel at full size under NaN poisoning.
 // The exponentials are split between the MUFU pipe (ex2.approx) and a degree-3 polynomial on the FMA pipe
 // (packed f32x2 arithmetic), since 16 ex2/clk/SM would otherwise co-limit the kernel at exactly the MMA time.
 //
@@ -428,7 +435,7 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
       tc_fence_before();
       __syncwarp();
       if (lane == 0) {                                   // QK_t(j+1) may overwrite S_t now
-        if (kPair) mbar_arrive_cluster(mapa(bar_s_free + 8 * t, 0)); else mbar_arrive(bar_s_free + 8 * t);
+        if (kPair) mbar_arrive_cluster_relaxed(mapa(bar_s_free + 8 * t, 0)); else mbar_arrive(bar_s_free + 8 * t);
       }
       if (j == n_kv - 1 && tail_valid < kBN) {
 #pragma unroll
@@ -514,7 +521,7 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
       fence_proxy_async_smem();     // generic-proxy stores -> visible to the tensor core's async-proxy reads
       __syncwarp();
       if (lane == 0) {
-        if (kPair) mbar_arrive_cluster(mapa(bar_p_full + 8 * t, 0)); else mbar_arrive(bar_p_full + 8 * t);
+        if (kPair) mbar_arrive_cluster_relaxed(mapa(bar_p_full + 8 * t, 0)); else mbar_arrive(bar_p_full + 8 * t);
       }
     }
 
@@ -616,7 +623,8 @@ KernelFn pick_kernel(int poly) {
   }
 }
 
-// HCMS_ATTN_PAIR=0/1: single-CTA kernel or the CTA-pair kernel (D = 128 only); read once.
+// HCMS_ATTN_PAIR=1 selects the CTA-pair kernel for every D = 128 launch of the process (tuning runs; read once);
+// HCMS_FLAG_ATTN_PAIR selects it per plan.
 bool pair_setting() {
   static int v = -1;
   if (v < 0) {
@@ -656,7 +664,7 @@ cudaError_t launch_attention(const AttnArgs& a, cudaStream_t stream) {
   prm.lse = a.lse;
   dim3 grid(static_cast<unsigned>((a.S + kQTiles * kBM - 1) / (kQTiles * kBM)), static_cast<unsigned>(a.P * a.h_c));
   const int poly = poly_setting();
-  if (a.D == 128 && pair_setting()) {
+  if (a.D == 128 && (a.pair || pair_setting())) {
     // CTA pairs: a cluster of 2 consecutive CTAs (512 query rows) per launch unit; an odd block count is padded by
     // one CTA whose query rows do not exist (its loads are zero fill, its stores are skipped)
     cudaLaunchConfig_t cfg{};

@@ -61,6 +61,7 @@ struct AttnArgs {
   int D, P, h_c;
   float scale;
   float* lse = nullptr;   // optional [P*h_c][S] fp32: log sum_k exp(scale q.k) per row (saved for the backward)
+  bool pair = false;      // CTA-pair kernel (HCMS_FLAG_ATTN_PAIR; D = 128 only, ignored otherwise)
 };
 cudaError_t launch_attention(const AttnArgs& a, cudaStream_t stream);
 cudaError_t attention_init();  // sets kernel attributes once; resolves cuTensorMapEncodeTiled

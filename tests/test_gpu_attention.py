@@ -244,3 +244,32 @@ def test_forward_argument_errors():
         with pytest.raises(H.HcmsError) as ei:
             H.hcms_attention_forward(plan32, q, k, v, out, 0.125)
         assert ei.value.status == H.HCMS_ERR_UNSUPPORTED_DTYPE
+
+
+# ---------------------------------------------------------------------------------------------
+# HCMS_FLAG_ATTN_PAIR: the forward kernel on CTA pairs (tcgen05 cta_group::2)
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("S,Hh,P,C", [(1024, 4, 2, 2), (777, 2, 1, 1), (2100, 6, 2, 3), (130, 1, 1, 1)])
+def test_pair_kernel_same_bits_as_single_cta(S, Hh, P, C):
+    """The pair kernel computes every S tile, softmax and PV accumulation in the same order as the single-CTA kernel,
+    so the outputs must be bit-identical; ragged S, an odd number of 256-row blocks (the padded CTA of the last
+    pair has no rows), a single block."""
+    D = 128
+    w = I.Workload("pair", S, Hh, D, P, C, 61, "bf16", 1.0)
+    q, k, v = I.make_qkv(w)
+    a = run_forward(q, k, v, S, Hh, D, P, C, w.scale)
+    b = run_forward(q, k, v, S, Hh, D, P, C, w.scale, flags=H.HCMS_FLAG_ATTN_PAIR)
+    assert np.array_equal(a, b)
+    check(b, O.attention_full(q, k, v, w.scale), "pair kernel")
+
+
+def test_pair_kernel_cfg3_full_size_same_bits():
+    """BASELINE.json configs[2] at full size, launch configuration of the bench: 1536 + 1536 + 1024 + 1024 CTAs in
+    pairs, NaN-poisoned workspace and output; any ordering slip between the two CTAs of a pair shows as a bit."""
+    w = I.workload(3)
+    q, k, v = I.make_qkv(w)
+    a = run_forward(q, k, v, w.S, w.H, w.D, w.P, w.C, w.scale)
+    for _ in range(2):
+        b = run_forward(q, k, v, w.S, w.H, w.D, w.P, w.C, w.scale, flags=H.HCMS_FLAG_ATTN_PAIR)
+        assert np.array_equal(a, b)
