@@ -485,7 +485,7 @@ def run_hcms(args):
         result["e2e"] = {"value": round(v_e / 1e12, 2), "unit": UNIT, "h2d_bytes_per_step": 3 * tensor_bytes,
                          "d2h_bytes_per_step": tensor_bytes, "ms_per_step": round(ms_e_step, 3), "steps": n_e,
                          "host_wall_ms_per_step": round(wall_e / n_e, 3),
-                         "api": "hcms_attention_forward_host (pinned host q,k,v -> out)"}
+                         "api": "hcms_attention_forward_host (pinned host q,k,v -> out; strided H2D/D2H copies per rank and chunk are the all-to-all, overlapped with attention)"}
         same = bool(torch.equal(host_out.to(dev), out))
         result["e2e"]["bitwise_equal_to_device_path"] = same
         plan_e.close()

@@ -113,6 +113,12 @@ enum {
                                           Same bits as the single-CTA kernel.  Measured on B200 (cfg 3): -13 % power at
                                           equal clocks, +0.5 % throughput under the power cap; off by default. */
 
+#define HCMS_FLAG_HOST_STAGED 0x8000u   /* hcms_attention_forward_host copies whole tensors to device staging first and runs
+                                          the device path on them (the first implementation).  Default: the host link
+                                          is the wire -- strided cudaMemcpy2DAsync copies carry chunk c of rank p's
+                                          heads straight between the host tensors and the chunk buffers (they ARE the
+                                          all-to-all), chunk c+1's transfer overlapping chunk c's attention. */
+
 typedef struct hcms_plan hcms_plan_t;
 
 /* ---- introspection (host only, no GPU needed) ---------------------------------------- */
@@ -207,9 +213,13 @@ int hcms_attention_forward(hcms_plan_t* plan, const void* q, const void* k, cons
 
 /*
  * Same computation with HOST buffers (q,k,v,out: host pointers, bf16 [S,H,D]; pinned memory
- * makes the copies asynchronous): copies the inputs to plan-owned device staging, runs
- * hcms_attention_forward, copies `out` back and SYNCHRONISES `stream` before returning.
- * First use allocates 4*S*H*D*2 bytes of device staging inside the plan.
+ * makes the copies asynchronous) and SYNCHRONISES `stream` before returning.  Default: per head chunk,
+ * strided host-to-device copies on S_comm deliver every rank's heads of the chunk directly into Q'_c, K'_c, V'_c
+ * (the copy engines perform the input all-to-all), attention runs on S_comp as each chunk lands, strided
+ * device-to-host copies on a second communication stream return O'_c into `out` (output all-to-all + Concat);
+ * same events and ordering as hcms_attention_forward, same bits.  With HCMS_FLAG_HOST_STAGED (or SERIAL / GRAPH
+ * plans): whole tensors go to plan-owned device staging (4*S*H*D*2 bytes, allocated on first use), the device
+ * path runs on them, and `out` is copied back.
  */
 int hcms_attention_forward_host(hcms_plan_t* plan, const void* q, const void* k, const void* v, void* out,
                                 int64_t S, int H, int D, int P, int C, float scale, void* stream);

@@ -45,6 +45,7 @@ HCMS_FLAG_TRAINING = 0x800
 HCMS_FLAG_FUSE_A2A = 0x1000
 HCMS_FLAG_GRAPH = 0x2000
 HCMS_FLAG_ATTN_PAIR = 0x4000
+HCMS_FLAG_HOST_STAGED = 0x8000
 
 # every symbol include/hcms.h declares: name -> (restype, argtypes)
 _SIGNATURES = {

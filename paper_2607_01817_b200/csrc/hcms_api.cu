@@ -743,9 +743,65 @@ int hcms_attention_forward_host(hcms_plan_t* plan, const void* q, const void* k,
   if (S != sh.S || H != sh.H || D != sh.D || P != sh.P || C != sh.C)
     return fail(HCMS_ERR_PLAN_MISMATCH, "call shape differs from the plan's");
   const size_t bytes = static_cast<size_t>(S) * H * D * sh.es;
+  cudaStream_t caller = static_cast<cudaStream_t>(stream);
+  if (!(plan->flags & (HCMS_FLAG_HOST_STAGED | HCMS_FLAG_SERIAL | HCMS_FLAG_GRAPH)) && plan->dtype == HCMS_DTYPE_BF16) {
+    // The host link is the wire: strided copies on the copy engines perform the all-to-all layout change themselves.
+    // Chunk c of rank p's heads is a 2-D region of the host tensor (S rows of h_c*D elements, pitch H*D) and lands as
+    // the dense [S][h_c][D] slab of Q'_c / K'_c / V'_c; the output all-to-all is the reverse copy from O'_c into
+    // `out`.  H2D copies run on S_comm, D2H copies on the second communication stream (separate copy engines), the
+    // attention of chunk c on S_comp between them, ordered by the same events as Alg. 1: no scatter / gather
+    // kernels, no staging tensors, and the transfer of chunk c+1 overlaps the attention of chunk c.
+    int st = check_scale(scale);
+    if (st) return st;
+    if (!plan->ws) return fail(HCMS_ERR_WORKSPACE_TOO_SMALL, "plan has no workspace");
+    char* ws = static_cast<char*>(plan->ws);
+    const size_t row = static_cast<size_t>(H) * D * sh.es;       // host pitch
+    const bool dual_comp = !(plan->flags & HCMS_FLAG_SINGLE_COMP) && sh.C > 1;
+    plan->last_launches = 0;
+    HCMS_CUDA(cudaEventRecord(plan->e_main, caller));
+    for (cudaStream_t s : {plan->s_comm, plan->s_comm_out, plan->s_comp, plan->s_comp2}) HCMS_CUDA(cudaStreamWaitEvent(s, plan->e_main, 0));
+    const void* host_in[3] = {q, k, v};
+    for (int c = 0; c < sh.C; ++c) {
+      const Chunk& ck = plan->chunks[c];
+      const size_t width = static_cast<size_t>(ck.h) * D * sh.es, slab = width * S;
+      for (int t = 0; t < 3; ++t)
+        for (int p = 0; p < sh.P; ++p) {
+          const char* src = static_cast<const char*>(host_in[t]) + (static_cast<size_t>(p) * sh.Hl + ck.o) * D * sh.es;
+          HCMS_CUDA(cudaMemcpy2DAsync(ws + ck.off[t] + p * slab, width, src, row, width, S, cudaMemcpyHostToDevice, plan->s_comm));
+          plan->last_launches += 1;
+        }
+      HCMS_CUDA(cudaEventRecord(plan->e_comm[c], plan->s_comm));
+    }
+    for (int c = 0; c < sh.C; ++c) {
+      const Chunk& ck = plan->chunks[c];
+      cudaStream_t s_comp = (dual_comp && (c & 1)) ? plan->s_comp2 : plan->s_comp;
+      HCMS_CUDA(cudaStreamWaitEvent(s_comp, plan->e_comm[c], 0));
+      float* lse_c = plan->lse ? plan->lse + static_cast<size_t>(sh.P) * sh.S * ck.o : nullptr;
+      st = do_attention(plan, ws + ck.off[0], ws + ck.off[1], ws + ck.off[2], ws + ck.off[3], c, scale, s_comp, lse_c);
+      if (st) return st;
+      HCMS_CUDA(cudaEventRecord(plan->e_comp[c], s_comp));
+    }
+    for (int c = 0; c < sh.C; ++c) {
+      const Chunk& ck = plan->chunks[c];
+      const size_t width = static_cast<size_t>(ck.h) * D * sh.es, slab = width * S;
+      HCMS_CUDA(cudaStreamWaitEvent(plan->s_comm_out, plan->e_comp[c], 0));
+      for (int p = 0; p < sh.P; ++p) {
+        char* dst = static_cast<char*>(out) + (static_cast<size_t>(p) * sh.Hl + ck.o) * D * sh.es;
+        HCMS_CUDA(cudaMemcpy2DAsync(dst, row, ws + ck.off[3] + p * slab, width, width, S, cudaMemcpyDeviceToHost, plan->s_comm_out));
+        plan->last_launches += 1;
+      }
+    }
+    HCMS_CUDA(cudaEventRecord(plan->e_fin_comm, plan->s_comm_out));
+    HCMS_CUDA(cudaEventRecord(plan->e_fin_in, plan->s_comm));
+    HCMS_CUDA(cudaEventRecord(plan->e_fin_comp, plan->s_comp));
+    HCMS_CUDA(cudaEventRecord(plan->e_fin_comp2, plan->s_comp2));
+    for (cudaEvent_t e : {plan->e_fin_comm, plan->e_fin_in, plan->e_fin_comp, plan->e_fin_comp2}) HCMS_CUDA(cudaStreamWaitEvent(caller, e, 0));
+    plan->forward_done = true;
+    HCMS_CUDA(cudaStreamSynchronize(caller));
+    return HCMS_OK;
+  }
   for (int t = 0; t < 4; ++t)
     if (!plan->staging[t]) HCMS_CUDA(cudaMalloc(&plan->staging[t], bytes));
-  cudaStream_t caller = static_cast<cudaStream_t>(stream);
   const void* host_in[3] = {q, k, v};
   for (int t = 0; t < 3; ++t)
     HCMS_CUDA(cudaMemcpyAsync(plan->staging[t], host_in[t], bytes, cudaMemcpyHostToDevice, caller));

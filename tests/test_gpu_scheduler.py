@@ -169,3 +169,30 @@ def test_graph_on_a_side_stream_orders_with_the_caller():
                 q.zero_()
         side.synchronize()
         assert np.array_equal(to_host(res), want)
+
+
+# ---------------------------------------------------------------------------------------------
+# hcms_attention_forward_host: the host link as the wire (strided copies = the all-to-all)
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("S,Hh,D,P,C", [(1024, 4, 64, 2, 2), (2100, 12, 128, 4, 2), (777, 5, 128, 1, 3)])
+def test_host_entry_strided_copies_same_bits(S, Hh, D, P, C):
+    """Default host path (cudaMemcpy2DAsync per rank and chunk into / out of the chunk buffers, no layout kernels) ==
+    staged host path == device path, bit for bit; pageable and pinned host memory; poisoned output and workspace."""
+    w = I.Workload("host", S, Hh, D, P, C, 71, "bf16", 1.0)
+    q, k, v = I.make_qkv(w)
+    want = _forward(tuple(to_dev(t) for t in (q, k, v)), S, Hh, D, P, C, w.scale)
+    for flags, launches in ((0, 4 * P * C + C), (H.HCMS_FLAG_HOST_STAGED, 3 * C)):
+        with H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, flags) as plan:
+            n = H.hcms_plan_workspace_bytes(plan)
+            ws = nan_fill_(torch.empty((n + 1) // 2, dtype=torch.int16, device=DEV))
+            H.hcms_plan_set_workspace(plan, ws, n)
+            out = np.full_like(q, 0x7FC0)
+            H.hcms_attention_forward_host(plan, q, k, v, out, w.scale)              # pageable numpy memory
+            assert np.array_equal(out, want), flags
+            assert H.hcms_plan_last_launch_count(plan) == launches
+            pin = [torch.from_numpy(t.view(np.int16)).pin_memory() for t in (q, k, v)]
+            pout = torch.full(q.shape, 0x7FC0, dtype=torch.int16).pin_memory()
+            for _ in range(2):
+                H.hcms_attention_forward_host(plan, pin[0], pin[1], pin[2], pout, w.scale)
+            assert np.array_equal(pout.numpy().view(np.uint16), want), flags
