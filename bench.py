@@ -52,7 +52,7 @@ def parse_args(argv=None):
     ap.add_argument("--config", type=int, default=3, choices=sorted(I.WORKLOADS))
     ap.add_argument("--chunks", type=int, default=0, help="override the workload's C")
     ap.add_argument("--impl", default="hcms", choices=["hcms", "reference"])
-    ap.add_argument("--mode", default="bench", choices=["bench", "c-sweep", "rho-sweep", "timeline"],
+    ap.add_argument("--mode", default="bench", choices=["bench", "c-sweep", "host-c-sweep", "rho-sweep", "timeline"],
                     help="bench: the contract line (default).  c-sweep: every C in 1..H/P, Eq. 10 fit, C* (Table 7/12 "
                          "analogue).  rho-sweep: host-routed all-to-all, speedup vs rho against 1/(1-rho) (Table 13 "
                          "analogue; meant for --config 5).  timeline: per-chunk begin/end of scatter, attention, "
@@ -596,6 +596,56 @@ def run_c_sweep(args):
         "s_max_bound": round(H.hcms_model_s_max(t_comm / rows[0]["serial_ms"]), 4)}), flush=True)
 
 
+def run_host_c_sweep(args):
+    """Table 7 / Table 12 analogue over a REAL wire: hcms_attention_forward_host moves every head chunk between pinned
+    host memory and the chunk buffers over the host link (strided copies = the all-to-all), so rho is tens of percent as
+    on the paper's PCIe clusters.  For every C: the pipelined call, against the serial Ulysses order (all copies in, all
+    attention, all copies out = HCMS_FLAG_HOST_STAGED | HCMS_FLAG_SERIAL); Eq. 10 fit of beta, C* (Theorem 1), Eq. 11."""
+    ss = Session(args)
+    torch, H, w = ss.torch, ss.H, ss.w
+    Hl = w.H // w.P
+    steps = max(3, min(args.steps, 8))
+    host = [t.cpu().pin_memory() for t in (ss.q, ss.k, ss.v)]
+    host_out = torch.empty_like(host[0]).pin_memory()
+
+    def time_host(plan):
+        fn = lambda: H.hcms_attention_forward_host(plan, host[0], host[1], host[2], host_out, w.scale)
+        fn()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(steps):
+            fn()                                   # synchronises the stream itself
+        return (time.perf_counter() - t0) * 1e3 / steps
+
+    with ss.plan(1, H.HCMS_FLAG_HOST_STAGED | H.HCMS_FLAG_SERIAL) as pl:
+        serial_ms = time_host(pl)
+        _, kt = ss.time_plan(pl, 3)
+        t_attn = float(kt[1].sum())
+    t_comm = serial_ms - t_attn - float(kt[0].sum() + kt[2].sum())     # host <-> device copies of the serial call
+    rho = t_comm / serial_ms
+    rows = []
+    for C in range(1, Hl + 1):
+        with H.hcms_plan(w.S, w.H, w.D, w.P, C, H.HCMS_DTYPE_BF16, 0) as pl:
+            ms = time_host(pl)
+            _, h_c = H.hcms_chunk_table(pl)
+        rows.append({"C": C, "chunks": h_c, "hcms_ms": round(ms, 3), "speedup_vs_serial": round(serial_ms / ms, 4),
+                     "tflops": round(ss.flop / ms / 1e9, 1)})
+    Cs = np.array([r["C"] for r in rows], dtype=np.float64)
+    y = np.array([r["hcms_ms"] for r in rows]) - t_comm / Cs
+    beta, a = (np.polyfit(Cs, y, 1) if len(rows) > 1 else (0.0, y[0]))
+    best = min(rows, key=lambda r: r["hcms_ms"])
+    for r in rows:
+        r["eq11_speedup"] = round(H.hcms_model_speedup(r["C"], rho, max(float(beta), 0.0), serial_ms), 4)
+    print(json.dumps({
+        "mode": "host-c-sweep", "config": {"workload": w.name, "S": w.S, "H": w.H, "D": w.D, "P": w.P, "heads_per_rank": Hl},
+        "steps": steps, "serial_ms": round(serial_ms, 3), "t_attn_ms": round(t_attn, 3), "t_comm_ms": round(t_comm, 3),
+        "rho": round(rho, 4), "s_max_bound": round(H.hcms_model_s_max(rho), 4), "rows": rows,
+        "fit": {"model": "Eq. 10: T(C) = a + T_comm/C + beta*C", "a_ms": round(float(a), 3), "beta_ms": round(float(beta), 4),
+                "c_star": (round(H.hcms_model_c_star(t_comm, float(beta)), 2) if beta > 0 else None),
+                "choose_chunks": H.hcms_model_choose_chunks(Hl, t_comm, float(beta))},
+        "measured_best_C": best["C"], "speedup_best_vs_serial": round(serial_ms / best["hcms_ms"], 4)}), flush=True)
+
+
 def run_rho_sweep(args):
     """Table 13 analogue: route 0..4 of the chunk tensors through pinned host memory (the emulated wire of
     BASELINE.json configs[4]) and compare the measured speedup with Theorem 2's 1/(1-rho) and Eq. 11."""
@@ -702,6 +752,8 @@ def main(argv=None):
         run_reference(args)
     elif args.mode == "c-sweep":
         run_c_sweep(args)
+    elif args.mode == "host-c-sweep":
+        run_host_c_sweep(args)
     elif args.mode == "rho-sweep":
         run_rho_sweep(args)
     elif args.mode == "timeline":
