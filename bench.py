@@ -489,6 +489,14 @@ def run_hcms(args):
         same = bool(torch.equal(host_out.to(dev), out))
         result["e2e"]["bitwise_equal_to_device_path"] = same
         plan_e.close()
+        if world == 1:
+            # adaptive C over the host link (future work L346 via Theorem 1): every C in [1, H/P], 2 timed calls each
+            best_C, ms_C = H.hcms_autotune_chunks_host(S, Hh, D, P, base_flags & ~H.HCMS_FLAG_PROFILE, host[0], host[1],
+                                                       host[2], host_out, w.scale, Hh // P, 2)
+            result["e2e"]["autotuned"] = {"best_C": best_C, "ms_per_step": round(ms_C[best_C - 1], 3),
+                                          "value": round(flop_step / (ms_C[best_C - 1] * 1e-3) / 1e12, 2),
+                                          "ms_by_C": [round(m, 3) for m in ms_C],
+                                          "bitwise_equal_to_device_path": bool(torch.equal(host_out.to(dev), out))}
 
     # ---- the whole attention layer, Alg. 1 lines 2-27: projections + RoPE around the hot path ----
     if not args.no_layer:

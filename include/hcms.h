@@ -291,6 +291,15 @@ int hcms_autotune_chunks(int64_t S, int H, int D, int P, int dtype, uint32_t fla
                          const void* v, void* out, float scale, void* stream, int max_C, int reps, int* best_C,
                          float* ms_per_call);
 
+/*
+ * The same measurement through hcms_attention_forward_host: q,k,v,out are HOST pointers (pinned memory for
+ * asynchronous copies), the chunks cross the host link, where the communication ratio is large and the chunk count
+ * matters (measured on B200, cfg 3: C = 4 -> 23.6 ms, C = 6 -> 21.9 ms).  bf16 only; `flags` without SERIAL / PROFILE /
+ * GRAPH.  Arguments, results and errors as hcms_autotune_chunks.
+ */
+int hcms_autotune_chunks_host(int64_t S, int H, int D, int P, uint32_t flags, const void* q, const void* k, const void* v,
+                              void* out, float scale, void* stream, int max_C, int reps, int* best_C, float* ms_per_call);
+
 /* ---- the attention layer around the hot path --------------------------------- */
 /*
  * Section 3.1 (L59): "QKV projection -> RoPE positional encoding -> input all-to-all -> attention

@@ -87,6 +87,8 @@ _SIGNATURES = {
     "hcms_attention_backward_chunk": (c_int, [c_void_p] * 10 + [c_int, c_float, c_void_p]),
     "hcms_plan_lse": (c_void_p, [c_void_p]),
     "hcms_plan_graph_captures": (c_int, [c_void_p]),
+    "hcms_autotune_chunks_host": (c_int, [c_int64, c_int, c_int, c_int, c_uint32] + [c_void_p] * 4 +
+                                  [c_float, c_void_p, c_int, c_int, POINTER(c_int), POINTER(c_float)]),
 }
 
 
@@ -398,3 +400,12 @@ def hcms_plan_lse(plan: Plan) -> int:
 
 def hcms_plan_graph_captures(plan: Plan) -> int:
     return lib.hcms_plan_graph_captures(plan.handle)
+
+
+def hcms_autotune_chunks_host(S, H, D, P, flags, q, k, v, out, scale: float, max_C: int, reps: int = 3, stream=None):
+    """hcms_autotune_chunks over the host-buffer path (q, k, v, out in host memory) -> (best_C, [ms per call])."""
+    best = c_int()
+    ms = (c_float * max(int(max_C), 1))()
+    _check(lib.hcms_autotune_chunks_host(S, H, D, P, flags, _ptr(q), _ptr(k), _ptr(v), _ptr(out), scale, _stream(stream),
+                                         max_C, reps, ctypes.byref(best), ms), "hcms_autotune_chunks_host")
+    return int(best.value), list(ms)

@@ -196,3 +196,19 @@ def test_host_entry_strided_copies_same_bits(S, Hh, D, P, C):
             for _ in range(2):
                 H.hcms_attention_forward_host(plan, pin[0], pin[1], pin[2], pout, w.scale)
             assert np.array_equal(pout.numpy().view(np.uint16), want), flags
+
+
+def test_autotune_chunks_over_the_host_link():
+    """Adaptive C (L346, Theorem 1) where it matters: every C in [1, H/P] timed through the host-buffer path; the
+    result of the last measured call is the plain call's bits, and a single chunk (no overlap at all) is never best
+    when the transfer is a large share of the call."""
+    S, Hh, D, P = 8192, 8, 128, 2
+    w = I.Workload("tune", S, Hh, D, P, 1, 81, "bf16", 1.0)
+    q, k, v = I.make_qkv(w)
+    want = _forward(tuple(to_dev(t) for t in (q, k, v)), S, Hh, D, P, 2, w.scale)
+    pin = [torch.from_numpy(t.view(np.int16)).pin_memory() for t in (q, k, v)]
+    pout = torch.full(q.shape, 0x7FC0, dtype=torch.int16).pin_memory()
+    best, ms = H.hcms_autotune_chunks_host(S, Hh, D, P, 0, pin[0], pin[1], pin[2], pout, w.scale, 6, 3)
+    assert 1 <= best <= 4 and all(m > 0 for m in ms[:4]) and ms[4] == -1 and ms[5] == -1      # H/P = 4 caps the range
+    assert ms[best - 1] == min(ms[:4]) and best > 1
+    assert np.array_equal(pout.numpy().view(np.uint16), want)
