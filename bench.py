@@ -61,6 +61,7 @@ def parse_args(argv=None):
     ap.add_argument("--single-comp", action="store_true", help="HCMS_FLAG_SINGLE_COMP: one compute stream, as Alg. 1")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--host", action="store_true", help="--mode timeline: the host-buffer call (H2D / D2H copies are the wire)")
     ap.add_argument("--no-layer", action="store_true", help="skip the whole-layer (Alg. 1 lines 2-27) measurement")
     ap.add_argument("--no-backward", action="store_true", help="skip the forward+backward (Table 15 analogue) measurement")
     ap.add_argument("--cpu-rows", type=int, default=512, help="query rows per head in the cpu_baseline sample")
@@ -694,22 +695,31 @@ def run_timeline(args):
     C = args.chunks or w.C
     flags = (H.HCMS_FLAG_SINGLE_COMP if args.single_comp else 0)
     with ss.plan(C, flags) as pl:
-        ms, _ = ss.time_plan(pl, 3, warmup=2)
+        if args.host:
+            host = [t.cpu().pin_memory() for t in (ss.q, ss.k, ss.v)]
+            host_out = ss.torch.empty_like(host[0]).pin_memory()
+            t0 = time.perf_counter()
+            for _ in range(4):
+                H.hcms_attention_forward_host(pl, host[0], host[1], host[2], host_out, w.scale)
+            ms = (time.perf_counter() - t0) * 1e3 / 4
+        else:
+            ms, _ = ss.time_plan(pl, 3, warmup=2)
         b, e = H.hcms_plan_timeline(pl, 0)
-    names = ["scatter", "attention", "gather"]
-    ops = [{"op": names[kind], "chunk": c, "stream": ("S_comm" if kind != 1 else ("S_comp" if args.single_comp or c % 2 == 0 else "S_comp'")),
+    names = ["H2D copies", "attention", "D2H copies"] if args.host else ["scatter", "attention", "gather"]
+    ops = [{"op": names[kind], "chunk": c, "stream": (("S_comm" if kind == 0 or not args.host else "S_comm'") if kind != 1 else ("S_comp" if args.single_comp or c % 2 == 0 else "S_comp'")),
             "begin_ms": round(b[kind][c], 4), "end_ms": round(e[kind][c], 4)} for kind in range(3) for c in range(C)]
     ops.sort(key=lambda o: o["begin_ms"])
     span = max(o["end_ms"] for o in ops)
     width = 100
     for o in ops:
         x0, x1 = int(o["begin_ms"] / span * width), max(int(o["end_ms"] / span * width), int(o["begin_ms"] / span * width) + 1)
-        print(f'{o["op"]:>9s}[{o["chunk"]}] {o["stream"]:<7s} |' + " " * x0 + "#" * (x1 - x0) + " " * (width - x1) +
+        print(f'{o["op"]:>10s}[{o["chunk"]}] {o["stream"]:<7s} |' + " " * x0 + "#" * (x1 - x0) + " " * (width - x1) +
               f'| {o["begin_ms"]:8.3f} -> {o["end_ms"]:8.3f} ms', file=sys.stderr)
-    comm_busy = sum(o["end_ms"] - o["begin_ms"] for o in ops if o["op"] != "attention")
+    comm_busy = sum(o["end_ms"] - o["begin_ms"] for o in ops if o["op"] != "attention" and not (args.host and o["op"] == "D2H copies"))
     hidden = sum(max(0.0, min(o["end_ms"], a["end_ms"]) - max(o["begin_ms"], a["begin_ms"]))
-                 for o in ops if o["op"] != "attention" for a in ops if a["op"] == "attention")
-    print(json.dumps({"mode": "timeline", "C": C, "ms_per_call": round(ms, 4), "span_ms": round(span, 4),
+                 for o in ops if o["op"] != "attention" and not (args.host and o["op"] == "D2H copies")
+                 for a in ops if a["op"] == "attention")
+    print(json.dumps({"mode": "timeline", "path": "host buffers" if args.host else "device tensors", "C": C, "ms_per_call": round(ms, 4), "span_ms": round(span, 4),
                       "config": {"workload": w.name, "S": w.S, "H": w.H, "D": w.D, "P": w.P},
                       "comm_ms": round(comm_busy, 4), "comm_ms_overlapped_with_attention": round(min(hidden, comm_busy), 4),
                       "ops": ops}), flush=True)

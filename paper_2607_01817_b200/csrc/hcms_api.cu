@@ -811,15 +811,22 @@ int hcms_attention_forward_host(hcms_plan_t* plan, const void* q, const void* k,
     HCMS_CUDA(cudaEventRecord(plan->e_main, caller));
     for (cudaStream_t s : {plan->s_comm, plan->s_comm_out, plan->s_comp, plan->s_comp2}) HCMS_CUDA(cudaStreamWaitEvent(s, plan->e_main, 0));
     const void* host_in[3] = {q, k, v};
+    const bool profile = plan->flags & HCMS_FLAG_PROFILE;   // same event ring as the device path: 0 = H2D, 1 = attention, 2 = D2H
+    auto mark = [&](int step, int c, int side, cudaStream_t s) -> cudaError_t {
+      const size_t slot = static_cast<size_t>(plan->prof_calls % HCMS_PROFILE_RING) * sh.C + c;
+      return profile ? cudaEventRecord(plan->prof[step][side][slot], s) : cudaSuccess;
+    };
     for (int c = 0; c < sh.C; ++c) {
       const Chunk& ck = plan->chunks[c];
       const size_t width = static_cast<size_t>(ck.h) * D * sh.es, slab = width * S;
+      HCMS_CUDA(mark(0, c, 0, plan->s_comm));
       for (int t = 0; t < 3; ++t)
         for (int p = 0; p < sh.P; ++p) {
           const char* src = static_cast<const char*>(host_in[t]) + (static_cast<size_t>(p) * sh.Hl + ck.o) * D * sh.es;
           HCMS_CUDA(cudaMemcpy2DAsync(ws + ck.off[t] + p * slab, width, src, row, width, S, cudaMemcpyHostToDevice, plan->s_comm));
           plan->last_launches += 1;
         }
+      HCMS_CUDA(mark(0, c, 1, plan->s_comm));
       HCMS_CUDA(cudaEventRecord(plan->e_comm[c], plan->s_comm));
     }
     for (int c = 0; c < sh.C; ++c) {
@@ -827,20 +834,25 @@ int hcms_attention_forward_host(hcms_plan_t* plan, const void* q, const void* k,
       cudaStream_t s_comp = (dual_comp && (c & 1)) ? plan->s_comp2 : plan->s_comp;
       HCMS_CUDA(cudaStreamWaitEvent(s_comp, plan->e_comm[c], 0));
       float* lse_c = plan->lse ? plan->lse + static_cast<size_t>(sh.P) * sh.S * ck.o : nullptr;
+      HCMS_CUDA(mark(1, c, 0, s_comp));
       st = do_attention(plan, ws + ck.off[0], ws + ck.off[1], ws + ck.off[2], ws + ck.off[3], c, scale, s_comp, lse_c);
       if (st) return st;
+      HCMS_CUDA(mark(1, c, 1, s_comp));
       HCMS_CUDA(cudaEventRecord(plan->e_comp[c], s_comp));
     }
     for (int c = 0; c < sh.C; ++c) {
       const Chunk& ck = plan->chunks[c];
       const size_t width = static_cast<size_t>(ck.h) * D * sh.es, slab = width * S;
       HCMS_CUDA(cudaStreamWaitEvent(plan->s_comm_out, plan->e_comp[c], 0));
+      HCMS_CUDA(mark(2, c, 0, plan->s_comm_out));
       for (int p = 0; p < sh.P; ++p) {
         char* dst = static_cast<char*>(out) + (static_cast<size_t>(p) * sh.Hl + ck.o) * D * sh.es;
         HCMS_CUDA(cudaMemcpy2DAsync(dst, row, ws + ck.off[3] + p * slab, width, width, S, cudaMemcpyDeviceToHost, plan->s_comm_out));
         plan->last_launches += 1;
       }
+      HCMS_CUDA(mark(2, c, 1, plan->s_comm_out));
     }
+    if (profile) plan->prof_calls += 1;
     HCMS_CUDA(cudaEventRecord(plan->e_fin_comm, plan->s_comm_out));
     HCMS_CUDA(cudaEventRecord(plan->e_fin_in, plan->s_comm));
     HCMS_CUDA(cudaEventRecord(plan->e_fin_comp, plan->s_comp));
