@@ -5,6 +5,7 @@ import math
 import os
 import re
 
+import numpy as np
 import pytest
 
 import paper_2607_01817_b200 as H
@@ -164,3 +165,26 @@ def test_product_does_not_import_oracle():
                 assert "hcms_inputs" not in text, f
     otext = open(os.path.join(ROOT, "oracle", "hcms_oracle.py")).read()
     assert "import paper_2607_01817_b200" not in otext and "ctypes" not in otext
+
+
+def test_layer_and_tuner_argument_validation_precedes_device_use():
+    """Shape / NULL errors of the SURVEY 8(f) entry points are reported without touching a GPU."""
+    buf = np.zeros(128 * 128, dtype=np.uint16)
+    for args, code in [((buf, buf, None, 128, 128, 64), H.HCMS_ERR_INVALID_ARG),
+                       ((buf, buf, buf, 128, 100, 64), H.HCMS_ERR_UNSUPPORTED_SHAPE),      # N % 128
+                       ((buf, buf, buf, 128, 128, 60), H.HCMS_ERR_UNSUPPORTED_SHAPE),      # K % 8
+                       ((buf, buf, buf, -1, 128, 64), H.HCMS_ERR_INVALID_ARG)]:
+        with pytest.raises(H.HcmsError) as ei:
+            H.hcms_gemm_bf16_nt(*args, stream=0)
+        assert ei.value.status == code, args[3:]
+    with pytest.raises(H.HcmsError) as ei:
+        H.hcms_autotune_chunks_host(1024, 4, 64, 2, 0, buf, buf, buf, None, 0.1, 2, 1, stream=0)
+    assert ei.value.status == H.HCMS_ERR_INVALID_ARG
+    with pytest.raises(H.HcmsError) as ei:
+        H.hcms_autotune_chunks_host(1024, 5, 64, 2, 0, buf, buf, buf, buf, 0.1, 2, 1, stream=0)
+    assert ei.value.status == H.HCMS_ERR_UNSUPPORTED_SHAPE                                  # H % P
+    with pytest.raises(H.HcmsError) as ei:
+        H.hcms_autotune_chunks_host(1024, 4, 64, 2, 0, buf, buf, buf, buf, 0.1, 0, 1, stream=0)
+    assert ei.value.status == H.HCMS_ERR_INVALID_ARG                                        # max_C < 1
+    assert H.hcms_plan_graph_captures(H.Plan(0, 1, 1, 1, 1, 1, 0, 0)) == 0                 # NULL plan queries
+    assert H.hcms_plan_lse(H.Plan(0, 1, 1, 1, 1, 1, 0, 0)) == 0 and H.hcms_plan_layer_buffer(H.Plan(0, 1, 1, 1, 1, 1, 0, 0), 0) == 0
