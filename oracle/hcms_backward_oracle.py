@@ -71,10 +71,12 @@ def attention_backward(q, k, v, do, scale: float):
     return tuple(outs)
 
 
-def attention_backward_sampled(q, k, v, do, scale: float, q_rows, k_rows):
+def attention_backward_sampled(q, k, v, do, scale: float, q_rows, k_rows, row_block: int = 2048):
     """Large shapes: ``dq[q_rows]`` needs those query rows only; ``dk[k_rows]``, ``dv[k_rows]`` need column
     ``k`` of P for every query, i.e. every row's normaliser.  Returns fp64 ``(dq [Rq,H,D], dk [Rk,H,D], dv [Rk,H,D])``.
-    Row statistics are computed in row blocks; nothing inside a row is reordered."""
+    Row statistics are computed in blocks of ``row_block`` query rows (it only bounds the ``[rows, S]`` score
+    matrix); nothing inside a row is reordered, and the sums over queries ``dV_k = sum_i p_ik dO_i``,
+    ``dK_k = scale sum_i dS_ik q_i`` are accumulated block after block in row order."""
     q_rows, k_rows = np.asarray(q_rows, np.int64), np.asarray(k_rows, np.int64)
     S, H, D = q.shape
     dq = np.empty((len(q_rows), H, D))
@@ -88,8 +90,8 @@ def attention_backward_sampled(q, k, v, do, scale: float, q_rows, k_rows):
         ds = p * (dp - (p * dp).sum(axis=1, keepdims=True))
         dq[:, h, :] = float(scale) * (ds @ kh)
         # dk, dv for the sampled key rows: walk over all query rows in blocks
-        for r0 in range(0, S, 2048):
-            sl = slice(r0, min(r0 + 2048, S))
+        for r0 in range(0, S, row_block):
+            sl = slice(r0, min(r0 + row_block, S))
             p, _ = _probs(qh[sl], kh, scale)                            # [rows, S]
             delta = (doh[sl] * (p @ vh)).sum(axis=1, keepdims=True)     # dO_i . o_i
             pk = p[:, k_rows]                                           # [rows, Rk]

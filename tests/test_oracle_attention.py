@@ -159,3 +159,43 @@ def test_sampled_rows_equal_full():
     assert rows[0] == 0 and rows[-1] == S - 1 and 128 in rows and 127 in rows and 256 in rows and 255 in rows
     assert np.allclose(O.attention_sampled(q, k, v, 0.3, rows), O.attention_full(q, k, v, 0.3)[rows],
                        rtol=1e-13, atol=1e-14)
+
+
+# ---------------------------------------------------------------------------------------------
+# the row-block loop of attention_full (the reference for cfg 2 = 4 blocks and for the ragged shapes):
+# second and later blocks, a ragged last block, a block larger than S
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("S,row_block", [(40, 7), (40, 16), (300, 7), (300, 16), (129, 128), (64, 64), (50, 4096)])
+def test_attention_full_row_blocks_equal_single_block(S, row_block):
+    """Rows are independent (Eq. 2), so the block size may not change any row: every row of the multi-block
+    result equals the single-block result (to BLAS rounding of the [rows,S] product, <= 1e-14), the definition
+    evaluated one row at a time, and fp64 SDPA."""
+    H, D = 2, 8
+    q, k, v = rnd(40 + S + row_block, S, H, D)
+    scale = 0.3
+    multi = O.attention_full(q, k, v, scale, row_block=row_block)
+    single = O.attention_full(q, k, v, scale, row_block=S)
+    assert multi.shape == single.shape and np.isfinite(multi).all()
+    assert np.abs(multi - single).max() <= 1e-14
+    # one row at a time: no block structure at all
+    for h in range(H):
+        for i in list(range(0, S, max(1, S // 23))) + [S - 1]:
+            one = O.attention_rows(q[i:i + 1, h], k[:, h], v[:, h], scale)[0]
+            assert np.abs(multi[i, h] - one).max() <= 1e-14, (i, h)
+    tq, tk, tv = (torch.from_numpy(t).permute(1, 0, 2)[None] for t in (q, k, v))
+    ref = torch.nn.functional.scaled_dot_product_attention(tq, tk, tv, scale=scale)[0].permute(1, 0, 2).numpy()
+    assert np.abs(multi - ref).max() <= 1e-12
+
+
+def test_attention_full_row_blocks_write_every_row_once():
+    """A slip in the block slices (an off-by-one, a skipped tail) leaves rows of the np.empty output unwritten or
+    written from the wrong query: with V = one-hot(key index) and Q_i = 50*K_i the output row i is e_i exactly."""
+    S, D = 45, 45
+    k = np.eye(S)[:, None, :]                       # K_i = e_i  (H = 1)
+    q = 50.0 * k                                    # score(i, i) = 50*scale, others 0
+    v = np.eye(S)[:, None, :]
+    for rb in (1, 7, 16, 44, 45, 46):
+        out = O.attention_full(q, k, v, 1.0, row_block=rb)
+        assert np.abs(out[:, 0, :] - np.eye(S)).max() < 1e-12, rb
+        assert np.array_equal(out.argmax(axis=2)[:, 0], np.arange(S)), rb

@@ -132,3 +132,44 @@ def test_composed_backward_equals_direct_bitwise(P, C):
     composed = B.hcms_backward_composed(q, k, v, do, P, C, 0.5)
     for a, b in zip(direct, composed):
         assert np.array_equal(a, b)
+
+
+# ---------------------------------------------------------------------------------------------
+# the row-block accumulation of attention_backward_sampled (dK, dV summed over query blocks with +=): the
+# reference for the cfg 3 backward (16 blocks).  Second and later blocks, ragged last block, block > S.
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("S,row_block", [(40, 7), (40, 16), (300, 7), (300, 16), (129, 128), (50, 4096)])
+def test_sampled_backward_row_blocks(S, row_block):
+    q, k, v, do = _problem(S=S, H=2, D=8, seed=20 + S + row_block)
+    scale = 0.35
+    full = B.attention_backward(q, k, v, do, scale)
+    r = np.random.default_rng(S)
+    qr = np.unique(np.concatenate([[0, S - 1, min(row_block, S) - 1, min(row_block, S - 1)], r.integers(0, S, 6)]))
+    kr = np.unique(np.concatenate([[0, S - 1, min(row_block, S) - 1, min(row_block, S - 1)], r.integers(0, S, 6)]))
+    multi = B.attention_backward_sampled(q, k, v, do, scale, qr, kr, row_block=row_block)
+    single = B.attention_backward_sampled(q, k, v, do, scale, qr, kr, row_block=S)
+    for a, b in zip(multi, single):                    # accumulation order differs only by block boundaries
+        assert np.abs(a - b).max() <= 1e-13
+    assert np.abs(multi[0] - full[0][qr]).max() <= 1e-13
+    assert np.abs(multi[1] - full[1][kr]).max() <= 1e-13
+    assert np.abs(multi[2] - full[2][kr]).max() <= 1e-13
+    # and against an implementation that shares nothing with the oracle: torch.autograd through fp64 SDPA
+    tq, tk, tv = (torch.from_numpy(x).clone().requires_grad_(True) for x in (q, k, v))
+    o = torch.nn.functional.scaled_dot_product_attention(tq.transpose(0, 1)[None], tk.transpose(0, 1)[None],
+                                                         tv.transpose(0, 1)[None], scale=scale)[0].transpose(0, 1)
+    o.backward(torch.from_numpy(do))
+    assert np.abs(multi[0] - tq.grad.numpy()[qr]).max() <= 1e-12
+    assert np.abs(multi[1] - tk.grad.numpy()[kr]).max() <= 1e-12
+    assert np.abs(multi[2] - tv.grad.numpy()[kr]).max() <= 1e-12
+
+
+def test_sampled_backward_blocks_accumulate_not_overwrite():
+    """`=` for `+=` in the block loop would keep only the last block's contribution.  With scale = 0, P is uniform
+    1/S, so dV_k = mean_i dO_i needs every block; dK = 0."""
+    S = 37
+    q, k, v, do = _problem(S=S, H=1, D=4, seed=31)
+    kr = np.array([0, 5, 36])
+    _, dk, dv = B.attention_backward_sampled(q, k, v, do, 0.0, np.array([0]), kr, row_block=5)
+    assert np.abs(dv - do.mean(axis=0, keepdims=True)).max() < 1e-14
+    assert np.abs(dk).max() == 0.0
