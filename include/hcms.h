@@ -40,7 +40,7 @@
 extern "C" {
 #endif
 
-#define HCMS_VERSION 300 /* major*10000 + minor*100 + patch */
+#define HCMS_VERSION 400 /* major*10000 + minor*100 + patch */
 
 /* ---- status codes ------------------------------------------------------------------- */
 enum {
@@ -119,6 +119,15 @@ enum {
                                           heads straight between the host tensors and the chunk buffers (they ARE the
                                           all-to-all), chunk c+1's transfer overlapping chunk c's attention. */
 
+#define HCMS_FLAG_GEMM_1CTA 0x10000u    /* projections (hcms_qkv_projection_rope, hcms_output_projection, hcms_layer_forward):
+                                          use the single-CTA tcgen05 GEMM (128 x 256 tiles) also where the default
+                                          CTA-pair kernel (cta_group::2, 256 x 256 tiles) applies.  Same bits. */
+
+#define HCMS_FLAG_DEBUG_ATTN_ONLY 0x20000u /* MEASUREMENT ONLY: hcms_attention_forward skips the scatter and gather
+                                          kernels (events, streams and attention launches unchanged), so that the
+                                          compute side of the pipeline can be timed in the same stream arrangement
+                                          without copies; the chunk buffers must hold an earlier call's data */
+
 typedef struct hcms_plan hcms_plan_t;
 
 /* ---- introspection (host only, no GPU needed) ---------------------------------------- */
@@ -158,11 +167,19 @@ int hcms_model_choose_chunks(int heads_per_rank, double t_comm, double beta);
 /* ---- plan ------------------------------------------------------------------------------ */
 /*
  * Create a plan for global tensors [S,H,D], P logical ranks, C head chunks (Alg. 1's
- * `num_chunks`).  Validates the shape, builds the chunk table, creates the communication and
- * compute streams (device-level stream caching, L221) and 2+2C timing-disabled events, and
- * allocates the chunk workspace (4*S*H*D*es bytes + alignment) on the current device unless
- * hcms_plan_set_workspace is used.  `*plan` is owned by the library; free it with
- * hcms_plan_destroy.  May synchronise the host (allocation).
+ * `num_chunks`) on the CURRENT device.  Validates the shape, builds the chunk table, creates the
+ * communication and compute streams (device-level stream caching, L221) and 5+2C timing-disabled
+ * events, and sets the kernel attributes once per device.  The chunk workspace (4*S*H*D*es bytes +
+ * alignment; twice that plus H*S floats under HCMS_FLAG_TRAINING) is allocated on the first call
+ * that needs it, unless hcms_plan_set_workspace supplied caller memory before.  Every TMA
+ * descriptor a call needs is encoded once and cached in the plan, keyed by address and shape
+ * (hcms_plan_tensor_map_encodes counts the encodes).  `*plan` is owned by the library; free it
+ * with hcms_plan_destroy.
+ *
+ * Concurrency: a plan owns ONE set of streams, events and chunk buffers, so it serves one host
+ * thread and one caller stream at a time; calls on the same plan from two caller streams must be
+ * ordered by the caller (or use two plans).  Every call on a plan must be made with the plan's
+ * device current (PLAN_MISMATCH otherwise).
  * Errors: INVALID_ARG, UNSUPPORTED_SHAPE, UNSUPPORTED_DTYPE, UNSUPPORTED_DEVICE, CUDA.
  */
 int hcms_plan(hcms_plan_t** plan, int64_t S, int H, int D, int P, int C, int dtype, uint32_t flags);
@@ -172,7 +189,9 @@ int hcms_plan_destroy(hcms_plan_t* plan); /* synchronises the plan's streams; NU
 size_t hcms_plan_workspace_bytes(const hcms_plan_t* plan);
 /*
  * Use caller memory (device pointer, 256-byte aligned, >= hcms_plan_workspace_bytes) as the
- * workspace; the plan's own allocation, if any, is released.  The caller keeps ownership.
+ * workspace; the plan's own allocation, if any, is released (after synchronising the plan's
+ * streams).  The caller keeps ownership.  A captured graph (HCMS_FLAG_GRAPH) and the forward
+ * state saved for hcms_attention_backward are discarded: the next forward captures again.
  * Errors: INVALID_ARG, MISALIGNED, WORKSPACE_TOO_SMALL.
  */
 int hcms_plan_set_workspace(hcms_plan_t* plan, void* dev, size_t bytes);
@@ -186,8 +205,12 @@ int hcms_chunk_table(const hcms_plan_t* plan, int* o, int* h);
  */
 int hcms_chunk_layout(const hcms_plan_t* plan, int c, size_t* bytes, size_t* q_off, size_t* k_off,
                       size_t* v_off, size_t* o_off);
-/* Device address of the workspace (NULL if none); for tests (NaN poisoning, inspection). */
-void* hcms_plan_workspace(const hcms_plan_t* plan);
+/* Device address of the workspace (allocates the plan-owned one if none exists yet; NULL on failure); for tests
+ * (NaN poisoning, inspection). */
+void* hcms_plan_workspace(hcms_plan_t* plan);
+/* Number of cuTensorMapEncodeTiled calls this plan has made so far: constant across repeated calls on the same
+ * tensors (the descriptors live in the plan). */
+long long hcms_plan_tensor_map_encodes(const hcms_plan_t* plan);
 
 /* ---- the hot path ----------------------------------------------------------------------- */
 /*
@@ -369,7 +392,8 @@ int hcms_plan_layer_timings(hcms_plan_t* plan, float* qkv_ms, float* hcms_ms, fl
  * be the forward being differentiated (its Q'_c, K'_c, V'_c, O'_c and lse are read from the workspace; `scale`
  * must be the same).  dout: device [S,H,D] bf16 = dL/d(out); dq, dk, dv: device [S,H,D] bf16, distinct, not
  * overlapping dout.  Asynchronous on `stream` like the forward.  HCMS_FLAG_SERIAL runs it on `stream` alone.
- * Errors: INVALID_ARG (NULL, plan without TRAINING, no forward yet), PLAN_MISMATCH, MISALIGNED, ALIAS, CUDA.
+ * Errors: INVALID_ARG (NULL, plan without TRAINING, no forward yet or workspace replaced since, `scale` not
+ * bit-equal to the forward's -- the saved lse belongs to that scale), PLAN_MISMATCH, MISALIGNED, ALIAS, CUDA.
  */
 int hcms_attention_backward(hcms_plan_t* plan, const void* dout, void* dq, void* dk, void* dv, int64_t S, int H,
                             int D, int P, int C, float scale, void* stream);

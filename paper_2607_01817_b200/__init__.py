@@ -46,6 +46,8 @@ HCMS_FLAG_FUSE_A2A = 0x1000
 HCMS_FLAG_GRAPH = 0x2000
 HCMS_FLAG_ATTN_PAIR = 0x4000
 HCMS_FLAG_HOST_STAGED = 0x8000
+HCMS_FLAG_GEMM_1CTA = 0x10000
+HCMS_FLAG_DEBUG_ATTN_ONLY = 0x20000
 
 # every symbol include/hcms.h declares: name -> (restype, argtypes)
 _SIGNATURES = {
@@ -65,6 +67,7 @@ _SIGNATURES = {
     "hcms_chunk_table": (c_int, [c_void_p, POINTER(c_int), POINTER(c_int)]),
     "hcms_chunk_layout": (c_int, [c_void_p, c_int] + [POINTER(c_size_t)] * 5),
     "hcms_plan_workspace": (c_void_p, [c_void_p]),
+    "hcms_plan_tensor_map_encodes": (ctypes.c_longlong, [c_void_p]),
     "hcms_attention_forward": (c_int, [c_void_p] * 5 + [c_int64, c_int, c_int, c_int, c_int, c_float, c_void_p]),
     "hcms_attention_forward_host": (c_int, [c_void_p] * 5 + [c_int64, c_int, c_int, c_int, c_int, c_float, c_void_p]),
     "hcms_a2a_scatter": (c_int, [c_void_p, c_int, POINTER(c_void_p), POINTER(c_void_p), c_int, c_void_p]),
@@ -263,6 +266,10 @@ def hcms_chunk_layout(plan: Plan, c: int):
     vals = [c_size_t() for _ in range(5)]
     _check(lib.hcms_chunk_layout(plan.handle, c, *[ctypes.byref(v) for v in vals]), "hcms_chunk_layout")
     return dict(zip(("bytes", "q_off", "k_off", "v_off", "o_off"), (v.value for v in vals)))
+
+
+def hcms_plan_tensor_map_encodes(plan: Plan) -> int:
+    return lib.hcms_plan_tensor_map_encodes(plan.handle)
 
 
 def hcms_plan_last_launch_count(plan: Plan) -> int:

@@ -455,7 +455,7 @@ cudaError_t map4d(CUtensorMap* m, const void* base, const AttnBwdArgs& a, uint32
   const uint64_t strides[3] = {static_cast<uint64_t>(a.D) * 2, static_cast<uint64_t>(a.h_c) * a.D * 2,
                                static_cast<uint64_t>(a.S) * a.h_c * a.D * 2};
   const uint32_t box[4] = {64, 1, box_rows, 1};
-  return encode_tensor_map(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, base, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B);
+  return encode_tensor_map(a.cache, m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, base, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B);
 }
 
 template <int D>
@@ -505,7 +505,7 @@ cudaError_t launch(const AttnBwdArgs& a, cudaStream_t stream) {
 
 }  // namespace
 
-cudaError_t attention_bwd_init() {
+static cudaError_t bwd_set_attributes() {
   cudaError_t e;
 #define HCMS_SET(fn, bytes) \
   if ((e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes)) != cudaSuccess) return e;
@@ -515,6 +515,11 @@ cudaError_t attention_bwd_init() {
   HCMS_SET((attention_bwd_kernel<64, true>), Cfg<64>::kSmemBytes)
 #undef HCMS_SET
   return cudaSuccess;
+}
+
+cudaError_t attention_bwd_init() {
+  static PerDeviceOnce once;
+  return once_per_device(&once, bwd_set_attributes);
 }
 
 size_t attention_bwd_stats_bytes(int64_t S, int heads) {

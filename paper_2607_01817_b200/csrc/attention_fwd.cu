@@ -34,8 +34,6 @@
 // (the paper's "max error 0" claim, L304 / Table 14).
 #include <cuda_bf16.h>
 
-#include <cstdlib>
-
 #include "hcms_internal.h"
 #include "ptx.cuh"
 
@@ -577,70 +575,43 @@ cudaError_t make_maps(const AttnArgs& a, AttnMaps* m) {
   const void* ptrs[4] = {a.q, a.k, a.v, a.o};
   CUtensorMap* outs[4] = {&m->q, &m->k, &m->v, &m->o};
   for (int i = 0; i < 4; ++i) {
-    cudaError_t e = encode_tensor_map(outs[i], CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, ptrs[i], dims, strides, box,
+    cudaError_t e = encode_tensor_map(a.cache, outs[i], CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, ptrs[i], dims, strides, box,
                                       CU_TENSOR_MAP_SWIZZLE_128B);
     if (e != cudaSuccess) return e;
   }
+  if (!a.pair) {        // only the CTA-pair kernel reads the half-tile map
+    m->kh = m->k;
+    return cudaSuccess;
+  }
   const uint32_t box_half[4] = {64, 1, 64, 1};
-  return encode_tensor_map(&m->kh, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, a.k, dims, strides, box_half, CU_TENSOR_MAP_SWIZZLE_128B);
+  return encode_tensor_map(a.cache, &m->kh, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, a.k, dims, strides, box_half,
+                           CU_TENSOR_MAP_SWIZZLE_128B);
 }
 
-using KernelFn = void (*)(const AttnMaps, const AttnParams);
+// Of every 8 column pairs, kPolyPairs take their exponential on the FMA pipe (tuned on B200: profiles/ poly sweep)
+constexpr int kPolyPairs = 2;
 
-// Number of column pairs (of every 8) whose exponential runs on the FMA pipe.  The default was tuned on
-// B200 (profiles/); HCMS_ATTN_POLY=0..8 overrides it for tuning runs (read once).
-int poly_setting() {
-  static int v = -1;
-  if (v < 0) {
-    const char* e = std::getenv("HCMS_ATTN_POLY");
-    v = e ? std::atoi(e) : 2;
-    if (v < 0 || v > 8) v = 2;
-  }
-  return v;
-}
-
-template <int D, bool kPair = false>
-KernelFn pick_kernel(int poly) {
-  switch (poly) {
-    case 0: return attention_fwd_kernel<D, 0, kPair>;
-    case 1: return attention_fwd_kernel<D, 1, kPair>;
-    case 3: return attention_fwd_kernel<D, 3, kPair>;
-    case 4: return attention_fwd_kernel<D, 4, kPair>;
-    case 5: return attention_fwd_kernel<D, 5, kPair>;
-    case 6: return attention_fwd_kernel<D, 6, kPair>;
-    case 8: return attention_fwd_kernel<D, 8, kPair>;
-    default: return attention_fwd_kernel<D, 2, kPair>;
-  }
-}
-
-// HCMS_ATTN_PAIR=1 selects the CTA-pair kernel for every D = 128 launch of the process (tuning runs; read once);
-// HCMS_FLAG_ATTN_PAIR selects it per plan.
-bool pair_setting() {
-  static int v = -1;
-  if (v < 0) {
-    const char* e = std::getenv("HCMS_ATTN_PAIR");
-    v = e ? (std::atoi(e) != 0) : 0;
-  }
-  return v != 0;
+cudaError_t set_attributes() {
+  cudaError_t e = cudaFuncSetAttribute(attention_fwd_kernel<128, kPolyPairs, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       Cfg<128>::kSmemBytes);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(attention_fwd_kernel<64, kPolyPairs, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                           Cfg<64>::kSmemBytes);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(attention_fwd_kernel<128, kPolyPairs, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              Cfg<128, true>::kSmemBytes);
 }
 
 }  // namespace
 
 cudaError_t attention_init() {
-  for (int poly : {0, 1, 2, 3, 4, 5, 6, 8}) {
-    cudaError_t e = cudaFuncSetAttribute(pick_kernel<128>(poly), cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         Cfg<128>::kSmemBytes);
-    if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(pick_kernel<64>(poly), cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg<64>::kSmemBytes);
-    if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(pick_kernel<128, true>(poly), cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             Cfg<128, true>::kSmemBytes);
-    if (e != cudaSuccess) return e;
-  }
-  return cudaSuccess;
+  static PerDeviceOnce once;
+  return once_per_device(&once, set_attributes);
 }
 
-cudaError_t launch_attention(const AttnArgs& a, cudaStream_t stream) {
+cudaError_t launch_attention(const AttnArgs& a0, cudaStream_t stream) {
+  AttnArgs a = a0;
+  a.pair = a0.pair && a0.D == 128;
   AttnMaps maps;
   cudaError_t e = make_maps(a, &maps);
   if (e != cudaSuccess) return e;
@@ -653,8 +624,7 @@ cudaError_t launch_attention(const AttnArgs& a, cudaStream_t stream) {
   prm.scale_log2 = fmaxf(a.scale * 1.4426950408889634f, 1e-30f);
   prm.lse = a.lse;
   dim3 grid(static_cast<unsigned>((a.S + kQTiles * kBM - 1) / (kQTiles * kBM)), static_cast<unsigned>(a.P * a.h_c));
-  const int poly = poly_setting();
-  if (a.D == 128 && (a.pair || pair_setting())) {
+  if (a.pair) {
     // CTA pairs: a cluster of 2 consecutive CTAs (512 query rows) per launch unit; an odd block count is padded by
     // one CTA whose query rows do not exist (its loads are zero fill, its stores are skipped)
     cudaLaunchConfig_t cfg{};
@@ -669,12 +639,12 @@ cudaError_t launch_attention(const AttnArgs& a, cudaStream_t stream) {
     attr.val.clusterDim.z = 1;
     cfg.attrs = &attr;
     cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, pick_kernel<128, true>(poly), maps, prm);
+    return cudaLaunchKernelEx(&cfg, attention_fwd_kernel<128, kPolyPairs, true>, maps, prm);
   }
   if (a.D == 128)
-    pick_kernel<128>(poly)<<<grid, kThreads, Cfg<128>::kSmemBytes, stream>>>(maps, prm);
+    attention_fwd_kernel<128, kPolyPairs, false><<<grid, kThreads, Cfg<128>::kSmemBytes, stream>>>(maps, prm);
   else if (a.D == 64)
-    pick_kernel<64>(poly)<<<grid, kThreads, Cfg<64>::kSmemBytes, stream>>>(maps, prm);
+    attention_fwd_kernel<64, kPolyPairs, false><<<grid, kThreads, Cfg<64>::kSmemBytes, stream>>>(maps, prm);
   else
     return cudaErrorInvalidValue;
   return cudaGetLastError();

@@ -10,7 +10,7 @@
 // rotated by the angle whose cos/sin the caller tabulates per (token, i)  (reading R-23).
 //
 // Two kernels: the CTA-pair kernel below (cta_group::2, 256 x 256 tiles; default when the output width allows) and this
-// single-CTA kernel (128 x 256 or 128 x 128 tiles), which also serves as the fallback (HCMS_GEMM_2CTA=0).
+// single-CTA kernel (128 x 256 or 128 x 128 tiles), which also serves as the fallback (HCMS_FLAG_GEMM_1CTA).
 // Persistent kernel, one CTA per SM, 256 threads:
 //   warp 0     TMA producer: A tile [128 x 64] and B tile [BN x 64] per k-block into a shared-memory ring
 //   warp 1     MMA issuer (one elected lane): tcgen05.mma.cta_group::1.kind::f16, M=128, N=BN, K=16, SS
@@ -20,9 +20,6 @@
 // Tiles are visited in bands of 16 m-tiles x all n-tiles so that the ~148 tiles in flight share A and B
 // panels through L2.
 #include <cuda_bf16.h>
-
-#include <cstdlib>
-#include <mutex>
 
 #include "hcms_internal.h"
 #include "ptx.cuh"
@@ -511,51 +508,33 @@ gemm_bf16_nt_2cta_kernel(const __grid_constant__ GemmMaps maps, const __grid_con
 // ------------------------------------------------------------------------------------------
 namespace {
 
-cudaError_t map2d(CUtensorMap* m, const void* base, uint64_t inner, uint64_t outer, uint32_t box_inner,
+cudaError_t map2d(TmapCache* cache, CUtensorMap* m, const void* base, uint64_t inner, uint64_t outer, uint32_t box_inner,
                   uint32_t box_outer) {
   const uint64_t dims[2] = {inner, outer};
   const uint64_t strides[1] = {inner * 2};
   const uint32_t box[2] = {box_inner, box_outer};
-  return encode_tensor_map(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, base, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B);
+  return encode_tensor_map(cache, m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, base, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_128B);
 }
 
-// m-tiles per band: the ~148 tiles in flight cover group_m x (148 / group_m) tiles, and the whole B matrix is streamed
-// from HBM once per band.  HCMS_GEMM_GROUP_M overrides the default for tuning runs (read once).
-int group_m_setting() {
-  static int v = 0;
-  if (v == 0) {
-    const char* e = std::getenv("HCMS_GEMM_GROUP_M");
-    v = e ? std::atoi(e) : 16;
-    if (v < 1 || v > 4096) v = 16;
-  }
-  return v;
-}
-
-// HCMS_GEMM_2CTA=0/1 selects the single-CTA or the CTA-pair kernel for shapes with n_per_out % 256 == 0 (read once).
-bool pair_setting() {
-  static int v = -1;
-  if (v < 0) {
-    const char* e = std::getenv("HCMS_GEMM_2CTA");
-    v = e ? (std::atoi(e) != 0) : 1;   // measured on B200: 1527 vs 1416 TFLOP/s on the cfg 3 QKV projection
-  }
-  return v != 0;
-}
+// m-tiles per band: the ~148 tiles in flight cover kGroupM x (148 / kGroupM) tiles, and the whole B matrix is streamed
+// from HBM once per band.  Swept on B200: 8 / 16 / 32 / 64 -> 1374 / 1415 / 1382 / 1322 TFLOP/s.
+constexpr int kGroupM = 16;
 
 template <int BN, int kMode, bool k2Cta>
 cudaError_t launch(const GemmArgs& a, cudaStream_t stream) {
   GemmMaps maps;
   ChunkMaps cmaps;
-  cudaError_t e = map2d(&maps.b, a.b, static_cast<uint64_t>(a.K), static_cast<uint64_t>(a.N), kBK, k2Cta ? BN / 2 : BN);
+  cudaError_t e = map2d(a.cache, &maps.b, a.b, static_cast<uint64_t>(a.K), static_cast<uint64_t>(a.N), kBK, k2Cta ? BN / 2 : BN);
   if (e != cudaSuccess) return e;
   GemmParams p{};
   const int n_out = a.N / a.n_per_out;
   if (kMode == kPlain) {
-    e = map2d(&maps.a, a.a, static_cast<uint64_t>(a.K), static_cast<uint64_t>(a.M), kBK, kBM);
+    e = map2d(a.cache, &maps.a, a.a, static_cast<uint64_t>(a.K), static_cast<uint64_t>(a.M), kBK, kBM);
     if (e != cudaSuccess) return e;
     for (int t = 0; t < 3; ++t) {
       // unused slots repeat slot 0 so that the struct holds valid descriptors only
       void* base = a.out[t < n_out ? t : 0];
-      e = map2d(&maps.out[t], base, static_cast<uint64_t>(a.n_per_out), static_cast<uint64_t>(a.M), 64, kBM);
+      e = map2d(a.cache, &maps.out[t], base, static_cast<uint64_t>(a.n_per_out), static_cast<uint64_t>(a.M), 64, kBM);
       if (e != cudaSuccess) return e;
     }
     for (auto& m : cmaps.m) m = maps.b;
@@ -563,10 +542,10 @@ cudaError_t launch(const GemmArgs& a, cudaStream_t stream) {
     const GemmChunks& ck = *a.chunks;
     if (ck.C > kMaxChunks || ck.Hl > kMaxLocalHeads) return cudaErrorInvalidValue;
     if (kMode == kFusedOut) {
-      e = map2d(&maps.a, a.a, static_cast<uint64_t>(a.K), static_cast<uint64_t>(a.M), kBK, kBM);
+      e = map2d(a.cache, &maps.a, a.a, static_cast<uint64_t>(a.K), static_cast<uint64_t>(a.M), kBK, kBM);
     } else {
       maps.a = maps.b;
-      e = map2d(&maps.out[0], a.out[0], static_cast<uint64_t>(a.n_per_out), static_cast<uint64_t>(a.M), 64, kBM);
+      e = map2d(a.cache, &maps.out[0], a.out[0], static_cast<uint64_t>(a.n_per_out), static_cast<uint64_t>(a.M), 64, kBM);
     }
     if (e != cudaSuccess) return e;
     for (int t = 0; t < 3; ++t)
@@ -580,7 +559,7 @@ cudaError_t launch(const GemmArgs& a, cudaStream_t stream) {
         const uint64_t strides[3] = {static_cast<uint64_t>(a.D) * 2, static_cast<uint64_t>(ck.h[c]) * a.D * 2,
                                      static_cast<uint64_t>(a.M) * ck.h[c] * a.D * 2};
         const uint32_t box[4] = {64, 1, kBM, 1};
-        e = encode_tensor_map(&cmaps.m[t * ck.C + c], CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, ck.base[t][c], dims, strides, box,
+        e = encode_tensor_map(a.cache, &cmaps.m[t * ck.C + c], CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, ck.base[t][c], dims, strides, box,
                               CU_TENSOR_MAP_SWIZZLE_128B);
         if (e != cudaSuccess) return e;
       }
@@ -605,13 +584,13 @@ cudaError_t launch(const GemmArgs& a, cudaStream_t stream) {
   p.n_tiles = a.N / BN;
   if (k2Cta) {
     p.m_tiles = static_cast<int>((a.M + 2 * kBM - 1) / (2 * kBM));     // 256-row tiles of a CTA pair
-    p.group_m = (group_m_setting() + 1) / 2;
+    p.group_m = (kGroupM + 1) / 2;
     const int total = p.m_tiles * p.n_tiles, pairs = a.num_sms / 2;
     const int grid = 2 * (total < pairs ? total : pairs);
     gemm_bf16_nt_2cta_kernel<kMode><<<grid, kThreads, Cfg2::kSmemBytes, stream>>>(maps, cmaps, p);
   } else {
     p.m_tiles = static_cast<int>((a.M + kBM - 1) / kBM);
-    p.group_m = group_m_setting();
+    p.group_m = kGroupM;
     const int total = p.m_tiles * p.n_tiles;
     const int grid = total < a.num_sms ? total : a.num_sms;
     gemm_bf16_nt_kernel<BN, kMode><<<grid, kThreads, Cfg<BN>::kSmemBytes, stream>>>(maps, cmaps, p);
@@ -621,24 +600,26 @@ cudaError_t launch(const GemmArgs& a, cudaStream_t stream) {
 
 }  // namespace
 
-cudaError_t gemm_init() {
-  static std::once_flag once;
-  static cudaError_t status = cudaSuccess;
-  std::call_once(once, [] {
-    auto set = [](auto fn, int bytes) {
-      if (status == cudaSuccess) status = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-    };
-    set(gemm_bf16_nt_kernel<256, kPlain>, Cfg<256>::kSmemBytes);
-    set(gemm_bf16_nt_kernel<128, kPlain>, Cfg<128>::kSmemBytes);
-    set(gemm_bf16_nt_kernel<256, kFusedOut>, Cfg<256>::kSmemBytes);
-    set(gemm_bf16_nt_kernel<128, kFusedOut>, Cfg<128>::kSmemBytes);
-    set(gemm_bf16_nt_kernel<256, kFusedA>, Cfg<256>::kSmemBytes);
-    set(gemm_bf16_nt_kernel<128, kFusedA>, Cfg<128>::kSmemBytes);
-    set(gemm_bf16_nt_2cta_kernel<kPlain>, Cfg2::kSmemBytes);
-    set(gemm_bf16_nt_2cta_kernel<kFusedOut>, Cfg2::kSmemBytes);
-    set(gemm_bf16_nt_2cta_kernel<kFusedA>, Cfg2::kSmemBytes);
-  });
+static cudaError_t gemm_set_attributes() {
+  cudaError_t status = cudaSuccess;
+  auto set = [&](auto fn, int bytes) {
+    if (status == cudaSuccess) status = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  };
+  set(gemm_bf16_nt_kernel<256, kPlain>, Cfg<256>::kSmemBytes);
+  set(gemm_bf16_nt_kernel<128, kPlain>, Cfg<128>::kSmemBytes);
+  set(gemm_bf16_nt_kernel<256, kFusedOut>, Cfg<256>::kSmemBytes);
+  set(gemm_bf16_nt_kernel<128, kFusedOut>, Cfg<128>::kSmemBytes);
+  set(gemm_bf16_nt_kernel<256, kFusedA>, Cfg<256>::kSmemBytes);
+  set(gemm_bf16_nt_kernel<128, kFusedA>, Cfg<128>::kSmemBytes);
+  set(gemm_bf16_nt_2cta_kernel<kPlain>, Cfg2::kSmemBytes);
+  set(gemm_bf16_nt_2cta_kernel<kFusedOut>, Cfg2::kSmemBytes);
+  set(gemm_bf16_nt_2cta_kernel<kFusedA>, Cfg2::kSmemBytes);
   return status;
+}
+
+cudaError_t gemm_init() {
+  static PerDeviceOnce once;
+  return once_per_device(&once, gemm_set_attributes);
 }
 
 // Shape rules (checked by the callers in hcms_api.cu): K % 8 == 0 (16-byte row pitch), n_per_out % 128 == 0,
@@ -647,7 +628,7 @@ cudaError_t launch_gemm(const GemmArgs& a, cudaStream_t stream) {
   cudaError_t e = gemm_init();
   if (e != cudaSuccess) return e;
   const bool wide = a.n_per_out % 256 == 0;
-  if (wide && pair_setting()) {   // CTA pairs (cta_group::2), 256 x 256 tiles
+  if (wide && !a.one_cta) {   // CTA pairs (cta_group::2), 256 x 256 tiles: 1527 vs 1416 TFLOP/s on the cfg 3 QKV projection
     if (a.fuse == 1) return launch<256, kFusedOut, true>(a, stream);
     if (a.fuse == 2) return launch<256, kFusedA, true>(a, stream);
     return launch<256, kPlain, true>(a, stream);

@@ -7,6 +7,9 @@
 #include <cstddef>
 #include <cstdint>
 #include <cstdio>
+#include <cstring>
+#include <string>
+#include <unordered_map>
 #include <vector>
 
 #include "hcms.h"
@@ -38,6 +41,32 @@ struct Shape {
   int Hl;            // heads per logical rank
 };
 
+// ---- tensor maps (tma_desc.cu) ----------------------------------------------------------------
+// "Device-level caching" for TMA descriptors: a plan owns one TmapCache, every launch helper looks its
+// descriptors up by (base, dims, strides, box, type, swizzle) and encodes only on a miss, so a steady-state call
+// encodes nothing.  Workspace-side maps are hit from the second call on; caller tensors are hit as long as the caller
+// passes the same addresses.  Not thread-safe: a plan serves one host thread / caller stream at a time (hcms.h).
+struct TmapCache {
+  std::unordered_map<std::string, CUtensorMap> maps;
+  long long encodes = 0;   // misses = calls of cuTensorMapEncodeTiled
+  long long hits = 0;
+};
+// dims/strides innermost first; strides[0] is implied (element size).  `cache` may be NULL (always encodes).
+cudaError_t encode_tensor_map(TmapCache* cache, CUtensorMap* out, CUtensorMapDataType dt, int rank, const void* base,
+                              const uint64_t* dims, const uint64_t* strides_bytes, const uint32_t* box,
+                              CUtensorMapSwizzle swizzle);
+
+// ---- per-device one-time setup ------------------------------------------------------------------
+// Kernel attributes (MaxDynamicSharedMemorySize) are per device: `fn` runs once for every device that becomes
+// current when the helper is called (mutex-guarded; 64 devices at most).
+struct PerDeviceOnce {
+  bool done[64] = {};
+  cudaError_t status[64] = {};
+};
+cudaError_t once_per_device(PerDeviceOnce* state, cudaError_t (*fn)());
+// SM count of the current device (cached per device); HCMS status, fails on a non-sm_100 device
+int device_sms(int* sms);
+
 // ---- layout kernels (layout_kernels.cu) -------------------------------------------------
 struct LayoutArgs {
   const void* src[3];
@@ -47,6 +76,11 @@ struct LayoutArgs {
   int H, D, P, Hl, es;
   int o_c, h_c;
   bool gather;       // false: [S,H,D] -> [P][S][h_c][D];  true: the inverse
+  TmapCache* cache = nullptr;
+  // Distributed form (hcms_dist.cu): the strided tensor is this rank's shard [S_local][H][D] (S = S_local) and the
+  // dense block of logical rank p is NOT src/dst + p*S*h_c*D but the explicit address peer[t][p] (a region of rank
+  // p's chunk buffer, local or mapped peer memory).  NULL = the single-device emulation.
+  void* const* peer[3] = {nullptr, nullptr, nullptr};
 };
 cudaError_t launch_layout_vec(const LayoutArgs& a, cudaStream_t stream);
 cudaError_t launch_layout_tma(const LayoutArgs& a, cudaStream_t stream, int num_sms);
@@ -62,9 +96,10 @@ struct AttnArgs {
   float scale;
   float* lse = nullptr;   // optional [P*h_c][S] fp32: log sum_k exp(scale q.k) per row (saved for the backward)
   bool pair = false;      // CTA-pair kernel (HCMS_FLAG_ATTN_PAIR; D = 128 only, ignored otherwise)
+  TmapCache* cache = nullptr;
 };
 cudaError_t launch_attention(const AttnArgs& a, cudaStream_t stream);
-cudaError_t attention_init();  // sets kernel attributes once; resolves cuTensorMapEncodeTiled
+cudaError_t attention_init();  // sets kernel attributes once per device
 
 // ---- attention backward (attention_bwd.cu) -------------------------------------------------
 struct AttnBwdArgs {
@@ -81,6 +116,7 @@ struct AttnBwdArgs {
   int64_t S;
   int D, P, h_c;
   float scale;
+  TmapCache* cache = nullptr;
 };
 cudaError_t launch_attention_bwd(const AttnBwdArgs& a, cudaStream_t stream);   // 3 launches
 cudaError_t attention_bwd_init();
@@ -108,14 +144,10 @@ struct GemmArgs {
   int fuse = 0;                       // 0: plain; 1: outputs stored into the chunk buffers (`out` unused);
                                       // 2: A loaded from the O'_c chunk buffers (`a` unused)
   const GemmChunks* chunks = nullptr;
+  bool one_cta = false;               // HCMS_FLAG_GEMM_1CTA: the single-CTA kernel also where the CTA-pair kernel applies
+  TmapCache* cache = nullptr;
 };
 cudaError_t launch_gemm(const GemmArgs& a, cudaStream_t stream);
 cudaError_t gemm_init();
-
-// ---- driver entry point for tensor maps (tma_desc.cu) ------------------------------------
-// dims/strides innermost first; strides[0] is implied (element size). Returns cudaSuccess or an error.
-cudaError_t encode_tensor_map(CUtensorMap* out, CUtensorMapDataType dt, int rank, const void* base,
-                              const uint64_t* dims, const uint64_t* strides_bytes, const uint32_t* box,
-                              CUtensorMapSwizzle swizzle);
 
 }  // namespace hcms

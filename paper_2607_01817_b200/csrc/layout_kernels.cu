@@ -250,7 +250,7 @@ cudaError_t launch_layout_tma(const LayoutArgs& a, cudaStream_t stream, int num_
     const uint64_t dims[3] = {static_cast<uint64_t>(a.D), static_cast<uint64_t>(a.H), static_cast<uint64_t>(a.S)};
     const uint64_t strides[2] = {static_cast<uint64_t>(a.D) * a.es, static_cast<uint64_t>(a.H) * a.D * a.es};
     const uint32_t box[3] = {static_cast<uint32_t>(a.D), static_cast<uint32_t>(a.h_c), static_cast<uint32_t>(rows)};
-    cudaError_t e = encode_tensor_map(&maps.strided[t], dt, 3, strided, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_NONE);
+    cudaError_t e = encode_tensor_map(a.cache, &maps.strided[t], dt, 3, strided, dims, strides, box, CU_TENSOR_MAP_SWIZZLE_NONE);
     if (e != cudaSuccess) return e;
     p.dense_src[t] = static_cast<const uint8_t*>(a.src[t]);
     p.dense_dst[t] = static_cast<uint8_t*>(a.dst[t]);
@@ -266,12 +266,13 @@ cudaError_t launch_layout_tma(const LayoutArgs& a, cudaStream_t stream, int num_
   p.tiles_per_rank = static_cast<uint32_t>((a.S + rows - 1) / rows);
   p.n_tiles = static_cast<uint32_t>(a.n_tensors) * a.P * p.tiles_per_rank;
   const size_t smem = static_cast<size_t>(kTmaStages) * rows * row_bytes + 128;
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaFuncSetAttribute(layout_tma_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
-    cudaFuncSetAttribute(layout_tma_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
-    attr_set = true;
-  }
+  static PerDeviceOnce once;
+  cudaError_t ea = once_per_device(&once, [] {
+    cudaError_t e = cudaFuncSetAttribute(layout_tma_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(layout_tma_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+  });
+  if (ea != cudaSuccess) return ea;
   uint32_t grid = static_cast<uint32_t>(num_sms) * 3;
   if (grid > p.n_tiles) grid = p.n_tiles;
   if (a.gather)

@@ -84,10 +84,9 @@ def test_ragged_shapes_full(S, Hh, D, P, C):
     got = run_forward(q, k, v, S, Hh, D, P, C, w.scale)
     ref = O.attention_full(q, k, v, w.scale)
     check(got, ref, f"S={S}")
-    # the last (partial) KV tile and the last Q tile specifically
+    # the last (partial) Q tile specifically, with its own gates (it must not hide inside the whole-tensor norm)
     tail = S - (S % 128 or 128)
-    err_tail = np.abs(bf16_bits_to_f64(got[tail:]) - ref[tail:])
-    assert err_tail.max() <= MAX_ABS
+    check(got[tail:], ref[tail:], f"S={S} tail rows [{tail},{S})")
 
 
 # ---------------------------------------------------------------------------------------------
@@ -213,6 +212,57 @@ def test_full_size_configs_sampled_rows(cfg):
     assert (gf <= vf.max(axis=0, keepdims=True)).all() and (gf >= vf.min(axis=0, keepdims=True)).all()
     # sanity against an all-zero / wrong-magnitude output: sampled norm within 2 % of the oracle's
     assert abs(np.linalg.norm(bf16_bits_to_f64(got[rows])) / np.linalg.norm(ref) - 1) < 2e-2
+
+
+# ---------------------------------------------------------------------------------------------
+# O(1)-output closed forms at the FULL cfg 3-5 shapes (SURVEY 8(c) "GPU vs oracle": |O| ~ 0.007 on the N(0,1)
+# inputs makes the absolute gates nearly vacuous there), in the launch configuration bench.py times
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("cfg", [3, 4, 5])
+def test_full_size_uniform_v_per_head_constant(cfg):
+    """V[s,h,:] = c_h  =>  O[i,h,:] = c_h for ANY q, k (Eq. 2: softmax weights sum to 1).  c_h = 1 + h/4 is exact in
+    bf16 and differs per head, so a head routed to the wrong rank / chunk / slot by either all-to-all shows up.
+    Error budget: P is rounded to bf16 while l sums the unrounded fp32 p (relative 2^-9 per term, averaging out) and
+    the output is rounded once to bf16 (2^-9): |err| <= 2^-7 c_h."""
+    w = I.workload(cfg)
+    q, k, _ = I.make_qkv(w, threads=16)
+    c_h = I.f32_to_bf16_bits(np.float32([1.0 + 0.25 * h for h in range(w.H)]))
+    v = np.broadcast_to(c_h[None, :, None], (w.S, w.H, w.D)).copy()
+    got = I.bf16_bits_to_f32(run_forward(q, k, v, w.S, w.H, w.D, w.P, w.C, w.scale))
+    ref = I.bf16_bits_to_f32(c_h)[None, :, None]
+    assert not np.isnan(got).any()
+    rel = np.abs(got - ref) / ref
+    assert rel.max() <= 2.0 ** -7, rel.max()
+    assert np.array_equal(np.round(got[::997, :, 0] * 4), np.broadcast_to(np.round(ref[:, :, 0] * 4), got[::997, :, 0].shape))
+
+
+@pytest.mark.parametrize("cfg", [3, 4, 5])
+def test_full_size_one_hot_scores_select_v_row_bitwise(cfg):
+    """Q[i] = alpha K[pi(i)], alpha = 256 (exact in bf16): the target's score beats every other key's by >= 40 nats,
+    so O[i] = V[pi(i)] (closed form, checked in fp64 by the oracle on the sampled rows) and on the GPU every output
+    row is BIT-equal to that bf16 V row.  pi sends the first and last rows of every 128-row tile edge case and 64
+    random rows into the last KV tile (cfg 3: keys 32640..32759, a 120-key ragged tile; cfg 4: 56064..56159, 96 keys;
+    cfg 5: the full last tile), the rest is a random permutation: 256-438-768 KV tiles with the running max moving at
+    arbitrary tiles, i.e. the lazy-rescale path on every row."""
+    w = I.workload(cfg)
+    _, k, v = I.make_qkv(w, threads=16)
+    S = w.S
+    rng = np.random.default_rng(cfg)
+    pi = rng.permutation(S)
+    tail0 = S - (S % 128 or 128)
+    forced = np.unique(np.concatenate([[0, 1, 127, 128, 255, 256, S - 1, tail0 - 1, tail0], rng.integers(0, S, 64)]))
+    pi[forced] = tail0 + rng.integers(0, S - tail0, len(forced))
+    pi[S - 1] = S - 1                                           # last query -> last key
+    pi[0] = tail0                                               # first query -> first key of the last tile
+    alpha = np.float32(256.0)
+    q = I.f32_to_bf16_bits(alpha * I.bf16_bits_to_f32(k)[pi])   # exact: a power of two times a bf16 value
+    rows = np.unique(np.concatenate([forced, O.sample_rows(S, w.P, n_random=8, seed=cfg)]))
+    ref = O.attention_sampled(q, k, v, w.scale, rows)
+    assert np.abs(ref - bf16_bits_to_f64(v[pi[rows]])).max() < 1e-9          # the oracle's closed form (margin holds)
+    got = run_forward(q, k, v, w.S, w.H, w.D, w.P, w.C, w.scale)
+    same = (got == v[pi]).all(axis=2)                            # [S, H]
+    assert same.all(), f"{(~same).sum()} (row, head) pairs differ; first {np.argwhere(~same)[:5].tolist()}"
 
 
 # ---------------------------------------------------------------------------------------------

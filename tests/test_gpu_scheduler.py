@@ -152,6 +152,34 @@ def test_graph_replay_same_bits(extra):
         assert H.hcms_plan_graph_captures(plan) == 3 and not np.array_equal(to_host(out2), want)
 
 
+def test_graph_recaptures_after_a_workspace_swap():
+    """a captured graph holds the workspace addresses; hcms_plan_set_workspace must void it.  Capture on
+    the plan-owned workspace (freed by the swap), swap in a NaN-poisoned one, call again on the same tensors: same
+    bits, second capture, and the new workspace is the one that was written."""
+    S, Hh, D, P, C = 2048, 6, 64, 2, 3
+    qkv, scale = _inputs(S, Hh, D, seed=23)
+    want = _forward(qkv, S, Hh, D, P, C, scale)
+    q, k, v = qkv
+    out = nan_fill_(torch.empty_like(q))
+    with H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, H.HCMS_FLAG_GRAPH) as plan:
+        H.hcms_attention_forward(plan, q, k, v, out, scale)               # capture #1 on the plan-owned workspace
+        torch.cuda.synchronize()
+        assert np.array_equal(to_host(out), want) and H.hcms_plan_graph_captures(plan) == 1
+        n = H.hcms_plan_workspace_bytes(plan)
+        for _ in range(2):                                                # two swaps: caller-owned -> caller-owned too
+            ws = nan_fill_(torch.empty((n + 1) // 2, dtype=torch.int16, device=DEV))
+            H.hcms_plan_set_workspace(plan, ws, n)
+            captures = H.hcms_plan_graph_captures(plan)
+            nan_fill_(out)
+            H.hcms_attention_forward(plan, q, k, v, out, scale)
+            torch.cuda.synchronize()
+            assert np.array_equal(to_host(out), want)
+            assert H.hcms_plan_graph_captures(plan) == captures + 1
+            o_off = H.hcms_chunk_layout(plan, 0)["o_off"]
+            head = to_host(ws[o_off // 2:o_off // 2 + 4096])              # chunk 0's O'_c lives in the NEW workspace
+            assert not (head == 0x7FC0).all()
+
+
 def test_graph_on_a_side_stream_orders_with_the_caller():
     """The replay is ordered after work already on the caller's stream and before what follows it."""
     S, Hh, D, P, C = 1024, 4, 64, 2, 2
@@ -212,3 +240,81 @@ def test_autotune_chunks_over_the_host_link():
     assert 1 <= best <= 4 and all(m > 0 for m in ms[:4]) and ms[4] == -1 and ms[5] == -1      # H/P = 4 caps the range
     assert ms[best - 1] == min(ms[:4]) and best > 1
     assert np.array_equal(pout.numpy().view(np.uint16), want)
+
+
+# ---------------------------------------------------------------------------------------------
+# plan-level caching ("device-level caching"): descriptors, workspace
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("flags", [0, H.HCMS_FLAG_LAYOUT_TMA, H.HCMS_FLAG_ATTN_PAIR])
+def test_tensor_maps_are_encoded_once_per_plan(flags):
+    """Every TMA descriptor lives in the plan: the first call encodes them, later calls on the same tensors
+    encode nothing; another output tensor encodes only the maps that name it."""
+    S, Hh, D, P, C = 2048, 8, 128, 2, 2
+    qkv, scale = _inputs(S, Hh, D, seed=31)
+    q, k, v = qkv
+    out, out2 = torch.empty_like(q), torch.empty_like(q)
+    with H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, flags) as plan:
+        assert H.hcms_plan_tensor_map_encodes(plan) == 0
+        H.hcms_attention_forward(plan, q, k, v, out, scale)
+        first = H.hcms_plan_tensor_map_encodes(plan)
+        assert first >= 4 * C                                   # q, k, v, o maps of every chunk's attention launch
+        for _ in range(3):
+            H.hcms_attention_forward(plan, q, k, v, out, scale)
+        assert H.hcms_plan_tensor_map_encodes(plan) == first
+        H.hcms_attention_forward(plan, q, k, v, out2, scale)
+        extra = H.hcms_plan_tensor_map_encodes(plan) - first
+        _, h_c = H.hcms_chunk_table(plan)
+        assert extra == (len(set(h_c)) if flags & H.HCMS_FLAG_LAYOUT_TMA else 0)   # only the TMA gather's map(s) of `out`
+        torch.cuda.synchronize()
+        assert torch.equal(out, out2)
+
+
+def test_workspace_is_allocated_on_first_use_only():
+    """A caller-supplied workspace never coexists with a plan-owned one: creating the plan allocates
+    no chunk buffers; the first forward does, unless hcms_plan_set_workspace came first."""
+    S, Hh, D, P, C = 8192, 16, 128, 2, 2
+    qkv, scale = _inputs(S, Hh, D, seed=32)
+    q, k, v = qkv
+    out = torch.empty_like(q)
+    torch.cuda.synchronize()
+    free0, _ = torch.cuda.mem_get_info()
+    with H.hcms_plan(S, Hh, D, P, C) as plan:
+        n = H.hcms_plan_workspace_bytes(plan)
+        assert n >= 4 * S * Hh * D * 2
+        free1, _ = torch.cuda.mem_get_info()
+        assert free0 - free1 < n // 2                                     # no workspace yet
+        ws = torch.empty((n + 1) // 2, dtype=torch.int16, device=DEV)     # torch's allocation, counted before the call
+        free2, _ = torch.cuda.mem_get_info()
+        H.hcms_plan_set_workspace(plan, ws, n)
+        H.hcms_attention_forward(plan, q, k, v, out, scale)
+        torch.cuda.synchronize()
+        free3, _ = torch.cuda.mem_get_info()
+        assert free2 - free3 < n // 2                                     # the plan never allocated its own
+    with H.hcms_plan(S, Hh, D, P, C) as plan:
+        free4, _ = torch.cuda.mem_get_info()
+        H.hcms_attention_forward(plan, q, k, v, out, scale)
+        torch.cuda.synchronize()
+        free5, _ = torch.cuda.mem_get_info()
+        assert free4 - free5 >= n // 2                                    # allocated by the first call
+
+
+def test_backward_rejects_another_scale_and_a_replaced_workspace():
+    S, Hh, D, P, C = 512, 4, 64, 2, 2
+    qkv, scale = _inputs(S, Hh, D, seed=33)
+    q, k, v = qkv
+    out = torch.empty_like(q)
+    g = [torch.empty_like(q) for _ in range(4)]
+    with H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, H.HCMS_FLAG_TRAINING) as plan:
+        H.hcms_attention_forward(plan, q, k, v, out, scale)
+        with pytest.raises(H.HcmsError) as ei:
+            H.hcms_attention_backward(plan, g[0], g[1], g[2], g[3], scale * 0.5)
+        assert ei.value.status == H.HCMS_ERR_INVALID_ARG
+        H.hcms_attention_backward(plan, g[0], g[1], g[2], g[3], scale)
+        n = H.hcms_plan_workspace_bytes(plan)
+        ws = torch.empty((n + 1) // 2, dtype=torch.int16, device=DEV)
+        H.hcms_plan_set_workspace(plan, ws, n)
+        with pytest.raises(H.HcmsError) as ei:                              # the saved Q'_c .. O'_c are gone
+            H.hcms_attention_backward(plan, g[0], g[1], g[2], g[3], scale)
+        assert ei.value.status == H.HCMS_ERR_INVALID_ARG
+        torch.cuda.synchronize()
