@@ -59,6 +59,10 @@ def parse_args(argv=None):
                          "gather on their streams (Fig. 2 analogue)")
     ap.add_argument("--layout", default="vec", choices=["vec", "tma"])
     ap.add_argument("--single-comp", action="store_true", help="HCMS_FLAG_SINGLE_COMP: one compute stream, as Alg. 1")
+    ap.add_argument("--attn-pair", action="store_true", help="HCMS_FLAG_ATTN_PAIR: attention forward on CTA pairs (D = 128)")
+    ap.add_argument("--attn-split", action="store_true", help="HCMS_FLAG_ATTN_SPLIT: pair kernel, two softmax threads per row")
+    ap.add_argument("--quick", action="store_true", help="only the contract measurement of the hot path (no layer, backward, e2e, "
+                                                         "graph, value-independence, cpu baseline blocks)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--host", action="store_true", help="--mode timeline: the host-buffer call (H2D / D2H copies are the wire)")
@@ -388,7 +392,8 @@ def run_hcms(args):
     flush = 3 * tensor_bytes < 2 * L2_BYTES
     flush_buf = torch.empty(2 * L2_BYTES, dtype=torch.uint8, device=dev) if flush else None
     base_flags = (H.HCMS_FLAG_PROFILE | (H.HCMS_FLAG_LAYOUT_TMA if args.layout == "tma" else 0) |
-                  (H.HCMS_FLAG_SINGLE_COMP if args.single_comp else 0))
+                  (H.HCMS_FLAG_SINGLE_COMP if args.single_comp else 0) | (H.HCMS_FLAG_ATTN_PAIR if args.attn_pair else 0) |
+                  (H.HCMS_FLAG_ATTN_SPLIT if args.attn_split else 0))
     stream = torch.cuda.current_stream()
 
     def timed(plan, steps, fn):
@@ -456,7 +461,7 @@ def run_hcms(args):
         "config": {"workload": f"BASELINE.json configs[{args.config - 1}] ({w.name}): S={S} H={Hh} D={D} "
                                f"P={P} C={C} chunks={h_c} non-causal scale=1/sqrt(D)",
                    "S": S, "H": Hh, "D": D, "P": P, "C": C, "layout_kernel": args.layout,
-                   "compute_streams": 1 if args.single_comp else 2,
+                   "compute_streams": 1 if args.single_comp else 2, "attention_kernel": "cta pair" if args.attn_pair else "single cta",
                    "l2": "flushed between steps" if flush else "inputs larger than L2 (3 x %d MB)" % (tensor_bytes >> 20),
                    "multi_gpu": "replicas only" if world > 1 else "single GPU",
                    "inputs": "hcms_inputs counter-based N(0,1) -> bf16 (seed %d)" % w.seed},
@@ -471,6 +476,13 @@ def run_hcms(args):
                      "attn_ms_per_step": round(attn_ms, 4), "flop_per_step": sum(attn_flop)},
     }
     plan.close()
+    if args.quick:
+        if rank == 0:
+            print(json.dumps(result), flush=True)
+        if world > 1:
+            import torch.distributed as dist
+            dist.destroy_process_group()
+        return
 
     # ---- serial (Ulysses, Eq. 1) pass: solo kernel times and the pipeline ratio ---------------
     n_ser = min(args.steps, 10)

@@ -123,6 +123,10 @@ enum {
                                           use the single-CTA tcgen05 GEMM (128 x 256 tiles) also where the default
                                           CTA-pair kernel (cta_group::2, 256 x 256 tiles) applies.  Same bits. */
 
+#define HCMS_FLAG_ATTN_SPLIT 0x40000u   /* D = 128 only: the CTA-pair attention kernel with TWO softmax threads per query row
+                                          (16 softmax warps per CTA, each thread 64 of the tile's 128 keys; half-row maxima
+                                          and sums are exchanged through shared memory).  Implies HCMS_FLAG_ATTN_PAIR. */
+
 #define HCMS_FLAG_DEBUG_ATTN_ONLY 0x20000u /* MEASUREMENT ONLY: hcms_attention_forward skips the scatter and gather
                                           kernels (events, streams and attention launches unchanged), so that the
                                           compute side of the pipeline can be timed in the same stream arrangement
@@ -411,6 +415,61 @@ int hcms_attention_backward_chunk(hcms_plan_t* plan, const void* qc, const void*
 /* Device address of the lse the last forward saved on a TRAINING plan: [H][S] fp32 in the order chunk 0's
  * P*h_0 heads (p-major), chunk 1's, ...; NULL otherwise.  For tests. */
 void* hcms_plan_lse(const hcms_plan_t* plan);
+
+/* ---- HCMS between P real ranks ---------------------------------------------------- */
+/*
+ * The paper's actual setting (L45, L59; Alg. 1 lines 8, 21; Table 1 "2 rounds"): P GPUs (one process each, or one
+ * process driving several), rank r holding the sequence shard [S/P, H, D] of q, k, v and producing its shard of out.
+ * Rank p owns global heads [p*H/P, (p+1)*H/P); head chunks are Eq. 3 on H/P as everywhere else.
+ *
+ * No library collective is on the data path.  Every rank owns an "exchange block" (its chunk buffers Q'_c, K'_c, V'_c,
+ * O'_c, each [S][h_c][D], plus epoch flags) that the other ranks map through CUDA IPC (hcms_dist_export /
+ * hcms_dist_attach; between GPUs of a node this is NVLink / NVSwitch peer memory) or, inside one process, through
+ * peer access (hcms_dist_attach_local).  Per chunk c the input all-to-all is rank r's scatter kernel STORING its
+ * [S/P][h_c][D] slices into every rank's Q'_c, K'_c, V'_c (rows [r*S/P, (r+1)*S/P)), the output all-to-all is rank
+ * r's gather kernel LOADING its rows of every rank's O'_c into out[:, p*H/P + o_c + j, :].  E_c^comm and E_c^comp
+ * (Eq. 6-7) are 32-bit epoch flags in the consumer's block: written by a one-warp kernel with system-scope
+ * release stores after the producing kernel, awaited by the consumer's STREAM (cuStreamWaitValue32) -- no kernel spins
+ * on another rank and the host is never blocked.  S_comm runs the pushes of all chunks and then the pulls, S_comp the
+ * attention per chunk, exactly Alg. 1's three phases.  The attention kernel is the one of the single-device path, so
+ * the concatenated outputs of the P ranks are BIT-EQUAL to hcms_attention_forward on the concatenated inputs.
+ *
+ * hcms_dist_plan: collective in spirit (every rank creates its own with the same S, H, D, P, C); allocates the
+ * exchange block (4*S*(H/P)*D*2 bytes + flags) on the current device.  flags: 0, HCMS_FLAG_ATTN_PAIR or
+ * HCMS_FLAG_ATTN_SPLIT.  bf16 only.
+ * hcms_dist_export: writes HCMS_DIST_HANDLE_BYTES opaque bytes that another PROCESS passes to hcms_dist_attach.
+ * hcms_dist_attach: `handles` = P consecutive handles in rank order (this rank's own entry is checked, not opened);
+ * the caller moves the bytes between processes with any host channel (torch.distributed, files).
+ * hcms_dist_attach_local: the P plans live in this process (peers[r] = rank r's plan, peers[rank] = plan itself).
+ * hcms_dist_attention_forward: q, k, v, out = this rank's device shards [S/P, H, D] bf16, 16-byte aligned, out not
+ * overlapping the inputs; asynchronous on `stream` like hcms_attention_forward.  EVERY rank must make the call the
+ * same number of times (a rank that does not leaves the others' streams waiting).
+ * hcms_dist_attention_forward_group: the call for ranks that live in ONE process (attached with
+ * hcms_dist_attach_local): plans[r], q[r], k[r], v[r], out[r], streams[r] for r < n = P, in rank order, DISTINCT caller
+ * streams.  It enqueues phase by phase over all ranks (all pushes, then all attention, then all pulls), so that every
+ * flag a stream waits on is produced by work already enqueued: a stream blocked on a flag holds its hardware work
+ * queue, and a rank-by-rank enqueue could park rank 1's pushes behind rank 0's wait on a shared queue (measured: it
+ * deadlocks).  hcms_dist_attention_forward therefore rejects locally attached plans (INVALID_ARG); one process per
+ * rank -- the deployment the paper describes -- has no such constraint.  Switches to each plan's device for its part.
+ * All ranks must have finished (a host barrier after synchronising the streams) before any plan is destroyed.
+ * Errors: INVALID_ARG, UNSUPPORTED_SHAPE (also P > 16), UNSUPPORTED_DTYPE, UNSUPPORTED_DEVICE, PLAN_MISMATCH (handle of
+ * another shape / rank order, wrong device), MISALIGNED, ALIAS, CUDA.
+ */
+typedef struct hcms_dist_plan hcms_dist_plan_t;
+#define HCMS_DIST_HANDLE_BYTES 128
+int hcms_dist_plan(hcms_dist_plan_t** plan, int64_t S, int H, int D, int P, int C, int dtype, uint32_t flags, int rank);
+int hcms_dist_plan_destroy(hcms_dist_plan_t* plan); /* synchronises the plan's streams, unmaps the peers; NULL is a no-op */
+int hcms_dist_export(hcms_dist_plan_t* plan, void* handle);
+int hcms_dist_attach(hcms_dist_plan_t* plan, const void* handles, int n);
+int hcms_dist_attach_local(hcms_dist_plan_t* plan, hcms_dist_plan_t* const* peers, int n);
+int hcms_dist_attention_forward(hcms_dist_plan_t* plan, const void* q, const void* k, const void* v, void* out,
+                                float scale, void* stream);
+int hcms_dist_attention_forward_group(hcms_dist_plan_t* const* plans, int n, const void* const* q, const void* const* k,
+                                      const void* const* v, void* const* out, float scale, void* const* streams);
+/* Bytes of the rank's exchange block; kernels + signal launches of the last forward (C pushes + C attention + C pulls
+ * + 2C signals).  0 for a NULL plan. */
+size_t hcms_dist_block_bytes(const hcms_dist_plan_t* plan);
+int hcms_dist_last_launch_count(const hcms_dist_plan_t* plan);
 
 #ifdef __cplusplus
 }

@@ -48,6 +48,7 @@ HCMS_FLAG_ATTN_PAIR = 0x4000
 HCMS_FLAG_HOST_STAGED = 0x8000
 HCMS_FLAG_GEMM_1CTA = 0x10000
 HCMS_FLAG_DEBUG_ATTN_ONLY = 0x20000
+HCMS_FLAG_ATTN_SPLIT = 0x40000
 
 # every symbol include/hcms.h declares: name -> (restype, argtypes)
 _SIGNATURES = {
@@ -90,6 +91,15 @@ _SIGNATURES = {
     "hcms_attention_backward_chunk": (c_int, [c_void_p] * 10 + [c_int, c_float, c_void_p]),
     "hcms_plan_lse": (c_void_p, [c_void_p]),
     "hcms_plan_graph_captures": (c_int, [c_void_p]),
+    "hcms_dist_plan": (c_int, [POINTER(c_void_p), c_int64, c_int, c_int, c_int, c_int, c_int, c_uint32, c_int]),
+    "hcms_dist_plan_destroy": (c_int, [c_void_p]),
+    "hcms_dist_export": (c_int, [c_void_p, c_void_p]),
+    "hcms_dist_attach": (c_int, [c_void_p, c_void_p, c_int]),
+    "hcms_dist_attach_local": (c_int, [c_void_p, POINTER(c_void_p), c_int]),
+    "hcms_dist_attention_forward": (c_int, [c_void_p] * 5 + [c_float, c_void_p]),
+    "hcms_dist_attention_forward_group": (c_int, [POINTER(c_void_p), c_int] + [POINTER(c_void_p)] * 4 + [c_float, POINTER(c_void_p)]),
+    "hcms_dist_block_bytes": (c_size_t, [c_void_p]),
+    "hcms_dist_last_launch_count": (c_int, [c_void_p]),
     "hcms_autotune_chunks_host": (c_int, [c_int64, c_int, c_int, c_int, c_uint32] + [c_void_p] * 4 +
                                   [c_float, c_void_p, c_int, c_int, POINTER(c_int), POINTER(c_float)]),
 }
@@ -416,3 +426,107 @@ def hcms_autotune_chunks_host(S, H, D, P, flags, q, k, v, out, scale: float, max
     _check(lib.hcms_autotune_chunks_host(S, H, D, P, flags, _ptr(q), _ptr(k), _ptr(v), _ptr(out), scale, _stream(stream),
                                          max_C, reps, ctypes.byref(best), ms), "hcms_autotune_chunks_host")
     return int(best.value), list(ms)
+
+
+# ---- HCMS between P real ranks --------------------------------------------------------
+
+HCMS_DIST_HANDLE_BYTES = 128
+
+
+class DistPlan:
+    """Owns one rank's hcms_dist_plan_t*; use as a context manager or call close()."""
+
+    def __init__(self, handle: int, S: int, H: int, D: int, P: int, C: int, rank: int):
+        self.handle = c_void_p(handle)
+        self.S, self.H, self.D, self.P, self.C, self.rank = S, H, D, P, C, rank
+
+    def close(self) -> None:
+        if self.handle:
+            lib.hcms_dist_plan_destroy(self.handle)
+            self.handle = c_void_p(0)
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def hcms_dist_plan(S: int, H: int, D: int, P: int, C: int, rank: int, dtype: int = HCMS_DTYPE_BF16, flags: int = 0) -> DistPlan:
+    h = c_void_p(0)
+    _check(lib.hcms_dist_plan(ctypes.byref(h), S, H, D, P, C, dtype, flags, rank), "hcms_dist_plan")
+    return DistPlan(h.value, S, H, D, P, C, rank)
+
+
+def hcms_dist_export(plan: DistPlan) -> bytes:
+    buf = ctypes.create_string_buffer(HCMS_DIST_HANDLE_BYTES)
+    _check(lib.hcms_dist_export(plan.handle, buf), "hcms_dist_export")
+    return buf.raw
+
+
+def hcms_dist_attach(plan: DistPlan, handles) -> None:
+    """handles: the P ranks' hcms_dist_export bytes in rank order."""
+    blob = b"".join(handles)
+    if len(blob) != HCMS_DIST_HANDLE_BYTES * len(handles):
+        raise ValueError("every handle must be HCMS_DIST_HANDLE_BYTES long")
+    buf = ctypes.create_string_buffer(blob, len(blob))
+    _check(lib.hcms_dist_attach(plan.handle, buf, len(handles)), "hcms_dist_attach")
+
+
+def hcms_dist_attach_local(plan: DistPlan, peers) -> None:
+    arr = (c_void_p * len(peers))(*[p.handle.value for p in peers])
+    _check(lib.hcms_dist_attach_local(plan.handle, arr, len(peers)), "hcms_dist_attach_local")
+
+
+def hcms_dist_attention_forward(plan: DistPlan, q, k, v, out, scale: float, stream=None) -> None:
+    _check(lib.hcms_dist_attention_forward(plan.handle, _ptr(q), _ptr(k), _ptr(v), _ptr(out), scale, _stream(stream)),
+           "hcms_dist_attention_forward")
+
+
+def hcms_dist_attention_forward_group(plans, qs, ks, vs, outs, scale: float, streams) -> None:
+    """All P ranks of one process in one call (plans attached with hcms_dist_attach_local), distinct caller streams."""
+    n = len(plans)
+    arr = lambda xs: (c_void_p * n)(*[_ptr(x) for x in xs])
+    pl = (c_void_p * n)(*[p.handle.value for p in plans])
+    st = (c_void_p * n)(*[_stream(s) for s in streams])
+    _check(lib.hcms_dist_attention_forward_group(pl, n, arr(qs), arr(ks), arr(vs), arr(outs), scale, st),
+           "hcms_dist_attention_forward_group")
+
+
+def hcms_dist_block_bytes(plan: DistPlan) -> int:
+    return lib.hcms_dist_block_bytes(plan.handle)
+
+
+def hcms_dist_last_launch_count(plan: DistPlan) -> int:
+    return lib.hcms_dist_last_launch_count(plan.handle)
+
+
+def all_gather_bytes(blob: bytes, group=None):
+    """Every rank's `blob` (equal lengths) in rank order, over torch.distributed (any backend: the bytes travel as a
+    uint8 tensor on the backend's device).  Plumbing only."""
+    import torch
+    import torch.distributed as dist
+    mine = torch.frombuffer(bytearray(blob), dtype=torch.uint8)
+    if dist.get_backend(group) == "nccl":
+        mine = mine.cuda()
+    parts = [torch.empty_like(mine) for _ in range(dist.get_world_size(group))]
+    dist.all_gather(parts, mine, group=group)
+    return [t.cpu().numpy().tobytes() for t in parts]
+
+
+def hcms_dist_exchange_handles(plan: DistPlan, group=None):
+    """All-gather the ranks' export handles over torch.distributed and attach.  The data path never touches
+    torch.distributed: only these 128 bytes per rank do."""
+    import torch.distributed as dist
+    world = dist.get_world_size(group)
+    if world != plan.P:
+        raise ValueError(f"process group has {world} ranks, the plan has P={plan.P}")
+    handles = all_gather_bytes(hcms_dist_export(plan), group)
+    hcms_dist_attach(plan, handles)
+    return handles

@@ -36,6 +36,14 @@ struct LayoutVecParams {
   uint32_t step_cols;        // kVecThreads % run_vecs : ... and in vectors inside the run
 };
 
+// Distributed form (hcms_dist.cu, Alg. 1 lines 8 and 21 between P real ranks): the dense block
+// of logical rank p is the address peer[t][p] -- a row range of rank p's own chunk buffer, reached through a
+// CUDA-IPC / peer mapping -- instead of dense base + p * n_per_rank.  Scatter = PUSH (local strided shard -> stores
+// into every peer's chunk buffer), gather = PULL (loads from every peer's O'_c -> local strided shard).
+struct LayoutPeerTable {
+  uint8_t* peer[3][kMaxPeers];   // kMaxPeers: hcms_internal.h
+};
+
 // 128-bit and 256-bit (sm_100: LDG.256 / STG.256) streaming accesses that stay out of L1
 struct alignas(16) Vec16 {
   uint32_t v[4];
@@ -71,15 +79,19 @@ constexpr int kVecUnroll = 4;
 // Thread order follows the dense (contiguous) side: vector i of a rank's dense block is row s = i / run_vecs,
 // column w = i % run_vecs of the run.  One division per thread; the thread's next vectors lie kVecThreads
 // further, i.e. (step_rows, step_cols) further with a carry.  All loads are issued before the first store.
-template <bool kGather, typename Vec>
-__global__ void __launch_bounds__(kVecThreads) layout_vec_kernel(const LayoutVecParams p) {
+template <bool kGather, typename Vec, bool kPeer>
+__device__ __forceinline__ void layout_vec_body(const LayoutVecParams& p, const LayoutPeerTable* tab) {
   const uint32_t rank = blockIdx.y;
   // selects, not p.src[blockIdx.z]: a dynamically indexed kernel parameter is copied to the stack
   const uint32_t z = blockIdx.z;
   const uint8_t* __restrict__ src = z == 0 ? p.src[0] : (z == 1 ? p.src[1] : p.src[2]);
   uint8_t* __restrict__ dst = z == 0 ? p.dst[0] : (z == 1 ? p.dst[1] : p.dst[2]);
+  if (kPeer) {   // the dense side is rank `rank`'s buffer: one indexed constant-bank load of its address
+    uint8_t* dense = tab->peer[z][rank];
+    if (kGather) src = dense; else dst = dense;
+  }
   const uint32_t i0 = blockIdx.x * (kVecThreads * kVecUnroll) + threadIdx.x;
-  const size_t dense_base = static_cast<size_t>(rank) * p.n_per_rank;
+  const size_t dense_base = kPeer ? 0 : static_cast<size_t>(rank) * p.n_per_rank;
   const size_t strided_base = static_cast<size_t>(rank) * p.rank_stride_vecs + p.chunk_off_vecs;
   uint32_t s = i0 / p.run_vecs;
   uint32_t w = i0 - s * p.run_vecs;
@@ -109,13 +121,37 @@ __global__ void __launch_bounds__(kVecThreads) layout_vec_kernel(const LayoutVec
   }
 }
 
+template <bool kGather, typename Vec>
+__global__ void __launch_bounds__(kVecThreads) layout_vec_kernel(const LayoutVecParams p) {
+  layout_vec_body<kGather, Vec, false>(p, nullptr);
+}
+template <bool kGather, typename Vec>
+__global__ void __launch_bounds__(kVecThreads)
+layout_vec_peer_kernel(const LayoutVecParams p, const __grid_constant__ LayoutPeerTable tab) {
+  layout_vec_body<kGather, Vec, true>(p, &tab);
+}
+
 cudaError_t launch_layout_vec(const LayoutArgs& a, cudaStream_t stream) {
   LayoutVecParams p{};
   const size_t run_bytes = static_cast<size_t>(a.h_c) * a.D * a.es;
   // 256-bit accesses when every address is 32-byte aligned (runs are multiples of 128 B for D >= 64), else 128-bit
   bool wide = run_bytes % 32 == 0 && (static_cast<size_t>(a.D) * a.es) % 32 == 0;
-  for (int t = 0; t < a.n_tensors; ++t)
-    wide = wide && reinterpret_cast<uintptr_t>(a.src[t]) % 32 == 0 && reinterpret_cast<uintptr_t>(a.dst[t]) % 32 == 0;
+  const bool peer = a.peer[0] != nullptr;
+  if (peer && a.P > kMaxPeers) return cudaErrorInvalidValue;
+  LayoutPeerTable tab{};
+  for (int t = 0; t < a.n_tensors; ++t) {
+    // peer form: the strided side is src (scatter) / dst (gather); the dense side comes from the table
+    const void* strided = a.gather ? a.dst[t] : a.src[t];
+    if (peer) {
+      wide = wide && reinterpret_cast<uintptr_t>(strided) % 32 == 0;
+      for (int r = 0; r < a.P; ++r) {
+        tab.peer[t][r] = static_cast<uint8_t*>(a.peer[t][r]);
+        wide = wide && reinterpret_cast<uintptr_t>(a.peer[t][r]) % 32 == 0;
+      }
+    } else {
+      wide = wide && reinterpret_cast<uintptr_t>(a.src[t]) % 32 == 0 && reinterpret_cast<uintptr_t>(a.dst[t]) % 32 == 0;
+    }
+  }
   const size_t vb = wide ? 32 : 16;
   const size_t n_per_rank = static_cast<size_t>(a.S) * (run_bytes / vb);
   if (run_bytes % vb || n_per_rank >= (1ull << 31)) return cudaErrorInvalidValue;
@@ -132,6 +168,20 @@ cudaError_t launch_layout_vec(const LayoutArgs& a, cudaStream_t stream) {
   p.step_cols = kVecThreads % p.run_vecs;
   const uint32_t per_block = kVecThreads * kVecUnroll;
   dim3 grid((p.n_per_rank + per_block - 1) / per_block, a.P, a.n_tensors);
+  if (peer) {
+    if (a.gather) {
+      if (wide)
+        layout_vec_peer_kernel<true, Vec32><<<grid, kVecThreads, 0, stream>>>(p, tab);
+      else
+        layout_vec_peer_kernel<true, Vec16><<<grid, kVecThreads, 0, stream>>>(p, tab);
+    } else {
+      if (wide)
+        layout_vec_peer_kernel<false, Vec32><<<grid, kVecThreads, 0, stream>>>(p, tab);
+      else
+        layout_vec_peer_kernel<false, Vec16><<<grid, kVecThreads, 0, stream>>>(p, tab);
+    }
+    return cudaGetLastError();
+  }
   if (a.gather) {
     if (wide)
       layout_vec_kernel<true, Vec32><<<grid, kVecThreads, 0, stream>>>(p);

@@ -59,3 +59,52 @@ def test_reference_arm_prints_one_line_on_rank0_only():
     assert line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["cores"] >= 1
     for key in ("metric", "unit", "steps", "warmup", "ms_per_step", "higher_is_better", "config"):
         assert key in line
+
+
+# ---------------------------------------------------------------------------------------------
+# hcms_dist: host-side plumbing of the multi-rank path, no GPU
+# ---------------------------------------------------------------------------------------------
+
+def _gather_worker(rank, world, port, q):
+    os.environ.update(RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    sys.path.insert(0, ROOT)
+    import torch.distributed as dist
+    import paper_2607_01817_b200 as H
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    blob = bytes([rank + 1]) * H.HCMS_DIST_HANDLE_BYTES                # stands in for this rank's export handle
+    parts = H.all_gather_bytes(blob)
+    q.put((rank, [p[0] for p in parts], [len(p) for p in parts]))
+    dist.destroy_process_group()
+
+
+def test_handle_exchange_is_rank_ordered_gloo():
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 29950 + os.getpid() % 40
+    procs = [ctx.Process(target=_gather_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    for rank, firsts, lens in res:
+        assert firsts == [1, 2] and lens == [128, 128]                 # rank order, on every rank
+
+
+def test_dist_plan_validation_precedes_device_use():
+    sys.path.insert(0, ROOT)
+    import paper_2607_01817_b200 as H
+    for args, code in [((1024, 4, 64, 2, 2, 2), H.HCMS_ERR_INVALID_ARG),            # rank >= P
+                       ((1024, 4, 64, 2, 3, 0), H.HCMS_ERR_UNSUPPORTED_SHAPE),      # C > H/P
+                       ((1000, 4, 64, 3, 1, 0), H.HCMS_ERR_UNSUPPORTED_SHAPE),      # S % P
+                       ((1024, 4, 96, 2, 1, 0), H.HCMS_ERR_UNSUPPORTED_SHAPE),      # D
+                       ((1088, 34, 64, 17, 1, 0), H.HCMS_ERR_UNSUPPORTED_SHAPE)]:   # P > 16 peers
+        with pytest.raises(H.HcmsError) as ei:
+            H.hcms_dist_plan(*args)
+        assert ei.value.status == code, args
+    with pytest.raises(H.HcmsError) as ei:
+        H.hcms_dist_plan(1024, 4, 64, 2, 2, 0, H.HCMS_DTYPE_F32)
+    assert ei.value.status == H.HCMS_ERR_UNSUPPORTED_DTYPE
+    assert H.lib.hcms_dist_block_bytes(None) == 0 and H.lib.hcms_dist_plan_destroy(None) == 0
+    assert H.lib.hcms_dist_attention_forward(None, None, None, None, None, 1.0, None) == H.HCMS_ERR_INVALID_ARG
