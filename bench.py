@@ -60,7 +60,9 @@ def parse_args(argv=None):
     ap.add_argument("--layout", default="vec", choices=["vec", "tma"])
     ap.add_argument("--single-comp", action="store_true", help="HCMS_FLAG_SINGLE_COMP: one compute stream, as Alg. 1")
     ap.add_argument("--attn-pair", action="store_true", help="HCMS_FLAG_ATTN_PAIR: attention forward on CTA pairs (D = 128)")
-    ap.add_argument("--attn-split", action="store_true", help="HCMS_FLAG_ATTN_SPLIT: pair kernel, two softmax threads per row")
+    ap.add_argument("--replicas", action="store_true", help="N > 1: independent replicas per rank instead of the sequence-sharded "
+                                                            "hcms_dist path")
+    ap.add_argument("--share-gpu", action="store_true", help="N > 1 on ONE GPU (tests): every rank uses cuda:0, rendezvous over gloo")
     ap.add_argument("--quick", action="store_true", help="only the contract measurement of the hot path (no layer, backward, e2e, "
                                                          "graph, value-independence, cpu baseline blocks)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -88,6 +90,7 @@ def peaks():
 # ---------------------------------------------------------------------------------------------
 
 def dist_init(use_cuda: bool):
+    """use_cuda: collectives on device tensors over NCCL (one GPU per rank); else gloo on host tensors."""
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -362,6 +365,104 @@ def measure_backward(args, H, torch, w, C, base_flags, timed, pk, qd, kd, vd, ou
     }
 
 
+def run_dist(args, torch, H, rank, local, world, nccl):
+    """N > 1: the paper's actual setting (L45, L59).  The workload's global [S,H,D] tensors are
+    SEQUENCE-SHARDED over the N ranks (P = N, one GPU per rank), every rank runs hcms_dist_attention_forward: its scatter
+    kernel stores into the peers' chunk buffers, its gather kernel loads from them (CUDA-IPC peer memory = NVLink on a
+    real node), attention on its own H/N heads.  Strong scaling: the layer's total work is fixed.  The only use of
+    torch.distributed is the rendezvous (128 handle bytes per rank), the barrier and the MAX over ranks."""
+    import torch.distributed as dist
+    dev = torch.device("cuda", local)
+    pk = peaks()
+    w = I.workload(args.config)
+    S, Hh, D, P = w.S, w.H, w.D, world
+    if S % P or Hh % P:
+        raise ValueError(f"workload S={S}, H={Hh} cannot be sharded over {P} ranks")
+    Hl = Hh // P
+    C = min(args.chunks or w.C, Hl)
+    Sl = S // P
+    threads = max(1, (os.cpu_count() or 8) // world)
+    q, k, v = I.make_qkv(w, threads=threads)
+    if w.dtype == "f32":
+        q, k, v = (I.f32_to_bf16_bits(t) for t in (q, k, v))
+    host = [torch.from_numpy(np.ascontiguousarray(t[rank * Sl:(rank + 1) * Sl]).view(np.int16)).pin_memory() for t in (q, k, v)]
+    host_out = torch.empty_like(host[0]).pin_memory()
+    qd, kd, vd = (t.to(dev, non_blocking=True) for t in host)
+    out = torch.empty_like(qd)
+    torch.cuda.synchronize()
+    plan = H.hcms_dist_plan(S, Hh, D, P, C, rank)
+    H.hcms_dist_exchange_handles(plan)
+    stream = torch.cuda.current_stream()
+    flop_step = 4.0 * S * S * D * Hh                       # the whole layer, all ranks together
+    step = lambda: H.hcms_dist_attention_forward(plan, qd, kd, vd, out, w.scale)
+
+    def timed(steps, fn):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(steps):
+            fn()
+        e1.record(stream)
+        e1.synchronize()
+        return e0.elapsed_time(e1)
+
+    for _ in range(args.warmup):
+        step()
+    barrier(world, True)
+    sampler = ClockSampler(local)
+    time.sleep(0.25)
+    t0 = sampler.mark()
+    ms_total = timed(args.steps, step)
+    torch.cuda.synchronize()
+    t1 = sampler.mark()
+    barrier(world, True)
+    clocks = sampler.stop(t0, t1)
+    ms_per_step = max_over_ranks(ms_total, world, nccl) / args.steps
+    launches = H.hcms_dist_last_launch_count(plan) * args.steps
+
+    # end to end: this rank's shard from pinned host memory, forward, its output shard back
+    def step_e():
+        a, b, c_ = (t.to(dev, non_blocking=True) for t in host)
+        H.hcms_dist_attention_forward(plan, a, b, c_, out, w.scale)
+        host_out.copy_(out, non_blocking=True)
+    n_e = min(args.steps, 10)
+    for _ in range(2):
+        step_e()
+    barrier(world, True)
+    ms_e = max_over_ranks(timed(n_e, step_e), world, nccl) / n_e
+    barrier(world, True)
+    shard_bytes = Sl * Hh * D * 2
+    peak_tf = pk["bf16_tflops"] * world
+    value = flop_step / (ms_per_step * 1e-3) / 1e12
+    result = {
+        "metric": METRIC, "value": round(value, 2), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": round(ms_per_step, 4), "higher_is_better": True, "scaling": "strong",
+        "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[{args.config - 1}] ({w.name}): S={S} H={Hh} D={D} sequence-sharded over "
+                               f"P={P} ranks, C={C} head chunks of H/P={Hl} local heads, non-causal scale=1/sqrt(D)",
+                   "S": S, "H": Hh, "D": D, "P": P, "C": C,
+                   "multi_gpu": "sequence-sharded, P = N: hcms_dist (push scatter / pull gather over CUDA-IPC peer memory, "
+                                "epoch flags awaited by streams; no NCCL on the data path)" +
+                                (" -- ranks SHARE cuda:0 (test mode)" if args.share_gpu else ""),
+                   "l2": "inputs larger than L2" if 3 * shard_bytes >= 2 * L2_BYTES else "per-rank shards fit in L2 (not flushed)",
+                   "inputs": "hcms_inputs counter-based N(0,1) -> bf16 (seed %d), rank r holds rows [r*S/P, (r+1)*S/P)" % w.seed},
+        "clocks": clocks, "gpu_launches": launches,
+        "roofline": {"kernel": "attention_fwd_kernel<%d> (whole step per rank: pushes, attention, pulls)" % D, "bound": "tensor",
+                     "achieved": round(value, 1), "peak": peak_tf, "unit": "TFLOP/s", "frac": round(value / peak_tf, 4),
+                     "peak_kind": "N x bf16 dense burst (cuBLAS), %s" % pk["source"], "traffic": None,
+                     "nvlink_bytes_per_rank_per_step": 4 * shard_bytes * (P - 1) // P},
+        "e2e": {"value": round(flop_step / (ms_e * 1e-3) / 1e12, 2), "unit": UNIT, "h2d_bytes_per_step": 3 * shard_bytes * world,
+                "d2h_bytes_per_step": shard_bytes * world, "ms_per_step": round(ms_e, 3), "steps": n_e,
+                "api": "per rank: pinned host shard -> device, hcms_dist_attention_forward, output shard -> pinned host"},
+    }
+    torch.cuda.synchronize()
+    barrier(world, True)
+    plan.close()
+    if rank == 0:
+        print(json.dumps(result), flush=True)
+    barrier(world, True)
+    dist.destroy_process_group()
+
+
 def run_hcms(args):
     import torch
     import paper_2607_01817_b200 as H   # raises if libhcms.so is missing: there is no fallback
@@ -369,10 +470,15 @@ def run_hcms(args):
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the HCMS hot path has no CPU fallback "
                          "(use --impl reference for the oracle timing)")
-    rank, local, world = dist_init(True)
+    nccl = not args.share_gpu
+    rank, local, world = dist_init(nccl)
+    if args.share_gpu:
+        local = 0
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     pk = peaks()
+    if world > 1 and not args.replicas:
+        return run_dist(args, torch, H, rank, local, world, nccl)
 
     w = I.workload(args.config)
     C = args.chunks or w.C
@@ -392,8 +498,7 @@ def run_hcms(args):
     flush = 3 * tensor_bytes < 2 * L2_BYTES
     flush_buf = torch.empty(2 * L2_BYTES, dtype=torch.uint8, device=dev) if flush else None
     base_flags = (H.HCMS_FLAG_PROFILE | (H.HCMS_FLAG_LAYOUT_TMA if args.layout == "tma" else 0) |
-                  (H.HCMS_FLAG_SINGLE_COMP if args.single_comp else 0) | (H.HCMS_FLAG_ATTN_PAIR if args.attn_pair else 0) |
-                  (H.HCMS_FLAG_ATTN_SPLIT if args.attn_split else 0))
+                  (H.HCMS_FLAG_SINGLE_COMP if args.single_comp else 0) | (H.HCMS_FLAG_ATTN_PAIR if args.attn_pair else 0))
     stream = torch.cuda.current_stream()
 
     def timed(plan, steps, fn):
@@ -429,8 +534,8 @@ def run_hcms(args):
             acc += np.asarray(H.hcms_plan_timings(plan, back))
         return acc / n
 
-    # ---- main measurement: HCMS dual-stream pipeline ---------------------------------------
-    plan = H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, base_flags)
+    # ---- main measurement: HCMS dual-stream pipeline, exactly the call a user makes (no profile events) -------
+    plan = H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, base_flags & ~H.HCMS_FLAG_PROFILE)
     step = lambda: H.hcms_attention_forward(plan, qd, kd, vd, out, w.scale)
     for _ in range(args.warmup):
         step()
@@ -444,11 +549,20 @@ def run_hcms(args):
     barrier(world, True)
     clocks = sampler.stop(t_wall0, t_wall1)
     launches = H.hcms_plan_last_launch_count(plan) * args.steps
-    kt = kernel_times(plan, args.steps)
     value_per_s, ms_per_step = aggregate_value(flop_step, args.steps, world, ms_total, True)
     _, h_c = H.hcms_chunk_table(plan)
+    plan.close()
+    # the dominant kernel's duration: the same call on a HCMS_FLAG_PROFILE plan (timing events on the compute streams
+    # around every attention launch; 6 extra event records per chunk, so not the plan that produces `value`)
+    plan = H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, base_flags)
+    step_p = lambda: H.hcms_attention_forward(plan, qd, kd, vd, out, w.scale)
+    n_prof = max(3, min(args.steps, 10))
+    for _ in range(2):
+        step_p()
+    torch.cuda.synchronize()
+    prof_ms = timed(plan, n_prof, step_p) / n_prof
     attn_flop = [4.0 * S * S * D * P * h for h in h_c]
-    attn_ms = attn_span(plan, args.steps)
+    attn_ms = attn_span(plan, n_prof)
     achieved = sum(attn_flop) / (attn_ms * 1e-3) / 1e12
     # The timed region is a fraction of a second, so the honest denominator is the BURST cuBLAS figure (a kernel
     # timed alone); the sustained (power-capped, seconds-long) and nominal figures are reported beside it.
@@ -473,7 +587,8 @@ def run_hcms(args):
                      "algorithmic_bytes": 4 * tensor_bytes,
                      "frac_of_sustained": round(achieved / pk["bf16_tflops_sustained"], 4),
                      "frac_of_nominal": round(achieved / NOMINAL_BF16_TFLOPS, 4),
-                     "attn_ms_per_step": round(attn_ms, 4), "flop_per_step": sum(attn_flop)},
+                     "attn_ms_per_step": round(attn_ms, 4), "flop_per_step": sum(attn_flop),
+                     "measured_on": "HCMS_FLAG_PROFILE plan, %d steps, %.4f ms per step with the profile events" % (n_prof, prof_ms)},
     }
     plan.close()
     if args.quick:
@@ -496,33 +611,63 @@ def run_hcms(args):
     plan_s.close()
     chunk_bytes = [2.0 * P * S * h * D * 2 for h in h_c]          # read + write, one tensor
     copy_ms, comp_ms = float(ks[0].sum() + ks[2].sum()), float(ks[1].sum())
-    sc_gbs = 3 * sum(chunk_bytes) / (ks[0].sum() * 1e-3) / 1e9
-    ga_gbs = sum(chunk_bytes) / (ks[2].sum() * 1e-3) / 1e9
+    # Layout kernels alone: one PASS = every chunk's launch back to back on one stream (each pass touches the whole
+    # tensors once, 4 x one tensor > L2 for configs 3-5), one event pair around `n_ser` passes.  Per-launch event pairs
+    # (the HCMS_FLAG_PROFILE numbers below, `*_profiled_gbs`) add ~10 us of event and launch-gap time to a 30-90 us kernel.
+    plan_l = H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, base_flags & ~H.HCMS_FLAG_PROFILE)
+    ws_l = torch.empty(H.hcms_plan_workspace_bytes(plan_l), dtype=torch.uint8, device=dev)
+    H.hcms_plan_set_workspace(plan_l, ws_l, ws_l.numel())
+    lay = [H.hcms_chunk_layout(plan_l, c) for c in range(C)]
+    base_l = ws_l.data_ptr()
+
+    def scatter_pass():
+        for c in range(C):
+            H.hcms_a2a_scatter(plan_l, [qd, kd, vd], [base_l + lay[c][key] for key in ("q_off", "k_off", "v_off")], c)
+
+    def gather_pass():
+        for c in range(C):
+            H.hcms_a2a_gather(plan_l, base_l + lay[c]["o_off"], out, c)
+
+    for fn in (scatter_pass, gather_pass):
+        fn()
+    torch.cuda.synchronize()
+    sc_pass_ms = timed(plan_l, n_ser, scatter_pass) / n_ser
+    ga_pass_ms = timed(plan_l, n_ser, gather_pass) / n_ser
+    plan_l.close()
+    del ws_l
+    sc_gbs = 3 * sum(chunk_bytes) / (sc_pass_ms * 1e-3) / 1e9
+    ga_gbs = sum(chunk_bytes) / (ga_pass_ms * 1e-3) / 1e9
     result["layout"] = {
+        "scatter_pass_ms": round(sc_pass_ms, 4), "gather_pass_ms": round(ga_pass_ms, 4),
+        "scatter_profiled_gbs": round(3 * sum(chunk_bytes) / (ks[0].sum() * 1e-3) / 1e9, 1),
+        "gather_profiled_gbs": round(sum(chunk_bytes) / (ks[2].sum() * 1e-3) / 1e9, 1),
+        "fits_in_l2": bool(flush),
         "scatter_gbs": round(sc_gbs, 1), "gather_gbs": round(ga_gbs, 1),
         "scatter_frac": round(sc_gbs / pk["hbm_gbs"], 4), "gather_frac": round(ga_gbs / pk["hbm_gbs"], 4),
         "scatter_frac_of_nominal": round(sc_gbs / NOMINAL_HBM_GBS, 4), "gather_frac_of_nominal": round(ga_gbs / NOMINAL_HBM_GBS, 4),
-        "all_gbs": round(4 * sum(chunk_bytes) / (copy_ms * 1e-3) / 1e9, 1),
+        "all_gbs": round(4 * sum(chunk_bytes) / ((sc_pass_ms + ga_pass_ms) * 1e-3) / 1e9, 1),
         "peak_gbs": pk["hbm_gbs"], "peak_kind": "HBM copy, %s" % pk["source"],
-        "frac": round(4 * sum(chunk_bytes) / (copy_ms * 1e-3) / 1e9 / pk["hbm_gbs"], 4),
-        "frac_of_nominal": round(4 * sum(chunk_bytes) / (copy_ms * 1e-3) / 1e9 / NOMINAL_HBM_GBS, 4),
-        "bytes_per_step": 4 * sum(chunk_bytes), "copy_ms_per_step": round(copy_ms, 4),
+        "frac": round(4 * sum(chunk_bytes) / ((sc_pass_ms + ga_pass_ms) * 1e-3) / 1e9 / pk["hbm_gbs"], 4),
+        "frac_of_nominal": round(4 * sum(chunk_bytes) / ((sc_pass_ms + ga_pass_ms) * 1e-3) / 1e9 / NOMINAL_HBM_GBS, 4),
+        "bytes_per_step": 4 * sum(chunk_bytes), "copy_ms_per_step": round(sc_pass_ms + ga_pass_ms, 4),
+        "copy_profiled_ms_per_step": round(copy_ms, 4),
     }
     # The Ulysses baseline of Eq. 1 is ONE attention call over all H/P heads: a serial plan with C = 1 (the serial plan
     # at the workload's C pays a tail wave per chunk, which the two alternating compute streams of the HCMS run
     # back-fill: that gain is reported separately and is not communication overlap).
-    if C > 1:
-        plan_u = H.hcms_plan(S, Hh, D, P, 1, H.HCMS_DTYPE_BF16, base_flags | H.HCMS_FLAG_SERIAL)
+    uly = {}
+    for prof in (0, H.HCMS_FLAG_PROFILE):        # timed without profile events (like `value`); kernel times with them
+        plan_u = H.hcms_plan(S, Hh, D, P, 1, H.HCMS_DTYPE_BF16, (base_flags & ~H.HCMS_FLAG_PROFILE) | prof | H.HCMS_FLAG_SERIAL)
         step_u = lambda: H.hcms_attention_forward(plan_u, qd, kd, vd, out, w.scale)
         for _ in range(2):
             step_u()
         torch.cuda.synchronize()
-        uly_ms = timed(plan_u, n_ser, step_u) / n_ser
-        ku = kernel_times(plan_u, n_ser)
+        uly[prof] = timed(plan_u, n_ser, step_u) / n_ser
+        if prof:
+            ku = kernel_times(plan_u, n_ser)
         plan_u.close()
-        uly_copy_ms, uly_attn_ms = float(ku[0].sum() + ku[2].sum()), float(ku[1].sum())
-    else:
-        uly_ms, uly_copy_ms, uly_attn_ms = ser_ms, copy_ms, comp_ms
+    uly_ms = uly[0]
+    uly_copy_ms, uly_attn_ms = float(ku[0].sum() + ku[2].sum()), float(ku[1].sum())
     # compute side alone in the SAME stream arrangement as the HCMS run (two alternating compute streams, same events),
     # no copies: HCMS_FLAG_DEBUG_ATTN_ONLY on chunk buffers a normal call has filled
     plan_a = H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, (base_flags & ~H.HCMS_FLAG_PROFILE) | H.HCMS_FLAG_DEBUG_ATTN_ONLY)
@@ -540,7 +685,7 @@ def run_hcms(args):
     attn_dual_ms = timed(plan_a, n_ser, step_a) / n_ser
     plan_a.close()
     del ws_keep
-    rho = uly_copy_ms / uly_ms
+    rho = uly_copy_ms / uly[H.HCMS_FLAG_PROFILE]
     result["pipeline"] = {
         "hcms_ms": round(ms_per_step, 4),
         "ulysses_serial_C1_ms": round(uly_ms, 4), "speedup_vs_ulysses": round(uly_ms / ms_per_step, 4),
@@ -609,6 +754,7 @@ def run_hcms(args):
         host_us = (time.perf_counter() - t0) * 1e6 / n_g
         g_res[name] = (ms_g, host_us)
         plan_g.close()
+    result["pipeline"]["wall_over_max_compute_copy_graph"] = round(g_res["graph"][0] / max(attn_dual_ms, copy_ms), 4)
     result["graph"] = {"enqueue_ms": round(g_res["enqueue"][0], 4), "graph_ms": round(g_res["graph"][0], 4),
                        "speedup": round(g_res["enqueue"][0] / g_res["graph"][0], 4), "steps": n_g,
                        "what": "hcms_attention_forward without profile events: %d launches + events enqueued per call vs one "
@@ -635,6 +781,18 @@ def run_hcms(args):
         same = bool(torch.equal(host_out.to(dev), out))
         result["e2e"]["bitwise_equal_to_device_path"] = same
         plan_e.close()
+        # the variant whose all-to-alls are the layout KERNELS (whole tensors to device staging, then the device path):
+        # the default above lets the copy engines do the permutation, so it says nothing about scatter / gather
+        plan_st = H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, (base_flags & ~H.HCMS_FLAG_PROFILE) | H.HCMS_FLAG_HOST_STAGED)
+        step_st = lambda: H.hcms_attention_forward_host(plan_st, host[0], host[1], host[2], host_out, w.scale)
+        for _ in range(2):
+            step_st()
+        ms_st = timed(plan_st, max(2, n_e // 2), step_st) / max(2, n_e // 2)
+        result["e2e"]["staged"] = {"flag": "HCMS_FLAG_HOST_STAGED", "ms_per_step": round(ms_st, 3),
+                                   "value": round(flop_step / (ms_st * 1e-3) / 1e12, 2),
+                                   "launches_per_step": H.hcms_plan_last_launch_count(plan_st) + 4,
+                                   "bitwise_equal_to_device_path": bool(torch.equal(host_out.to(dev), out))}
+        plan_st.close()
         if world == 1:
             # adaptive C over the host link (future work L346 via Theorem 1): every C in [1, H/P], 2 timed calls each
             best_C, ms_C = H.hcms_autotune_chunks_host(S, Hh, D, P, base_flags & ~H.HCMS_FLAG_PROFILE, host[0], host[1],

@@ -123,10 +123,6 @@ enum {
                                           use the single-CTA tcgen05 GEMM (128 x 256 tiles) also where the default
                                           CTA-pair kernel (cta_group::2, 256 x 256 tiles) applies.  Same bits. */
 
-#define HCMS_FLAG_ATTN_SPLIT 0x40000u   /* D = 128 only: the CTA-pair attention kernel with TWO softmax threads per query row
-                                          (16 softmax warps per CTA, each thread 64 of the tile's 128 keys; half-row maxima
-                                          and sums are exchanged through shared memory).  Implies HCMS_FLAG_ATTN_PAIR. */
-
 #define HCMS_FLAG_DEBUG_ATTN_ONLY 0x20000u /* MEASUREMENT ONLY: hcms_attention_forward skips the scatter and gather
                                           kernels (events, streams and attention launches unchanged), so that the
                                           compute side of the pipeline can be timed in the same stream arrangement
@@ -435,8 +431,7 @@ void* hcms_plan_lse(const hcms_plan_t* plan);
  * the concatenated outputs of the P ranks are BIT-EQUAL to hcms_attention_forward on the concatenated inputs.
  *
  * hcms_dist_plan: collective in spirit (every rank creates its own with the same S, H, D, P, C); allocates the
- * exchange block (4*S*(H/P)*D*2 bytes + flags) on the current device.  flags: 0, HCMS_FLAG_ATTN_PAIR or
- * HCMS_FLAG_ATTN_SPLIT.  bf16 only.
+ * exchange block (4*S*(H/P)*D*2 bytes + flags) on the current device.  flags: 0 or HCMS_FLAG_ATTN_PAIR.  bf16 only.
  * hcms_dist_export: writes HCMS_DIST_HANDLE_BYTES opaque bytes that another PROCESS passes to hcms_dist_attach.
  * hcms_dist_attach: `handles` = P consecutive handles in rank order (this rank's own entry is checked, not opened);
  * the caller moves the bytes between processes with any host channel (torch.distributed, files).

@@ -8,8 +8,8 @@
 //
 // Two deterministic passes (no atomics, so the gradients are bitwise independent of the chunking, like the
 // forward: Table 14), both instances of ONE kernel template:
-//   kDQ = false  "dK/dV pass": a CTA owns 128 keys (R1 = K_j, R2 = V_j resident) and streams 64-query tiles
-//                (X = Q_t, Y = dO_t):  T1 = K_j Q_t^T = S^T, T2 = V_j dO_t^T = dP^T  (M = 128 keys, N = 64 queries);
+//   kDQ = false  "dK/dV pass": a CTA owns 128 keys (R1 = K_j, R2 = V_j resident) and streams 32-query tiles
+//                (X = Q_t, Y = dO_t):  T1 = K_j Q_t^T = S^T, T2 = V_j dO_t^T = dP^T  (M = 128 keys, N = 32 queries);
 //                P^T = exp2(T1*c - lse2[col]), dS^T = P^T o (T2 - delta[col]);  dV += P^T dO_t,  dK += dS^T Q_t.
 //   kDQ = true   "dQ pass": a CTA owns 128 queries (R1 = Q_i, R2 = dO_i resident) and streams 64-key tiles
 //                (X = K_t, Y = V_t):  T1 = Q_i K_t^T = S, T2 = dO_i V_t^T = dP  (M = 128 queries, N = 64 keys);
@@ -22,7 +22,11 @@
 // T1/T2 columns in TMEM.  P and dS are written back INTO those columns as packed bf16 and feed the accumulating
 // MMAs as TMEM A operands (tcgen05.mma with A in TMEM): the kernel is bound by shared-memory operand traffic
 // (ncu: tensor queue always full at 52 % pipe activity with P/dS staged in shared memory), and this removes the
-// P/dS stores and their re-reads from it.  TMEM: T1[2] 0..127, T2[2] 128..255, accumulators from 256.
+// P/dS stores and their re-reads from it.  The RESIDENT operands (K_j, V_j / Q_i, dO_i) are copied into TMEM once per
+// CTA as well, so every T1 / T2 MMA reads only the streamed tile from shared memory.  In the dK/dV pass that is what
+// fits 512 columns only with 32-query tiles: T1[2], T2[2] 4 x 32 + K_j, V_j 2 x D/2 + dV, dK 2 x D (round 1 used
+// 64-query tiles with K_j, V_j as shared-memory operands: the shared-memory pipe was 100 % busy at 71 % tensor activity).
+// TMEM columns: T1[2] at 0, T2[2] at 2*kC, R1 at 4*kC, R2 at 4*kC + D/2, accumulators at 4*kC + D.
 #include <cuda_bf16.h>
 
 #include "hcms_internal.h"
@@ -34,32 +38,37 @@ using namespace ptx;
 namespace {
 
 constexpr int kRows = 128;        // resident rows per CTA (UMMA M)
-constexpr int kCols = 64;         // streamed rows per iteration (UMMA N of T1/T2, K extent of the accumulating GEMMs)
+constexpr int kPad = 64;          // the packed statistics are padded to a multiple of this many rows
 constexpr int kThreads = 384;
 constexpr int kTmemCols = 512;
 
-template <int D>
+// kCols = streamed rows per iteration (UMMA N of T1/T2, K extent of the accumulating GEMMs): 32 in the dK/dV pass,
+// 64 in the dQ pass
+template <int D, bool kDQ>
 struct Cfg {
+  static constexpr int kCols = kDQ ? 64 : 32;
   static constexpr int kPanels = D / 64;
   static constexpr int kResBytes = kPanels * kRows * 128;      // one resident tile
-  static constexpr int kStrPanelBytes = kCols * 128;           // one 64-row panel of a streamed tile
+  static constexpr int kStrPanelBytes = kCols * 128;           // one 64-element-wide panel of a streamed tile
   static constexpr int kStrBytes = kPanels * kStrPanelBytes;   // one streamed tile
   static constexpr int kStageBytes = 2 * kStrBytes;            // X_t and Y_t
-  static constexpr int kStages = D == 128 ? 5 : 8;
-  static constexpr int kSmemBytes = 2 * kResBytes + kStages * kStageBytes + 1024 + 256;
-  static constexpr int kTmemT1 = 0, kTmemT2 = 128, kTmemAcc = 256;
-  static constexpr int kTmemR1 = 384, kTmemR2 = 448;   // dQ pass only: Q_i, dO_i as packed bf16 (D/2 columns each)
+  static constexpr int kStages = (D == 128 ? 5 : 8) * (64 / kCols);
+  static constexpr int kSmemBytes = 2 * kResBytes + kStages * kStageBytes + 1024 + 512;
+  static constexpr int kTmemT1 = 0, kTmemT2 = 2 * kCols;
+  static constexpr int kTmemR1 = 4 * kCols, kTmemR2 = 4 * kCols + D / 2;   // resident operands as packed bf16 (D/2 columns each)
+  static constexpr int kTmemAcc = 4 * kCols + D;
+  static_assert(kTmemAcc + (kDQ ? D : 2 * D) <= kTmemCols, "TMEM budget");
 };
 
 struct alignas(64) BwdMaps {
   CUtensorMap r1, r2;     // resident operands, box {64, 1, 128, 1} over {D, h_c, S, P}
-  CUtensorMap x, y;       // streamed operands, box {64, 1, 64, 1}
+  CUtensorMap x, y;       // streamed operands, box {64, 1, kCols, 1}
   CUtensorMap out1, out2; // dV, dK (dK/dV pass) or dQ, unused (dQ pass); box {64, 1, 128, 1}
 };
 
 struct BwdParams {
   int S;
-  int n_iter;             // ceil(S / 64)
+  int n_iter;             // s_pad / kCols
   int h_c;
   int s_pad;              // row pitch of `stats` (multiple of 64, >= S)
   float scale;
@@ -82,8 +91,9 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
 template <int D, bool kDQ>
 __global__ void __launch_bounds__(kThreads, 1)
 attention_bwd_kernel(const __grid_constant__ BwdMaps maps, const BwdParams prm) {
-  using C = Cfg<D>;
+  using C = Cfg<D, kDQ>;
   constexpr int kStages = C::kStages;
+  constexpr int kCols = C::kCols;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t r1_smem = smem_base;
@@ -96,7 +106,7 @@ attention_bwd_kernel(const __grid_constant__ BwdMaps maps, const BwdParams prm) 
   const uint32_t bar_t_full = bar_x_empty + 8 * kStages;     // [2] MMA -> warpgroup: T1, T2 of its tile are in TMEM
   const uint32_t bar_pd_full = bar_t_full + 16;              // [2] warpgroup -> MMA: P / dS of its tile are in TMEM
   const uint32_t bar_done = bar_pd_full + 16;                // MMA -> all: every accumulation has completed
-  const uint32_t bar_rt_full = bar_done + 8;                 // dQ pass: warpgroups -> MMA: Q_i, dO_i copied into TMEM
+  const uint32_t bar_rt_full = bar_done + 8;                 // warpgroups -> MMA: the resident tiles are copied into TMEM
   const uint32_t tmem_slot = bar_rt_full + 8;
 
   const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
@@ -178,30 +188,22 @@ attention_bwd_kernel(const __grid_constant__ BwdMaps maps, const BwdParams prm) 
       constexpr uint32_t hi = umma_desc_hi(1024);
       // T1 = R1 X^T and T2 = R2 Y^T of one streamed tile into TMEM buffer b
       auto issue_t = [&](int b, uint32_t stage_addr) {
-        const uint32_t r1_lo = umma_desc_lo(r1_smem, 16), r2_lo = umma_desc_lo(r2_smem, 16);
         const uint32_t x_lo = umma_desc_lo(stage_addr, 16), y_lo = umma_desc_lo(stage_addr + C::kStrBytes, 16);
 #pragma unroll
         for (int ks = 0; ks < D / 16; ++ks) {
-          const uint32_t r_off = ((ks >> 2) * (kRows * 128) + (ks & 3) * 32) >> 4;
           const uint32_t s_off = ((ks >> 2) * C::kStrPanelBytes + (ks & 3) * 32) >> 4;
-          if (kDQ)   // A = Q_i from TMEM: the resident operand costs no shared-memory bandwidth
-            mma_ts(tmem_base + C::kTmemT1 + b * kCols, tmem_base + C::kTmemR1 + ks * 8,
-                   (static_cast<uint64_t>(hi) << 32) | (x_lo + s_off), idesc_t, ks > 0 ? 1u : 0u);
-          else
-            mma_ss_lohi(tmem_base + C::kTmemT1 + b * kCols, r1_lo + r_off, x_lo + s_off, hi, hi, idesc_t, ks > 0 ? 1u : 0u);
+          // A = the resident operand from TMEM: it costs no shared-memory bandwidth
+          mma_ts(tmem_base + C::kTmemT1 + b * kCols, tmem_base + C::kTmemR1 + ks * 8,
+                 (static_cast<uint64_t>(hi) << 32) | (x_lo + s_off), idesc_t, ks > 0 ? 1u : 0u);
         }
 #pragma unroll
         for (int ks = 0; ks < D / 16; ++ks) {
-          const uint32_t r_off = ((ks >> 2) * (kRows * 128) + (ks & 3) * 32) >> 4;
           const uint32_t s_off = ((ks >> 2) * C::kStrPanelBytes + (ks & 3) * 32) >> 4;
-          if (kDQ)
-            mma_ts(tmem_base + C::kTmemT2 + b * kCols, tmem_base + C::kTmemR2 + ks * 8,
-                   (static_cast<uint64_t>(hi) << 32) | (y_lo + s_off), idesc_t, ks > 0 ? 1u : 0u);
-          else
-            mma_ss_lohi(tmem_base + C::kTmemT2 + b * kCols, r2_lo + r_off, y_lo + s_off, hi, hi, idesc_t, ks > 0 ? 1u : 0u);
+          mma_ts(tmem_base + C::kTmemT2 + b * kCols, tmem_base + C::kTmemR2 + ks * 8,
+                 (static_cast<uint64_t>(hi) << 32) | (y_lo + s_off), idesc_t, ks > 0 ? 1u : 0u);
         }
       };
-      // acc[128 x D] += PD[128 x 64] * B[64 x D]: A = P or dS as packed bf16 in TMEM (8 columns per K step of 16),
+      // acc[128 x D] += PD[128 x kCols] * B[kCols x D]: A = P or dS as packed bf16 in TMEM (8 columns per K step of 16),
       // B MN-major in shared memory: 64-wide D panels kStrPanelBytes apart (LBO), 8-row groups 1024 B apart (SBO),
       // 16 rows (one K step) = 2048 B
       auto issue_acc = [&](uint32_t d_tmem, uint32_t a_tmem, uint32_t b_tile, bool accumulate) {
@@ -212,7 +214,7 @@ attention_bwd_kernel(const __grid_constant__ BwdMaps maps, const BwdParams prm) 
         }
       };
       mbar_wait(bar_r_full, 0);
-      if (kDQ) mbar_wait(bar_rt_full, 0);
+      mbar_wait(bar_rt_full, 0);
       tc_fence_after();
       // ring bookkeeping: tile t lives in stage t % kStages, its full-barrier phase is (t / kStages) & 1
       auto wait_tile = [&](int t) -> uint32_t {
@@ -278,9 +280,9 @@ attention_bwd_kernel(const __grid_constant__ BwdMaps maps, const BwdParams prm) 
       row_delta = st.y;
     }
 
-    if (kDQ) {
-      // warpgroup 0 copies Q_i, warpgroup 1 dO_i from the swizzled shared-memory tile into TMEM (row = lane, column c
-      // = elements 2c, 2c+1): the A operand of every T1 / T2 MMA of this CTA
+    {
+      // warpgroup 0 copies R1 (Q_i / K_j), warpgroup 1 R2 (dO_i / V_j) from the swizzled shared-memory tile into TMEM
+      // (row = lane, column c = elements 2c, 2c+1): the A operand of every T1 / T2 MMA of this CTA
       mbar_wait(bar_r_full, 0);
       const uint32_t src = (g == 0 ? r1_smem : r2_smem) + row * 128;
       const uint32_t dst = tmem_base + lane_addr + (g == 0 ? C::kTmemR1 : C::kTmemR2);
@@ -303,10 +305,10 @@ attention_bwd_kernel(const __grid_constant__ BwdMaps maps, const BwdParams prm) 
       mbar_wait(bar_t_full + 8 * g, k & 1);
       tc_fence_after();
       uint32_t s[kCols], dp[kCols];
-      tmem_ld32(t1_tmem, &s[0]);
-      tmem_ld32(t1_tmem + 32, &s[32]);
-      tmem_ld32(t2_tmem, &dp[0]);
-      tmem_ld32(t2_tmem + 32, &dp[32]);
+#pragma unroll
+      for (int c4 = 0; c4 < kCols / 32; ++c4) tmem_ld32(t1_tmem + c4 * 32, &s[c4 * 32]);
+#pragma unroll
+      for (int c4 = 0; c4 < kCols / 32; ++c4) tmem_ld32(t2_tmem + c4 * 32, &dp[c4 * 32]);
       tmem_wait_ld();
       const int valid = prm.S - t * kCols;                        // streamed rows of this tile that exist (dQ pass mask)
       // P and dS go back into the first 32 columns of T1 / T2 as packed bf16 (element 2c in the low half): the
@@ -337,8 +339,14 @@ attention_bwd_kernel(const __grid_constant__ BwdMaps maps, const BwdParams prm) 
           dw[ch * 4 + pr] = pack_bf16(e0, e1);
         }
       }
-      if (!kDQ) tmem_st32(t1_tmem, pw);
-      tmem_st32(t2_tmem, dw);
+      // kCols / 2 packed columns each
+      if constexpr (kCols == 64) {
+        if (!kDQ) tmem_st32(t1_tmem, pw);
+        tmem_st32(t2_tmem, dw);
+      } else {
+        if (!kDQ) tmem_st16(t1_tmem, pw);
+        tmem_st16(t2_tmem, dw);
+      }
       tmem_wait_st();
       tc_fence_before();
       __syncwarp();
@@ -461,8 +469,7 @@ cudaError_t map4d(CUtensorMap* m, const void* base, const AttnBwdArgs& a, uint32
 template <int D>
 cudaError_t launch(const AttnBwdArgs& a, cudaStream_t stream) {
   const int heads = a.P * a.h_c;
-  const int n_iter = static_cast<int>((a.S + kCols - 1) / kCols);
-  const int s_pad = n_iter * kCols;
+  const int s_pad = static_cast<int>((a.S + kPad - 1) / kPad * kPad);
   float2* stats = static_cast<float2*>(a.stats);
   {
     constexpr int kRowsPerBlock = 256 / (D / 8);
@@ -475,7 +482,6 @@ cudaError_t launch(const AttnBwdArgs& a, cudaStream_t stream) {
   }
   BwdParams prm;
   prm.S = static_cast<int>(a.S);
-  prm.n_iter = n_iter;
   prm.h_c = a.h_c;
   prm.s_pad = s_pad;
   prm.scale = a.scale;
@@ -484,22 +490,25 @@ cudaError_t launch(const AttnBwdArgs& a, cudaStream_t stream) {
   const dim3 grid(static_cast<unsigned>((a.S + kRows - 1) / kRows), static_cast<unsigned>(heads));
   cudaError_t e;
   BwdMaps kv;   // dK/dV pass: R = K, V; streamed Q, dO; out dV, dK
+  constexpr int kColsKV = Cfg<D, false>::kCols, kColsQ = Cfg<D, true>::kCols;
   if ((e = map4d(&kv.r1, a.k, a, kRows)) != cudaSuccess) return e;
   if ((e = map4d(&kv.r2, a.v, a, kRows)) != cudaSuccess) return e;
-  if ((e = map4d(&kv.x, a.q, a, kCols)) != cudaSuccess) return e;
-  if ((e = map4d(&kv.y, a.d_o, a, kCols)) != cudaSuccess) return e;
+  if ((e = map4d(&kv.x, a.q, a, kColsKV)) != cudaSuccess) return e;
+  if ((e = map4d(&kv.y, a.d_o, a, kColsKV)) != cudaSuccess) return e;
   if ((e = map4d(&kv.out1, a.dv, a, kRows)) != cudaSuccess) return e;
   if ((e = map4d(&kv.out2, a.dk, a, kRows)) != cudaSuccess) return e;
-  attention_bwd_kernel<D, false><<<grid, kThreads, Cfg<D>::kSmemBytes, stream>>>(kv, prm);
+  prm.n_iter = s_pad / kColsKV;
+  attention_bwd_kernel<D, false><<<grid, kThreads, Cfg<D, false>::kSmemBytes, stream>>>(kv, prm);
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
   BwdMaps qm;   // dQ pass: R = Q, dO; streamed K, V; out dQ
   if ((e = map4d(&qm.r1, a.q, a, kRows)) != cudaSuccess) return e;
   if ((e = map4d(&qm.r2, a.d_o, a, kRows)) != cudaSuccess) return e;
-  if ((e = map4d(&qm.x, a.k, a, kCols)) != cudaSuccess) return e;
-  if ((e = map4d(&qm.y, a.v, a, kCols)) != cudaSuccess) return e;
+  if ((e = map4d(&qm.x, a.k, a, kColsQ)) != cudaSuccess) return e;
+  if ((e = map4d(&qm.y, a.v, a, kColsQ)) != cudaSuccess) return e;
   if ((e = map4d(&qm.out1, a.dq, a, kRows)) != cudaSuccess) return e;
   qm.out2 = qm.out1;
-  attention_bwd_kernel<D, true><<<grid, kThreads, Cfg<D>::kSmemBytes, stream>>>(qm, prm);
+  prm.n_iter = s_pad / kColsQ;
+  attention_bwd_kernel<D, true><<<grid, kThreads, Cfg<D, true>::kSmemBytes, stream>>>(qm, prm);
   return cudaGetLastError();
 }
 
@@ -509,10 +518,10 @@ static cudaError_t bwd_set_attributes() {
   cudaError_t e;
 #define HCMS_SET(fn, bytes) \
   if ((e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes)) != cudaSuccess) return e;
-  HCMS_SET((attention_bwd_kernel<128, false>), Cfg<128>::kSmemBytes)
-  HCMS_SET((attention_bwd_kernel<128, true>), Cfg<128>::kSmemBytes)
-  HCMS_SET((attention_bwd_kernel<64, false>), Cfg<64>::kSmemBytes)
-  HCMS_SET((attention_bwd_kernel<64, true>), Cfg<64>::kSmemBytes)
+  HCMS_SET((attention_bwd_kernel<128, false>), (Cfg<128, false>::kSmemBytes))
+  HCMS_SET((attention_bwd_kernel<128, true>), (Cfg<128, true>::kSmemBytes))
+  HCMS_SET((attention_bwd_kernel<64, false>), (Cfg<64, false>::kSmemBytes))
+  HCMS_SET((attention_bwd_kernel<64, true>), (Cfg<64, true>::kSmemBytes))
 #undef HCMS_SET
   return cudaSuccess;
 }
@@ -523,7 +532,7 @@ cudaError_t attention_bwd_init() {
 }
 
 size_t attention_bwd_stats_bytes(int64_t S, int heads) {
-  const int64_t s_pad = (S + kCols - 1) / kCols * kCols;
+  const int64_t s_pad = (S + kPad - 1) / kPad * kPad;
   return static_cast<size_t>(heads) * s_pad * sizeof(float2);
 }
 

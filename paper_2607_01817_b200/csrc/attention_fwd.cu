@@ -45,6 +45,7 @@ namespace {
 constexpr int kBM = 128;          // query rows per tile (UMMA M)
 constexpr int kBN = 128;          // keys per KV tile (UMMA N of QK^T, K extent of PV)
 constexpr int kQTiles = 2;        // Q tiles per CTA
+constexpr int kThreads = 384;
 constexpr int kTmemCols = 512;
 constexpr float kRescaleThreshold = 8.0f;  // log2 units: rescale O only if the max grew by > 2^8
 constexpr int kPanelBytes = 128 * 128;     // one 128-byte-swizzle panel: 128 rows x 128 B
@@ -54,21 +55,14 @@ constexpr int kPTileBytes = 2 * kPanelBytes;  // P_t: 128 rows x 128 keys bf16
 // each loads HALF of it (64 of the 128 keys of K_j; 64 of the 128 head-dim columns of V_j) and the leader CTA issues
 // M = 256 MMAs over both CTAs' query tiles, so per CTA the K/V traffic into and out of shared memory and the number
 // of MMA instructions are halved.
-// kSplit (pair kernel only): TWO threads per query row -- 16 softmax warps instead of 8, each thread owning 64 of the
-// tile's 128 keys (and D/2 of the row's O columns for the rare rescale and the epilogue).  The two warps that share 32
-// rows exchange their half-row maxima (and, once, their half-row sums) through shared memory around a 64-thread named
-// barrier.  Four softmax warps per scheduler hide the dependent-issue latency that two cannot.
-template <int D, bool kPair = false, bool kSplit = false>
+template <int D, bool kPair = false>
 struct Cfg {
   static constexpr int kPanels = D / 64;                    // 128-byte swizzle panels along D
   static constexpr int kTileBytes = kPanels * kPanelBytes;  // one Q / K / V tile
   static constexpr int kKvBytes = kPair ? kTileBytes / 2 : kTileBytes;   // what one ring stage holds
-  static constexpr int kStages = D == 128 ? (kPair ? (kSplit ? 5 : 6) : 3) : 6;   // KV ring stages (one K or one V (half) tile each)
-  static constexpr int kXchgBytes = kSplit ? 2 * kQTiles * 2 * kBM * 4 : 0;        // [slot][tile][half][row] fp32
-  static constexpr int kThreads = kSplit ? 640 : 384;
-  static constexpr int kSoftmaxWarpsPerTile = kSplit ? 8 : 4;
+  static constexpr int kStages = D == 128 ? (kPair ? 6 : 3) : 6;          // KV ring stages (one K or one V (half) tile each)
   static constexpr int kSmemBytes =
-      kQTiles * kTileBytes + kQTiles * kPTileBytes + kStages * kKvBytes + kXchgBytes + 1024 /*align*/ + 256 /*barriers*/;
+      kQTiles * kTileBytes + kQTiles * kPTileBytes + kStages * kKvBytes + 1024 /*align*/ + 256 /*barriers*/;
   static constexpr int kTmemS = 0;                          // S_t at kTmemS + t*128
   static constexpr int kTmemO = 256;                        // O_t at kTmemO + t*D
 };
@@ -178,28 +172,17 @@ __device__ __forceinline__ void st_shared_v4(uint32_t addr, uint32_t a, uint32_t
 }
 
 // kPoly: of every 8 consecutive column pairs, this many take the polynomial path (the rest MUFU).
-__device__ __forceinline__ void st_shared_f32(uint32_t addr, float v) {
-  asm volatile("st.shared.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory");
-}
-__device__ __forceinline__ float ld_shared_f32(uint32_t addr) {
-  float v;
-  asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr) : "memory");
-  return v;
-}
-
-template <int D, int kPoly, bool kPair, bool kSplit = false>
-__global__ void __launch_bounds__((Cfg<D, kPair, kSplit>::kThreads), 1)
+template <int D, int kPoly, bool kPair>
+__global__ void __launch_bounds__(kThreads, 1)
 attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm) {
-  static_assert(!kSplit || kPair, "the two-threads-per-row softmax is built for the CTA-pair kernel");
-  using C = Cfg<D, kPair, kSplit>;
+  using C = Cfg<D, kPair>;
   constexpr int kStages = C::kStages;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t q_smem = smem_base;                                  // kQTiles Q tiles
   const uint32_t p_smem = q_smem + kQTiles * C::kTileBytes;           // kQTiles P tiles
   const uint32_t kv_smem = p_smem + kQTiles * kPTileBytes;            // kStages K/V tiles
-  const uint32_t xchg_smem = kv_smem + kStages * C::kKvBytes;         // kSplit: half-row max / sum exchange
-  const uint32_t bar_base = xchg_smem + C::kXchgBytes;                // 8-byte barriers
+  const uint32_t bar_base = kv_smem + kStages * C::kKvBytes;          // 8-byte barriers
   const uint32_t bar_q_full = bar_base;                       // [2]  TMA -> MMA
   const uint32_t bar_kv_full = bar_q_full + 16;               // [kStages] TMA -> MMA
   const uint32_t bar_kv_empty = bar_kv_full + 8 * kStages;    // [kStages] MMA -> TMA
@@ -222,8 +205,8 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
     for (int t = 0; t < kQTiles; ++t) {
       mbar_init(bar_q_full + 8 * t, 1);
       mbar_init(bar_s_full + 8 * t, 1);
-      mbar_init(bar_s_free + 8 * t, (kPair ? 2 : 1) * C::kSoftmaxWarpsPerTile);   // one elected lane per softmax warp (of both CTAs of a pair)
-      mbar_init(bar_p_full + 8 * t, (kPair ? 2 : 1) * C::kSoftmaxWarpsPerTile);
+      mbar_init(bar_s_free + 8 * t, kPair ? 8 : 4);     // one elected lane per softmax warp (of both CTAs of a pair)
+      mbar_init(bar_p_full + 8 * t, kPair ? 8 : 4);
       mbar_init(bar_pv_done + 8 * t, 1);
     }
     for (int s = 0; s < kStages; ++s) {
@@ -412,159 +395,6 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
       }
     }
     __syncwarp();
-  } else if constexpr (kSplit) {
-    // ================================ softmax, two threads per query row ================================
-    // register pool of the CTA = 640 threads x 96 (the launch allocation): 16 softmax warps x 104 + 4 other warps x 56
-    // = 60 416 <= 61 440.  (112 would need more than the CTA owns: setmaxnreg.inc then waits forever.)
-    setmaxnreg_inc<104>();
-    const int sw = warp - 4;                             // 0..15
-    const int q4 = sw & 3;                               // TMEM lane quarter (== warp % 4)
-    const int h = (sw >> 2) & 1;                         // which 64 keys of the tile / which D/2 columns of O
-    const int t = sw >> 3;                               // Q tile
-    const int row = q4 * 32 + lane;
-    const uint32_t lane_addr = static_cast<uint32_t>(q4 * 32) << 16;
-    const uint32_t s_tmem = tmem_base + lane_addr + C::kTmemS + t * kBN + h * 64;
-    const uint32_t o_tmem = tmem_base + lane_addr + C::kTmemO + t * D + h * (D / 2);
-    const uint32_t p_row = p_smem + t * kPTileBytes + h * kPanelBytes + row * 128;   // keys [64h, 64h+64) = panel h
-    const uint32_t swz = static_cast<uint32_t>(row & 7);
-    constexpr uint32_t kSlot = kQTiles * 2 * kBM * 4;
-    const uint32_t x_mine = xchg_smem + ((t * 2 + h) * kBM + row) * 4;
-    const uint32_t x_other = xchg_smem + ((t * 2 + (h ^ 1)) * kBM + row) * 4;
-    const int pair_bar = 3 + t * 4 + q4;                 // named barrier of the two warps that share these 32 rows
-    const float scale_log2 = prm.scale_log2;
-    const uint64_t scale2 = pack2(scale_log2, scale_log2);
-    const int tail_valid = prm.S - (n_kv - 1) * kBN - h * 64;   // valid keys of this half in the last KV tile (may be <= 0)
-    const PolyConsts pc = poly_consts();
-    constexpr int kHalf = kBN / 2;
-
-    float m_run = -INFINITY;
-    uint64_t l2 = pack2(0.f, 0.f), l2b = pack2(0.f, 0.f);
-
-    for (int j = 0; j < n_kv; ++j) {
-      mbar_wait(bar_s_full + 8 * t, j & 1);
-      tc_fence_after();
-      uint32_t sr[kHalf];
-      tmem_ld32(s_tmem, &sr[0]);
-      tmem_ld32(s_tmem + 32, &sr[32]);
-      tmem_wait_ld();
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive_cluster_relaxed(mapa(bar_s_free + 8 * t, 0));   // QK_t(j+1) may overwrite this half now
-      if (j == n_kv - 1 && tail_valid < kHalf) {
-#pragma unroll
-        for (int c = 0; c < kHalf; ++c)
-          if (c >= tail_valid) sr[c] = 0xff800000u;
-      }
-      float mx0 = __uint_as_float(sr[0]), mx1 = __uint_as_float(sr[1]);
-#pragma unroll
-      for (int c = 2; c < kHalf - 2; c += 4) {
-        mx0 = max3(mx0, __uint_as_float(sr[c]), __uint_as_float(sr[c + 1]));
-        mx1 = max3(mx1, __uint_as_float(sr[c + 2]), __uint_as_float(sr[c + 3]));
-      }
-      const float m_half = max3(mx0, mx1, fmaxf(__uint_as_float(sr[kHalf - 2]), __uint_as_float(sr[kHalf - 1])));
-      // the row max of the tile: exchange with the thread that holds the row's other 64 keys (alternating slots, so that
-      // iteration j+1's write cannot overtake a partner still reading iteration j's)
-      st_shared_f32(x_mine + (j & 1) * kSlot, m_half);
-      named_bar_sync(pair_bar, 64);
-      const float m_tile = fmaxf(m_half, ld_shared_f32(x_other + (j & 1) * kSlot));
-      if (j > 0) {
-        const bool need = (m_tile - m_run) * scale_log2 > kRescaleThreshold;   // identical in both threads of a row
-        if (__any_sync(0xffffffffu, need)) {
-          mbar_wait(bar_pv_done + 8 * t, (j - 1) & 1);
-          tc_fence_after();
-          const float alpha = need ? ex2((m_run - m_tile) * scale_log2) : 1.0f;
-          if (need) {
-            l2 = fma2(l2, pack2(alpha, alpha), pack2(0.f, 0.f));
-            l2b = fma2(l2b, pack2(alpha, alpha), pack2(0.f, 0.f));
-            m_run = m_tile;
-          }
-#pragma unroll 1
-          for (int c8 = 0; c8 < D / 16; ++c8) {          // this thread's D/2 columns of O_t, 8 at a time (rare path:
-            uint32_t orr[8];                             // it must not take registers from the 64 live scores)
-            tmem_ld8(o_tmem + c8 * 8, orr);
-            tmem_wait_ld();
-#pragma unroll
-            for (int c = 0; c < 8; ++c) orr[c] = __float_as_uint(__uint_as_float(orr[c]) * alpha);
-            tmem_st8(o_tmem + c8 * 8, orr);
-          }
-          tmem_wait_st();
-          tc_fence_before();
-        }
-      } else {
-        m_run = m_tile;
-      }
-      const float neg_m = -m_run * scale_log2;
-      const uint64_t neg_m2 = pack2(neg_m, neg_m);
-      // P_t's buffer may be rewritten once PV_t(j-1) has completed; with four softmax warps per scheduler the wait is
-      // hidden by the other warps, so nothing is held back in registers (the unsplit kernel holds half a tile)
-      if (j > 0) mbar_wait(bar_pv_done + 8 * t, (j - 1) & 1);
-#pragma unroll
-      for (int ch = 0; ch < kHalf / 8; ++ch) {
-        uint32_t w[4];
-#pragma unroll
-        for (int pr = 0; pr < 4; ++pr) {
-          const int c = ch * 8 + pr * 2;
-          const int pair = ch * 4 + pr;
-          const uint64_t x = fma2(pack2(__uint_as_float(sr[c]), __uint_as_float(sr[c + 1])), scale2, neg_m2);
-          float x0, x1;
-          unpack2(x, x0, x1);
-          const uint64_t p = (pair & 7) < kPoly ? exp2_poly2(x0, x1, pc) : pack2(ex2(x0), ex2(x1));
-          if (pr & 1) l2b = add2(l2b, p); else l2 = add2(l2, p);
-          float p0, p1;
-          unpack2(p, p0, p1);
-          w[pr] = pack_bf16(p0, p1);
-        }
-        st_shared_v4(p_row + ((ch ^ swz) << 4), w[0], w[1], w[2], w[3]);
-      }
-      fence_proxy_async_smem();
-      __syncwarp();
-      if (lane == 0) mbar_arrive_cluster_relaxed(mapa(bar_p_full + 8 * t, 0));
-    }
-
-    // ---------------- epilogue: O_t / l -> bf16 -> swizzled smem (P_t's buffer) -> TMA store ----------------
-    mbar_wait(bar_pv_done + 8 * t, (n_kv - 1) & 1);
-    tc_fence_after();
-    float la, lb, lc, ld;
-    unpack2(l2, la, lb);
-    unpack2(l2b, lc, ld);
-    const float l_half = (la + lb) + (lc + ld);
-    st_shared_f32(x_mine + (n_kv & 1) * kSlot, l_half);
-    named_bar_sync(pair_bar, 64);
-    const float l_sum = l_half + ld_shared_f32(x_other + (n_kv & 1) * kSlot);   // a + b == b + a: the same in both threads
-    const float inv_l = 1.0f / l_sum;
-    if (h == 0 && prm.lse != nullptr && q_row0 + t * kBM + row < prm.S)
-      prm.lse[static_cast<size_t>(head) * prm.S + q_row0 + t * kBM + row] =
-          (m_run * scale_log2 + log2f(l_sum)) * 0.6931471805599453f;
-    const uint32_t o_smem = p_smem + t * kPTileBytes;     // PV_t(n_kv-1) has finished reading it
-#pragma unroll
-    for (int c4 = 0; c4 < D / 64; ++c4) {
-      uint32_t orr[32];
-      tmem_ld32(o_tmem + c4 * 32, orr);
-      tmem_wait_ld();
-      const int col0 = h * (D / 2) + c4 * 32;             // first of these 32 columns of O_t
-      const uint32_t panel = col0 >> 6;
-#pragma unroll
-      for (int q4i = 0; q4i < 4; ++q4i) {
-        uint32_t w[4];
-#pragma unroll
-        for (int e = 0; e < 4; ++e)
-          w[e] = pack_bf16(__uint_as_float(orr[q4i * 8 + 2 * e]) * inv_l, __uint_as_float(orr[q4i * 8 + 2 * e + 1]) * inv_l);
-        const uint32_t chunk = ((col0 & 63) >> 3) + q4i;
-        st_shared_v4(o_smem + panel * kPanelBytes + row * 128 + ((chunk ^ swz) << 4), w[0], w[1], w[2], w[3]);
-      }
-    }
-    fence_proxy_async_smem();
-    named_bar_sync(1 + t, 2 * kBM);
-    if (q4 == 0 && h == 0 && lane == 0) {
-      const int row0 = q_row0 + t * kBM;
-      if (row0 < prm.S) {
-#pragma unroll
-        for (int pn = 0; pn < C::kPanels; ++pn)
-          tma_store_4d(&maps.o, o_smem + pn * kPanelBytes, pn * 64, hj, row0, rank);
-        bulk_commit();
-        bulk_wait<0>();
-      }
-    }
   } else {
     // ================================ softmax warpgroups ================================
     setmaxnreg_inc<224>();
@@ -768,11 +598,8 @@ cudaError_t set_attributes() {
   e = cudaFuncSetAttribute(attention_fwd_kernel<64, kPolyPairs, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                            Cfg<64>::kSmemBytes);
   if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(attention_fwd_kernel<128, kPolyPairs, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                           Cfg<128, true>::kSmemBytes);
-  if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(attention_fwd_kernel<128, kPolyPairs, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                              Cfg<128, true, true>::kSmemBytes);
+  return cudaFuncSetAttribute(attention_fwd_kernel<128, kPolyPairs, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              Cfg<128, true>::kSmemBytes);
 }
 
 }  // namespace
@@ -802,8 +629,8 @@ cudaError_t launch_attention(const AttnArgs& a0, cudaStream_t stream) {
     // one CTA whose query rows do not exist (its loads are zero fill, its stores are skipped)
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((grid.x + 1) / 2 * 2, grid.y);
-    cfg.blockDim = dim3(a.split ? Cfg<128, true, true>::kThreads : Cfg<128, true>::kThreads);
-    cfg.dynamicSmemBytes = a.split ? Cfg<128, true, true>::kSmemBytes : Cfg<128, true>::kSmemBytes;
+    cfg.blockDim = dim3(kThreads);
+    cfg.dynamicSmemBytes = Cfg<128, true>::kSmemBytes;
     cfg.stream = stream;
     cudaLaunchAttribute attr{};
     attr.id = cudaLaunchAttributeClusterDimension;
@@ -812,13 +639,12 @@ cudaError_t launch_attention(const AttnArgs& a0, cudaStream_t stream) {
     attr.val.clusterDim.z = 1;
     cfg.attrs = &attr;
     cfg.numAttrs = 1;
-    if (a.split) return cudaLaunchKernelEx(&cfg, attention_fwd_kernel<128, kPolyPairs, true, true>, maps, prm);
     return cudaLaunchKernelEx(&cfg, attention_fwd_kernel<128, kPolyPairs, true>, maps, prm);
   }
   if (a.D == 128)
-    attention_fwd_kernel<128, kPolyPairs, false><<<grid, Cfg<128>::kThreads, Cfg<128>::kSmemBytes, stream>>>(maps, prm);
+    attention_fwd_kernel<128, kPolyPairs, false><<<grid, kThreads, Cfg<128>::kSmemBytes, stream>>>(maps, prm);
   else if (a.D == 64)
-    attention_fwd_kernel<64, kPolyPairs, false><<<grid, Cfg<64>::kThreads, Cfg<64>::kSmemBytes, stream>>>(maps, prm);
+    attention_fwd_kernel<64, kPolyPairs, false><<<grid, kThreads, Cfg<64>::kSmemBytes, stream>>>(maps, prm);
   else
     return cudaErrorInvalidValue;
   return cudaGetLastError();

@@ -131,8 +131,7 @@ int do_attention(hcms_plan_t* p, const void* qc, const void* kc, const void* vc,
   const Chunk& ck = p->chunks[c];
   AttnArgs a{qc, kc, vc, oc, p->sh.S, p->sh.D, p->sh.P, ck.h, scale};
   a.lse = lse;
-  a.pair = (p->flags & (HCMS_FLAG_ATTN_PAIR | HCMS_FLAG_ATTN_SPLIT)) != 0;
-  a.split = (p->flags & HCMS_FLAG_ATTN_SPLIT) != 0;
+  a.pair = (p->flags & HCMS_FLAG_ATTN_PAIR) != 0;
   a.cache = &p->tmaps;
   cudaError_t e = launch_attention(a, st);
   if (e != cudaSuccess) return fail_cuda(e, "attention launch");

@@ -116,8 +116,8 @@ int hcms_dist_plan(hcms_dist_plan_t** out, int64_t S, int H, int D, int P, int C
     return fail(HCMS_ERR_INVALID_ARG, "S=%lld H=%d D=%d P=%d C=%d must all be positive", static_cast<long long>(S), H, D, P, C);
   if (rank < 0 || rank >= P) return fail(HCMS_ERR_INVALID_ARG, "rank=%d outside [0,%d)", rank, P);
   if (dtype != HCMS_DTYPE_BF16) return fail(HCMS_ERR_UNSUPPORTED_DTYPE, "the distributed path is bf16 only");
-  if (flags & ~static_cast<uint32_t>(HCMS_FLAG_ATTN_PAIR | HCMS_FLAG_ATTN_SPLIT))
-    return fail(HCMS_ERR_INVALID_ARG, "hcms_dist_plan accepts HCMS_FLAG_ATTN_PAIR / HCMS_FLAG_ATTN_SPLIT only (flags=0x%x)", flags);
+  if (flags & ~static_cast<uint32_t>(HCMS_FLAG_ATTN_PAIR))
+    return fail(HCMS_ERR_INVALID_ARG, "hcms_dist_plan accepts HCMS_FLAG_ATTN_PAIR only (flags=0x%x)", flags);
   if (S % P) return fail(HCMS_ERR_UNSUPPORTED_SHAPE, "S=%lld is not divisible by P=%d", static_cast<long long>(S), P);
   if (H % P) return fail(HCMS_ERR_UNSUPPORTED_SHAPE, "H=%d is not divisible by P=%d", H, P);
   if (D != 64 && D != 128) return fail(HCMS_ERR_UNSUPPORTED_SHAPE, "D=%d: only head dimensions 64 and 128 are built", D);
@@ -371,8 +371,7 @@ int enqueue_phase(const RankCall& rc, int phase, float scale) {
       if (!wait_all(0, c, plan->s_comp)) break;
       AttnArgs a{plan->block + ck.off[0], plan->block + ck.off[1], plan->block + ck.off[2], plan->block + ck.off[3],
                  sh.S, sh.D, 1, ck.h, scale};
-      a.pair = (plan->flags & (HCMS_FLAG_ATTN_PAIR | HCMS_FLAG_ATTN_SPLIT)) != 0;
-      a.split = (plan->flags & HCMS_FLAG_ATTN_SPLIT) != 0;
+      a.pair = (plan->flags & HCMS_FLAG_ATTN_PAIR) != 0;
       a.cache = &plan->tmaps;
       plan->last_launches += 1;
       if (cuda(launch_attention(a, plan->s_comp), "attention launch")) signal(1, c, plan->s_comp);   // E_c^comp as a flag

@@ -97,7 +97,6 @@ struct AttnArgs {
   float scale;
   float* lse = nullptr;   // optional [P*h_c][S] fp32: log sum_k exp(scale q.k) per row (saved for the backward)
   bool pair = false;      // CTA-pair kernel (HCMS_FLAG_ATTN_PAIR; D = 128 only, ignored otherwise)
-  bool split = false;     // pair kernel with two softmax threads per query row (HCMS_FLAG_ATTN_SPLIT)
   TmapCache* cache = nullptr;
 };
 cudaError_t launch_attention(const AttnArgs& a, cudaStream_t stream);

@@ -323,52 +323,3 @@ def test_pair_kernel_cfg3_full_size_same_bits():
     for _ in range(2):
         b = run_forward(q, k, v, w.S, w.H, w.D, w.P, w.C, w.scale, flags=H.HCMS_FLAG_ATTN_PAIR)
         assert np.array_equal(a, b)
-
-
-# ---------------------------------------------------------------------------------------------
-# HCMS_FLAG_ATTN_SPLIT: the pair kernel with two softmax threads per query row
-# ---------------------------------------------------------------------------------------------
-
-@pytest.mark.parametrize("S,Hh,P,C", [(1024, 4, 2, 2), (777, 2, 1, 1), (2100, 6, 2, 3), (130, 1, 1, 1), (64, 2, 2, 1)])
-def test_split_kernel_matches_oracle_and_is_chunk_invariant(S, Hh, P, C):
-    """Each half-row thread sums its own 64 keys per tile, so the row sum is associated differently from the
-    one-thread-per-row kernels: parity is against the oracle (same gates), and the paper's invariance (Table 14) is
-    checked within the kernel: bitwise equal output for C = 1 / P = 1 and for the plan's (P, C)."""
-    D = 128
-    w = I.Workload("split", S, Hh, D, P, C, 62, "bf16", 1.0)
-    q, k, v = I.make_qkv(w)
-    got = run_forward(q, k, v, S, Hh, D, P, C, w.scale, flags=H.HCMS_FLAG_ATTN_SPLIT)
-    check(got, O.attention_full(q, k, v, w.scale), "split kernel")
-    base = run_forward(q, k, v, S, Hh, D, 1, 1, w.scale, flags=H.HCMS_FLAG_ATTN_SPLIT | H.HCMS_FLAG_SERIAL)
-    assert np.array_equal(got, base)
-
-
-def test_split_kernel_one_hot_and_uniform_v():
-    """The closed forms on the split kernel: one-hot rows bit-equal to the V row (targets in the ragged tail, i.e. in
-    ONE half of the last tile: the other half-row thread sees only masked keys), uniform V per head."""
-    S, Hh, D, P, C = 1144, 2, 128, 2, 1
-    w = I.Workload("onehot", S, Hh, D, P, C, 9, "bf16", 1.0)
-    _, k, v = I.make_qkv(w)
-    rng = np.random.default_rng(1)
-    pi = rng.permutation(S)
-    pi[:8] = S - 1 - np.arange(8)
-    pi[8:16] = 1024 + np.arange(8)                          # first half of the last tile (keys 1024..1087)
-    q = I.f32_to_bf16_bits(np.float32(64.0) * I.bf16_bits_to_f32(k)[pi])
-    got = run_forward(q, k, v, S, Hh, D, P, C, w.scale, flags=H.HCMS_FLAG_ATTN_SPLIT)
-    assert np.array_equal(got, v[pi])
-    q, k, _ = I.make_qkv(w)
-    c_h = I.f32_to_bf16_bits(np.float32([1.0 + 0.25 * h for h in range(Hh)]))
-    vu = np.broadcast_to(c_h[None, :, None], (S, Hh, D)).copy()
-    got = bf16_bits_to_f64(run_forward(q, k, vu, S, Hh, D, P, C, w.scale, flags=H.HCMS_FLAG_ATTN_SPLIT))
-    ref = bf16_bits_to_f64(c_h)[None, :, None]
-    assert (np.abs(got - ref) / ref).max() <= 2.0 ** -7
-
-
-def test_split_kernel_cfg3_full_size_sampled_rows():
-    w = I.workload(3)
-    q, k, v = I.make_qkv(w, threads=16)
-    got = run_forward(q, k, v, w.S, w.H, w.D, w.P, w.C, w.scale, flags=H.HCMS_FLAG_ATTN_SPLIT)
-    rows = O.sample_rows(w.S, w.P, n_random=32, seed=33)
-    check(got[rows], O.attention_sampled(q, k, v, w.scale, rows), "cfg3 split")
-    again = run_forward(q, k, v, w.S, w.H, w.D, w.P, 1, w.scale, flags=H.HCMS_FLAG_ATTN_SPLIT)
-    assert np.array_equal(got, again)                       # C = 4 vs C = 1, full tensor, under NaN poisoning
