@@ -7,25 +7,33 @@
 //
 // One CTA = one head x 256 query rows (two 128-row Q tiles), 384 threads:
 //   warp 0      TMA producer: Q tiles once, then K/V tiles through a shared-memory ring, in the order the
-//               tensor core consumes them (K_0, K_1, V_0, K_2, V_1, ...)
-//   warp 1      MMA issuer (one lane): S_t = Q_t K_j^T (SS, M=128, N=128) and O_t += P_t V_j (SS: P_t is read
-//               from SHARED memory, V_j MN-major)
-//   warp 2      TMEM allocator (512 columns: S_0, S_1 at 0/128, O_0, O_1 at 256/256+D)
+//               tensor core first touches them (K_0, K_1, V_0, K_2, V_1, ...)
+//   warp 1      MMA issuer (one lane): S_t = Q_t K_n^T (SS, M=128, N=128) and O_t += P_t V_n (TS: P_t is the A operand
+//               in TENSOR memory, V_n MN-major in shared memory)
+//   warp 2      TMEM allocator (512 columns: S at 0, P_0 / P_1 at 128 / 192, O_0 / O_1 at 256 / 256+D)
 //   warps 4-7   softmax warpgroup of tile 0: one thread per query row; online softmax in fp32 with lazy
 //   warps 8-11  softmax warpgroup of tile 1   rescaling of O (only when the row max grew by > 2^8); epilogue
 //
-// Pipeline.  P_t goes through shared memory, not TMEM, so that S_t's TMEM columns are free as soon as the
-// softmax warpgroup has pulled S_t(j) into registers: the MMA warp issues QK_t(j+1) right then, and PV_t(j)
-// when P_t(j) has been stored.  The softmax chain (S(j) -> P(j) -> S(j+1) ...) therefore never waits for a
-// tensor-core round trip, and the tensor queue always holds the next GEMM (measured: the QK/PV instruction
-// mix runs at the full 8192 flop/clk/SM with P in shared memory, with or without concurrent P stores).
+// Why P lives in tensor memory.  With P staged in shared memory (round 1) the kernel sat at 98 % of the shared-memory
+// data pipe (ncu: tensor-core operand reads 77 % + P stores 21 % of l1tex__data_pipe_*_wavefronts_mem_shared), i.e. 1280
+// wavefronts per 1024 tensor-pipe cycles of every (Q tile, KV tile) pair: tensor activity could not exceed 80 %, and it
+// measured 77-81 %.  As a TMEM A operand P costs neither the 32 KB store nor the 32 KB operand read: 768 wavefronts.
+// TMEM has 512 columns and O_0, O_1 take 256 (D = 128), so the two P tiles (64 columns each, bf16 pairs) fit only if
+// the two Q tiles SHARE one 128-column score buffer S.  They can, because a softmax warpgroup pulls S into registers
+// within ~150 cycles and the tensor pipe runs a PV in between: the issue order per KV tile n is
+//     QK_0(n) -> S     PV_1(n-2)     QK_1(n) -> S     PV_0(n-1)
+// so that (a) the PV between two QKs covers the time the previous owner needs to empty S, and (b) every softmax has
+// three MMA slots plus a whole iteration (~3000 cycles) between its scores and the PV that consumes its P.  P_t(n) is
+// kept in registers until PV_t(n-1) has completed (pv_done), then written with two tcgen05.st.  V_m is used by PV_0(m)
+// in iteration m+1 and PV_1(m) in iteration m+2, so K_n, V_{n-2}, V_{n-1} are live while K_{n+1}, V_n load: the ring has 5
+// stages at D = 128 (the shared memory P used to take).
 // Pair variant: the softmax warps of the peer CTA signal the leader's barriers with RELAXED cluster-scope arrives.  A
 // release.cluster arrive costs a cluster-wide fence per warp and iteration (measured: 20.7 ms instead of 16.4 ms at
-// BASELINE config 3).  What the leader's MMAs read after the arrive is (a) S columns already pulled out of TMEM,
-// ordered by tcgen05.wait::ld + tcgen05.fence::before_thread_sync, and (b) the P tile in the arriving CTA's own
-// shared memory, which every lane has pushed through fence.proxy.async before the __syncwarp that precedes the
-// arrive; the leader waits with acquire.cluster.  tests/test_gpu_attention.py compares the pair kernel bit for bit
-// with the single-CTA kernel at full size under NaN poisoning.
+// BASELINE config 3).  What the leader's MMAs touch after the arrive is tensor memory of the arriving CTA (S columns
+// already pulled out, ordered by tcgen05.wait::ld; P columns written, ordered by tcgen05.wait::st) followed by
+// tcgen05.fence::before_thread_sync and the __syncwarp that precedes the arrive; the leader waits with acquire.cluster.
+// tests/test_gpu_attention.py compares the pair kernel bit for bit with the single-CTA kernel at full size under NaN
+// poisoning.
 // The exponentials are split between the MUFU pipe (ex2.approx) and a degree-3 polynomial on the FMA pipe
 // (packed f32x2 arithmetic), since 16 ex2/clk/SM would otherwise co-limit the kernel at exactly the MMA time.
 //
@@ -49,10 +57,10 @@ constexpr int kThreads = 384;
 constexpr int kTmemCols = 512;
 constexpr float kRescaleThreshold = 8.0f;  // log2 units: rescale O only if the max grew by > 2^8
 constexpr int kPanelBytes = 128 * 128;     // one 128-byte-swizzle panel: 128 rows x 128 B
-constexpr int kPTileBytes = 2 * kPanelBytes;  // P_t: 128 rows x 128 keys bf16
+constexpr int kPCols = kBN / 2;            // P_t in TMEM: 128 keys as bf16 pairs
 
-// kPair: the CTA-pair variant (tcgen05 cta_group::2, D = 128 only).  Two CTAs of a cluster share every K_j / V_j tile:
-// each loads HALF of it (64 of the 128 keys of K_j; 64 of the 128 head-dim columns of V_j) and the leader CTA issues
+// kPair: the CTA-pair variant (tcgen05 cta_group::2, D = 128 only).  Two CTAs of a cluster share every K_n / V_n tile:
+// each loads HALF of it (64 of the 128 keys of K_n; 64 of the 128 head-dim columns of V_n) and the leader CTA issues
 // M = 256 MMAs over both CTAs' query tiles, so per CTA the K/V traffic into and out of shared memory and the number
 // of MMA instructions are halved.
 template <int D, bool kPair = false>
@@ -60,11 +68,12 @@ struct Cfg {
   static constexpr int kPanels = D / 64;                    // 128-byte swizzle panels along D
   static constexpr int kTileBytes = kPanels * kPanelBytes;  // one Q / K / V tile
   static constexpr int kKvBytes = kPair ? kTileBytes / 2 : kTileBytes;   // what one ring stage holds
-  static constexpr int kStages = D == 128 ? (kPair ? 6 : 3) : 6;          // KV ring stages (one K or one V (half) tile each)
-  static constexpr int kSmemBytes =
-      kQTiles * kTileBytes + kQTiles * kPTileBytes + kStages * kKvBytes + 1024 /*align*/ + 256 /*barriers*/;
-  static constexpr int kTmemS = 0;                          // S_t at kTmemS + t*128
+  static constexpr int kStages = D == 128 ? (kPair ? 10 : 5) : 8;         // KV ring stages (one K or one V (half) tile each)
+  static constexpr int kSmemBytes = kQTiles * kTileBytes + kStages * kKvBytes + 1024 /*align*/ + 256 /*barriers*/;
+  static constexpr int kTmemS = 0;                          // the score buffer both Q tiles take turns in
+  static constexpr int kTmemP = kBN;                        // P_t at kTmemP + t*64
   static constexpr int kTmemO = 256;                        // O_t at kTmemO + t*D
+  static_assert(kSmemBytes <= 227 * 1024, "shared memory budget");
 };
 
 // Shared-memory matrix descriptor, 128-byte swizzle (cute::UMMA::SmemDescriptor bit layout):
@@ -180,16 +189,15 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t q_smem = smem_base;                                  // kQTiles Q tiles
-  const uint32_t p_smem = q_smem + kQTiles * C::kTileBytes;           // kQTiles P tiles
-  const uint32_t kv_smem = p_smem + kQTiles * kPTileBytes;            // kStages K/V tiles
+  const uint32_t kv_smem = q_smem + kQTiles * C::kTileBytes;          // kStages K/V tiles
   const uint32_t bar_base = kv_smem + kStages * C::kKvBytes;          // 8-byte barriers
   const uint32_t bar_q_full = bar_base;                       // [2]  TMA -> MMA
   const uint32_t bar_kv_full = bar_q_full + 16;               // [kStages] TMA -> MMA
   const uint32_t bar_kv_empty = bar_kv_full + 8 * kStages;    // [kStages] MMA -> TMA
-  const uint32_t bar_s_full = bar_kv_empty + 8 * kStages;     // [2]  MMA -> softmax: S_t(j) is in TMEM
-  const uint32_t bar_s_free = bar_s_full + 16;                // [2]  softmax -> MMA: S_t(j) is in registers
-  const uint32_t bar_p_full = bar_s_free + 16;                // [2]  softmax -> MMA: P_t(j) is in shared memory
-  const uint32_t bar_pv_done = bar_p_full + 16;               // [2]  MMA -> softmax: PV_t(j) has completed
+  const uint32_t bar_s_full = bar_kv_empty + 8 * kStages;     // [2]  MMA -> softmax: S_t(n) is in the score buffer
+  const uint32_t bar_s_free = bar_s_full + 16;                // [2]  softmax -> MMA: S_t(n) is in registers, the buffer is free
+  const uint32_t bar_p_full = bar_s_free + 16;                // [2]  softmax -> MMA: P_t(n) is in TMEM (O_t rescaled if needed)
+  const uint32_t bar_pv_done = bar_p_full + 16;               // [2]  MMA -> softmax: PV_t(n) has completed
   const uint32_t tmem_slot = bar_pv_done + 16;                // 4 bytes
 
   const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);   // warp-uniform by construction
@@ -312,8 +320,8 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
       };
       constexpr uint32_t kKPanel = kPair ? kPanelBytes / 2 : kPanelBytes;   // a K panel holds 64 or 128 keys
       auto issue_qk = [&](int t, uint32_t k_tile) {
-        // S_t[128 x 128] = Q_t[128 x D] * K_j[128 x D]^T ; both operands K-major, 128B-swizzled panels
-        const uint32_t d_tmem = tmem_base + C::kTmemS + t * kBN;
+        // S[128 x 128] = Q_t[128 x D] * K_n[128 x D]^T ; both operands K-major, 128B-swizzled panels
+        const uint32_t d_tmem = tmem_base + C::kTmemS;
         const uint32_t q_lo = desc_lo(q_smem + t * C::kTileBytes, 16);
         const uint32_t k_lo = desc_lo(k_tile, 16);
 #pragma unroll
@@ -324,73 +332,82 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
         }
       };
       auto issue_pv = [&](int t, uint32_t v_tile, bool accumulate) {
-        // O_t[128 x D] += P_t[128 x 128 keys] * V_j[128 keys x D]; A = P_t K-major from shared memory (two
-        // 64-key panels), B = V_j MN-major: 64-wide D panels (LBO = panel stride), 8-key groups 1024 B apart
+        // O_t[128 x D] += P_t[128 x 128 keys] * V_n[128 keys x D]; A = P_t in TMEM (bf16 pairs: 8 columns per K step of
+        // 16 keys), B = V_n MN-major: 64-wide D panels (LBO = panel stride), 8-key groups 1024 B apart
         const uint32_t d_tmem = tmem_base + C::kTmemO + t * D;
-        const uint32_t p_lo = desc_lo(p_smem + t * kPTileBytes, 16);
+        const uint32_t a_tmem = tmem_base + C::kTmemP + t * kPCols;
         const uint32_t v_lo = desc_lo(v_tile, kPanelBytes);
 #pragma unroll
         for (int ks = 0; ks < kBN / 16; ++ks) {
-          const uint32_t off = ((ks >> 2) * kPanelBytes + (ks & 3) * 32) >> 4;
-          mma(d_tmem, p_lo + off, v_lo + ks * (2048 >> 4), idesc_pv, (accumulate || ks > 0) ? 1u : 0u);
+          const uint32_t acc = (accumulate || ks > 0) ? 1u : 0u;
+          if (kPair) mma_ts_lohi_2sm(d_tmem, a_tmem + ks * 8, v_lo + ks * (2048 >> 4), hi, idesc_pv, acc);
+          else mma_ts_lohi(d_tmem, a_tmem + ks * 8, v_lo + ks * (2048 >> 4), hi, idesc_pv, acc);
         }
       };
-      int stage = 0;
+      // The ring is a FIFO: tiles are first touched in load order (K_0, K_1, V_0, K_2, V_1, ...) and released in the same
+      // order (K_n after QK_1(n); V_m after PV_1(m), two iterations after its K), so acquire and release keep their own
+      // positions.
+      int stage = 0, rel_stage = 0;
       uint32_t phase = 0;
-      auto kv_wait = [&]() -> uint32_t {
+      auto kv_acquire = [&]() -> uint32_t {
         mbar_wait(bar_kv_full + 8 * stage, phase);
-        return kv_smem + stage * C::kKvBytes;
-      };
-      auto kv_release = [&]() {
-        if (leader) commit(bar_kv_empty + 8 * stage);
-        __syncwarp();
+        const uint32_t addr = kv_smem + stage * C::kKvBytes;
         if (++stage == kStages) {
           stage = 0;
           phase ^= 1;
         }
+        return addr;
+      };
+      auto kv_release = [&]() {       // the oldest tile still held: free once every MMA issued so far has completed
+        if (leader) commit(bar_kv_empty + 8 * rel_stage);
+        __syncwarp();
+        if (++rel_stage == kStages) rel_stage = 0;
+      };
+      auto qk_step = [&](int t, uint32_t k_tile) {
+        tc_fence_after();
+        if (leader) {
+          issue_qk(t, k_tile);
+          commit(bar_s_full + 8 * t);
+        }
+        __syncwarp();
+      };
+      auto pv_step = [&](int t, uint32_t v_tile, int m) {     // PV_t(m)
+        wait_softmax(bar_p_full + 8 * t, m & 1);                // P_t(m) is in TMEM, O_t rescaled if needed
+        tc_fence_after();
+        if (leader) {
+          issue_pv(t, v_tile, m > 0);
+          commit(bar_pv_done + 8 * t);
+        }
+        __syncwarp();
       };
 
-      // prologue: S_0(0), S_1(0)
-      {
-        const uint32_t k_tile = kv_wait();
-#pragma unroll
-        for (int t = 0; t < kQTiles; ++t) {
-          mbar_wait(bar_q_full + 8 * t, 0);
-          tc_fence_after();
-          if (leader) {
-            issue_qk(t, k_tile);
-            commit(bar_s_full + 8 * t);
-          }
-          __syncwarp();
+      mbar_wait(bar_q_full, 0);
+      mbar_wait(bar_q_full + 8, 0);
+      uint32_t v_prev = 0;                                      // V_{n-2} while iteration n runs: PV_1 still needs it
+      for (int n = 0; n < n_kv; ++n) {
+        const uint32_t k_tile = kv_acquire();
+        if (n >= 1) wait_softmax(bar_s_free + 8, (n - 1) & 1);  // S_1(n-1) has left the score buffer
+        qk_step(0, k_tile);
+        if (n >= 2) {
+          pv_step(1, v_prev, n - 2);
+          kv_release();                                         // V_{n-2}
         }
+        wait_softmax(bar_s_free, n & 1);                        // S_0(n) has left the score buffer
+        qk_step(1, k_tile);
+        kv_release();                                           // K_n
+        if (n >= 1) {
+          v_prev = kv_acquire();                                // V_{n-1}
+          pv_step(0, v_prev, n - 1);
+        }
+      }
+      if (n_kv >= 2) {
+        pv_step(1, v_prev, n_kv - 2);
         kv_release();
       }
-      for (int j = 0; j < n_kv; ++j) {
-        if (j + 1 < n_kv) {
-          const uint32_t k_tile = kv_wait();
-#pragma unroll
-          for (int t = 0; t < kQTiles; ++t) {
-            wait_softmax(bar_s_free + 8 * t, j & 1);  // S_t(j) sits in the softmax registers
-            tc_fence_after();
-            if (leader) {
-              issue_qk(t, k_tile);
-              commit(bar_s_full + 8 * t);
-            }
-            __syncwarp();
-          }
-          kv_release();
-        }
-        const uint32_t v_tile = kv_wait();
-#pragma unroll
-        for (int t = 0; t < kQTiles; ++t) {
-          wait_softmax(bar_p_full + 8 * t, j & 1);    // P_t(j) stored, O_t rescaled if needed
-          tc_fence_after();
-          if (leader) {
-            issue_pv(t, v_tile, j > 0);
-            commit(bar_pv_done + 8 * t);
-          }
-          __syncwarp();
-        }
+      {
+        const uint32_t v_tile = kv_acquire();                   // V_{n_kv-1}
+        pv_step(0, v_tile, n_kv - 1);
+        pv_step(1, v_tile, n_kv - 1);
         kv_release();
       }
     }
@@ -401,9 +418,9 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
     const int t = (warp >> 2) - 1;                       // Q tile of this warpgroup
     const int row = (warp & 3) * 32 + lane;              // row inside the tile == TMEM lane
     const uint32_t lane_addr = static_cast<uint32_t>((warp & 3) * 32) << 16;
-    const uint32_t s_tmem = tmem_base + lane_addr + C::kTmemS + t * kBN;
+    const uint32_t s_tmem = tmem_base + lane_addr + C::kTmemS;
+    const uint32_t p_tmem = tmem_base + lane_addr + C::kTmemP + t * kPCols;
     const uint32_t o_tmem = tmem_base + lane_addr + C::kTmemO + t * D;
-    const uint32_t p_row = p_smem + t * kPTileBytes + row * 128;   // + panel*kPanelBytes + ((chunk ^ (row&7)) << 4)
     const uint32_t swz = static_cast<uint32_t>(row & 7);
     const float scale_log2 = prm.scale_log2;
     const uint64_t scale2 = pack2(scale_log2, scale_log2);
@@ -422,7 +439,7 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
       tmem_wait_ld();
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) {                                   // QK_t(j+1) may overwrite S_t now
+      if (lane == 0) {                                   // the other tile's QK may overwrite the score buffer now
         if (kPair) mbar_arrive_cluster_relaxed(mapa(bar_s_free + 8 * t, 0)); else mbar_arrive(bar_s_free + 8 * t);
       }
       if (j == n_kv - 1 && tail_valid < kBN) {
@@ -454,14 +471,15 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
             l2b = fma2(l2b, pack2(alpha, alpha), pack2(0.f, 0.f));
             m_run = m_tile;
           }
-#pragma unroll
-          for (int c4 = 0; c4 < D / 32; ++c4) {
-            uint32_t orr[32];
-            tmem_ld32(o_tmem + c4 * 32, orr);
+          // 16 columns at a time: the 128 scores of the tile stay in registers beside them
+#pragma unroll 1
+          for (int c16 = 0; c16 < D / 16; ++c16) {
+            uint32_t orr[16];
+            tmem_ld16(o_tmem + c16 * 16, orr);
             tmem_wait_ld();
 #pragma unroll
-            for (int c = 0; c < 32; ++c) orr[c] = __float_as_uint(__uint_as_float(orr[c]) * alpha);
-            tmem_st32(o_tmem + c4 * 32, orr);
+            for (int c = 0; c < 16; ++c) orr[c] = __float_as_uint(__uint_as_float(orr[c]) * alpha);
+            tmem_st16(o_tmem + c16 * 16, orr);
           }
           tmem_wait_st();
           tc_fence_before();
@@ -471,49 +489,37 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
       }
       const float neg_m = -m_run * scale_log2;
       const uint64_t neg_m2 = pack2(neg_m, neg_m);
-      // 16 chunks of 8 keys: x = s*scale_log2 - m*scale_log2, p = 2^x, row sum in fp32, P rounded to bf16.
-      // The first kHold chunks stay in registers: P_t's buffer may only be rewritten once PV_t(j-1) has
-      // completed, and by the time they are done that wait has normally been satisfied already.
-      constexpr int kHold = 8;
-      uint32_t held[kHold][4];
+      // 64 key pairs: x = s*scale_log2 - m*scale_log2, p = 2^x, row sum in fp32, P rounded to bf16.  The packed tile
+      // (64 registers, taking the place of the scores as they die) waits in registers for PV_t(j-1) to finish with
+      // P_t's columns; by then that has normally happened (it was issued one to two iterations ago).
+      uint32_t pw[kPCols];
 #pragma unroll
-      for (int ch = 0; ch < kBN / 8; ++ch) {
-        uint32_t w[4];
-#pragma unroll
-        for (int pr = 0; pr < 4; ++pr) {
-          const int c = ch * 8 + pr * 2;
-          const int pair = ch * 4 + pr;                 // 0..63
-          const uint64_t x = fma2(pack2(__uint_as_float(sr[c]), __uint_as_float(sr[c + 1])), scale2, neg_m2);
-          float x0, x1;
-          unpack2(x, x0, x1);
-          const uint64_t p = (pair & 7) < kPoly ? exp2_poly2(x0, x1, pc) : pack2(ex2(x0), ex2(x1));
-          if (pr & 1) l2b = add2(l2b, p); else l2 = add2(l2, p);
-          float p0, p1;
-          unpack2(p, p0, p1);
-          w[pr] = pack_bf16(p0, p1);
-        }
-        if (ch < kHold) {
-#pragma unroll
-          for (int e = 0; e < 4; ++e) held[ch][e] = w[e];
-        }
-        if (ch == kHold - 1) {
-          if (j > 0) mbar_wait(bar_pv_done + 8 * t, (j - 1) & 1);
-#pragma unroll
-          for (int h = 0; h < kHold; ++h)
-            st_shared_v4(p_row + (h >> 3) * kPanelBytes + (((h & 7) ^ swz) << 4), held[h][0], held[h][1], held[h][2],
-                         held[h][3]);
-        }
-        if (ch >= kHold)
-          st_shared_v4(p_row + (ch >> 3) * kPanelBytes + (((ch & 7) ^ swz) << 4), w[0], w[1], w[2], w[3]);
+      for (int pair = 0; pair < kPCols; ++pair) {
+        const int c = pair * 2;
+        const uint64_t x = fma2(pack2(__uint_as_float(sr[c]), __uint_as_float(sr[c + 1])), scale2, neg_m2);
+        float x0, x1;
+        unpack2(x, x0, x1);
+        const uint64_t p = (pair & 7) < kPoly ? exp2_poly2(x0, x1, pc) : pack2(ex2(x0), ex2(x1));
+        if (pair & 1) l2b = add2(l2b, p); else l2 = add2(l2, p);
+        float p0, p1;
+        unpack2(p, p0, p1);
+        pw[pair] = pack_bf16(p0, p1);       // key 2*pair in the low half: column `pair` of the TMEM A operand
       }
-      fence_proxy_async_smem();     // generic-proxy stores -> visible to the tensor core's async-proxy reads
+      if (j > 0) {
+        mbar_wait(bar_pv_done + 8 * t, (j - 1) & 1);
+        tc_fence_after();
+      }
+      tmem_st32(p_tmem, pw);
+      tmem_st32(p_tmem + 32, pw + 32);
+      tmem_wait_st();
+      tc_fence_before();
       __syncwarp();
       if (lane == 0) {
         if (kPair) mbar_arrive_cluster_relaxed(mapa(bar_p_full + 8 * t, 0)); else mbar_arrive(bar_p_full + 8 * t);
       }
     }
 
-    // ---------------- epilogue: O_t / l -> bf16 -> swizzled smem (P_t's buffer) -> TMA store ----------------
+    // ---------------- epilogue: O_t / l -> bf16 -> swizzled smem (Q_t's tile: every QK_t has completed) -> TMA store ----------------
     mbar_wait(bar_pv_done + 8 * t, (n_kv - 1) & 1);
     tc_fence_after();
     float la, lb, lc, ld;
@@ -524,7 +530,7 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
     if (prm.lse != nullptr && q_row0 + t * kBM + row < prm.S)      // sum_k exp(s_k) = l * exp(m): lse = m*scale + log l
       prm.lse[static_cast<size_t>(head) * prm.S + q_row0 + t * kBM + row] =
           (m_run * scale_log2 + log2f(l_sum)) * 0.6931471805599453f;
-    const uint32_t o_smem = p_smem + t * kPTileBytes;     // PV_t(n_kv-1) has finished reading it
+    const uint32_t o_smem = q_smem + t * C::kTileBytes;
 #pragma unroll
     for (int c4 = 0; c4 < D / 32; ++c4) {
       uint32_t orr[32];

@@ -90,6 +90,11 @@ __device__ __forceinline__ void layout_vec_body(const LayoutVecParams& p, const 
     uint8_t* dense = tab->peer[z][rank];
     if (kGather) src = dense; else dst = dense;
   }
+  // Programmatic dependent launch: a layout kernel that directly follows another kernel in its stream may be placed on
+  // the SMs while that kernel drains (its blocks compute their addresses, then wait here until the predecessor has
+  // completed and its writes are visible).  One chunk's copy is a 30-90 us kernel, so the launch gap and the ramp that
+  // this hides are 5-8 % of it.  Without the launch attribute, or behind an event wait or a copy, both are no-ops.
+  asm volatile("griddepcontrol.launch_dependents;");
   const uint32_t i0 = blockIdx.x * (kVecThreads * kVecUnroll) + threadIdx.x;
   const size_t dense_base = kPeer ? 0 : static_cast<size_t>(rank) * p.n_per_rank;
   const size_t strided_base = static_cast<size_t>(rank) * p.rank_stride_vecs + p.chunk_off_vecs;
@@ -98,6 +103,7 @@ __device__ __forceinline__ void layout_vec_body(const LayoutVecParams& p, const 
 
   Vec val[kVecUnroll];
   size_t out_idx[kVecUnroll];
+  asm volatile("griddepcontrol.wait;" ::: "memory");
 #pragma unroll
   for (int u = 0; u < kVecUnroll; ++u) {
     const uint32_t i = i0 + u * kVecThreads;
@@ -168,32 +174,25 @@ cudaError_t launch_layout_vec(const LayoutArgs& a, cudaStream_t stream) {
   p.step_cols = kVecThreads % p.run_vecs;
   const uint32_t per_block = kVecThreads * kVecUnroll;
   dim3 grid((p.n_per_rank + per_block - 1) / per_block, a.P, a.n_tensors);
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = grid;
+  cfg.blockDim = dim3(kVecThreads);
+  cfg.stream = stream;
+  cudaLaunchAttribute attr{};
+  attr.id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr.val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = &attr;
+  cfg.numAttrs = 1;
   if (peer) {
-    if (a.gather) {
-      if (wide)
-        layout_vec_peer_kernel<true, Vec32><<<grid, kVecThreads, 0, stream>>>(p, tab);
-      else
-        layout_vec_peer_kernel<true, Vec16><<<grid, kVecThreads, 0, stream>>>(p, tab);
-    } else {
-      if (wide)
-        layout_vec_peer_kernel<false, Vec32><<<grid, kVecThreads, 0, stream>>>(p, tab);
-      else
-        layout_vec_peer_kernel<false, Vec16><<<grid, kVecThreads, 0, stream>>>(p, tab);
-    }
-    return cudaGetLastError();
+    if (a.gather)
+      return wide ? cudaLaunchKernelEx(&cfg, layout_vec_peer_kernel<true, Vec32>, p, tab)
+                  : cudaLaunchKernelEx(&cfg, layout_vec_peer_kernel<true, Vec16>, p, tab);
+    return wide ? cudaLaunchKernelEx(&cfg, layout_vec_peer_kernel<false, Vec32>, p, tab)
+                : cudaLaunchKernelEx(&cfg, layout_vec_peer_kernel<false, Vec16>, p, tab);
   }
-  if (a.gather) {
-    if (wide)
-      layout_vec_kernel<true, Vec32><<<grid, kVecThreads, 0, stream>>>(p);
-    else
-      layout_vec_kernel<true, Vec16><<<grid, kVecThreads, 0, stream>>>(p);
-  } else {
-    if (wide)
-      layout_vec_kernel<false, Vec32><<<grid, kVecThreads, 0, stream>>>(p);
-    else
-      layout_vec_kernel<false, Vec16><<<grid, kVecThreads, 0, stream>>>(p);
-  }
-  return cudaGetLastError();
+  if (a.gather)
+    return wide ? cudaLaunchKernelEx(&cfg, layout_vec_kernel<true, Vec32>, p) : cudaLaunchKernelEx(&cfg, layout_vec_kernel<true, Vec16>, p);
+  return wide ? cudaLaunchKernelEx(&cfg, layout_vec_kernel<false, Vec32>, p) : cudaLaunchKernelEx(&cfg, layout_vec_kernel<false, Vec16>, p);
 }
 
 // ------------------------------------------------------------------------------------------
