@@ -390,10 +390,39 @@ def run_dist(args, torch, H, rank, local, world, nccl):
     qd, kd, vd = (t.to(dev, non_blocking=True) for t in host)
     out = torch.empty_like(qd)
     torch.cuda.synchronize()
-    plan = H.hcms_dist_plan(S, Hh, D, P, C, rank)
-    H.hcms_dist_exchange_handles(plan)
     stream = torch.cuda.current_stream()
     flop_step = 4.0 * S * S * D * Hh                       # the whole layer, all ranks together
+    # Bring-up in three stages, each agreed on by ALL ranks (MIN over ranks of "it worked here"), so that a rank on
+    # which peer mapping is refused (no P2P between two devices, IPC disabled in a container) cannot leave the others
+    # waiting in a collective: if any stage fails anywhere, every rank falls back to independent replicas and says so.
+    plan, why = None, ""
+
+    def agreed(ok: bool) -> bool:
+        return max_over_ranks(0.0 if ok else 1.0, world, nccl) == 0.0
+    try:
+        plan = H.hcms_dist_plan(S, Hh, D, P, C, rank)
+    except Exception as e:  # noqa: BLE001
+        why = f"hcms_dist_plan: {e}"
+    ok = agreed(plan is not None)
+    if ok:
+        try:
+            H.hcms_dist_exchange_handles(plan)
+        except Exception as e:  # noqa: BLE001
+            why = f"hcms_dist_attach: {e}"
+        ok = agreed(not why)
+    if ok:
+        try:
+            H.hcms_dist_attention_forward(plan, qd, kd, vd, out, w.scale)
+            torch.cuda.synchronize()
+        except Exception as e:  # noqa: BLE001
+            why = f"hcms_dist_attention_forward: {e}"
+        ok = agreed(not why)
+    if not ok:
+        if why:
+            print(f"bench.py rank {rank}: {why}", file=sys.stderr, flush=True)
+        if plan is not None:
+            plan.close()
+        return "hcms_dist bring-up failed on at least one rank" + (f" ({why})" if why else "")
     step = lambda: H.hcms_dist_attention_forward(plan, qd, kd, vd, out, w.scale)
 
     def timed(steps, fn):
@@ -461,6 +490,7 @@ def run_dist(args, torch, H, rank, local, world, nccl):
         print(json.dumps(result), flush=True)
     barrier(world, True)
     dist.destroy_process_group()
+    return None
 
 
 def run_hcms(args):
@@ -477,8 +507,11 @@ def run_hcms(args):
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     pk = peaks()
+    dist_note = None
     if world > 1 and not args.replicas:
-        return run_dist(args, torch, H, rank, local, world, nccl)
+        dist_note = run_dist(args, torch, H, rank, local, world, nccl)
+        if dist_note is None:
+            return
 
     w = I.workload(args.config)
     C = args.chunks or w.C
@@ -577,7 +610,7 @@ def run_hcms(args):
                    "S": S, "H": Hh, "D": D, "P": P, "C": C, "layout_kernel": args.layout,
                    "compute_streams": 1 if args.single_comp else 2, "attention_kernel": "cta pair" if args.attn_pair else "single cta",
                    "l2": "flushed between steps" if flush else "inputs larger than L2 (3 x %d MB)" % (tensor_bytes >> 20),
-                   "multi_gpu": "replicas only" if world > 1 else "single GPU",
+                   "multi_gpu": ("replicas only" + (f": {dist_note}" if dist_note else "")) if world > 1 else "single GPU",
                    "inputs": "hcms_inputs counter-based N(0,1) -> bf16 (seed %d)" % w.seed},
         "clocks": clocks, "gpu_launches": launches,
         "roofline": {"kernel": "attention_fwd_kernel<%d>" % D, "bound": "tensor", "achieved": round(achieved, 1),

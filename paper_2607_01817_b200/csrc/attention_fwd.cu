@@ -594,7 +594,8 @@ cudaError_t make_maps(const AttnArgs& a, AttnMaps* m) {
                            CU_TENSOR_MAP_SWIZZLE_128B);
 }
 
-// Of every 8 column pairs, kPolyPairs take their exponential on the FMA pipe (tuned on B200: profiles/ poly sweep)
+// Of every 8 column pairs, kPolyPairs take their exponential on the FMA pipe (swept on B200 with this kernel, 40-step
+// sustained runs at cfg 3: 0 / 1 / 2 / 3 / 4 -> 16.79 / 16.75 / 16.52 / 16.91 / 17.36 ms; profiles/r2d_experiments.md)
 constexpr int kPolyPairs = 2;
 
 cudaError_t set_attributes() {

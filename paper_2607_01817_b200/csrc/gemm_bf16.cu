@@ -24,6 +24,7 @@
 #include "hcms_internal.h"
 #include "ptx.cuh"
 
+
 namespace hcms {
 using namespace ptx;
 
@@ -360,6 +361,9 @@ gemm_bf16_nt_2cta_kernel(const __grid_constant__ GemmMaps maps, const __grid_con
       prefetch_tensormap(&maps.a);
       prefetch_tensormap(&maps.b);
     }
+    // L2 policy (swept on B200, profiles/r2e_gemm_l2.md): operand tiles are re-read by the other clusters of the wave (B)
+    // and of the band (A), so both loads ask for evict_last; the output, written once, asks for evict_first below
+    const uint64_t pol_a = l2_policy_evict_last(), pol_b = pol_a;
     int stage = 0;
     uint32_t phase = 0;
     for (int tile = cluster_id; tile < total_tiles; tile += n_clusters) {
@@ -377,9 +381,9 @@ gemm_bf16_nt_2cta_kernel(const __grid_constant__ GemmMaps maps, const __grid_con
             const int head = (kb * kBK) >> prm.d_shift, hr = head / prm.Hl, lh = head - hr * prm.Hl;
             tma_load_4d_2sm(dst, &cmaps.m[prm.chunk_of[lh]], full0, (kb * kBK) & prm.d_mask, prm.j_of[lh], m0, hr);
           } else {
-            tma_load_2d_2sm(dst, &maps.a, full0, kb * kBK, m0);
+            tma_load_2d_2sm_hint(dst, &maps.a, full0, kb * kBK, m0, pol_a);
           }
-          tma_load_2d_2sm(dst + kABytes, &maps.b, full0, kb * kBK, n0);
+          tma_load_2d_2sm_hint(dst + kABytes, &maps.b, full0, kb * kBK, n0, pol_b);
         }
         __syncwarp();
         if (++stage == kStages) {
@@ -427,6 +431,7 @@ gemm_bf16_nt_2cta_kernel(const __grid_constant__ GemmMaps maps, const __grid_con
     const uint32_t lane_addr = static_cast<uint32_t>(ew * 32) << 16;
     const uint32_t swz = static_cast<uint32_t>(row & 7);
     const bool issuer = threadIdx.x == 128;
+    const uint64_t pol_out = l2_policy_evict_first();   // the output is written once and not read again here
     int it = 0;
     for (int tile = cluster_id; tile < total_tiles; tile += n_clusters, ++it) {
       const int acc = it & 1;
@@ -489,7 +494,7 @@ gemm_bf16_nt_2cta_kernel(const __grid_constant__ GemmMaps maps, const __grid_con
             const int head = within >> prm.d_shift, hr = head / prm.Hl, lh = head - hr * prm.Hl;
             tma_store_4d(&cmaps.m[t_out * prm.C + prm.chunk_of[lh]], buf, within & prm.d_mask, prm.j_of[lh], m0, hr);
           } else {
-            tma_store_2d(&maps.out[t_out], buf, col0 + ch * 64, m0);
+            tma_store_2d_hint(&maps.out[t_out], buf, col0 + ch * 64, m0, pol_out);
           }
         }
         if (issuer) bulk_commit();
@@ -519,6 +524,10 @@ cudaError_t map2d(TmapCache* cache, CUtensorMap* m, const void* base, uint64_t i
 // m-tiles per band: the ~148 tiles in flight cover kGroupM x (148 / kGroupM) tiles, and the whole B matrix is streamed
 // from HBM once per band.  Swept on B200: 8 / 16 / 32 / 64 -> 1374 / 1415 / 1382 / 1322 TFLOP/s.
 constexpr int kGroupM = 16;
+// CTA-pair kernel: 16 bands of 256-row tiles = 4096 rows (a 42 MB A band at K = 5120).  Swept on B200 at the cfg 3 QKV
+// shape (profiles/r2e_gemm_l2.md), DRAM reads / TFLOP/s: 8 -> 4.7 GB / 1449, 12 -> 3.7 / 1458, 16 -> 3.0-3.4 / 1497,
+// 20 -> 5.8 / 1406, 24 -> 6.2 / 1411, 32 -> 12.9 / 1348 (a band beyond ~45 MB no longer stays in L2).
+constexpr int kGroupM2 = 16;
 
 template <int BN, int kMode, bool k2Cta>
 cudaError_t launch(const GemmArgs& a, cudaStream_t stream) {
@@ -584,7 +593,7 @@ cudaError_t launch(const GemmArgs& a, cudaStream_t stream) {
   p.n_tiles = a.N / BN;
   if (k2Cta) {
     p.m_tiles = static_cast<int>((a.M + 2 * kBM - 1) / (2 * kBM));     // 256-row tiles of a CTA pair
-    p.group_m = (kGroupM + 1) / 2;
+    p.group_m = kGroupM2;
     const int total = p.m_tiles * p.n_tiles, pairs = a.num_sms / 2;
     const int grid = 2 * (total < pairs ? total : pairs);
     gemm_bf16_nt_2cta_kernel<kMode><<<grid, kThreads, Cfg2::kSmemBytes, stream>>>(maps, cmaps, p);
