@@ -337,7 +337,10 @@ def measure_backward(args, H, torch, w, C, base_flags, timed, pk, qd, kd, vd, ou
     dq, dk, dv = (torch.empty_like(qd) for _ in range(3))
     n = max(2, min(args.steps, 5))
     res = {}
-    for name, extra in (("hcms", 0), ("serial", H.HCMS_FLAG_SERIAL)):
+    variants = [("hcms", 0), ("serial", H.HCMS_FLAG_SERIAL)]
+    if D == 128:
+        variants.append(("one_pass", H.HCMS_FLAG_BWD_ONE_PASS))
+    for name, extra in variants:
         plan = H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, (base_flags & ~H.HCMS_FLAG_PROFILE) | H.HCMS_FLAG_TRAINING | extra)
         fwd = lambda: H.hcms_attention_forward(plan, qd, kd, vd, out, w.scale)
         bwd = lambda: H.hcms_attention_backward(plan, dout, dq, dk, dv, w.scale)
@@ -351,7 +354,15 @@ def measure_backward(args, H, torch, w, C, base_flags, timed, pk, qd, kd, vd, ou
         plan.close()
     f_ms, b_ms, launches = res["hcms"]
     alg = 10.0 * S * S * D * Hh
+    one = None
+    if "one_pass" in res:
+        ob = res["one_pass"][1]
+        one = {"flag": "HCMS_FLAG_BWD_ONE_PASS", "bwd_ms": round(ob, 4), "bwd_tflops_algorithmic": round(alg / (ob * 1e-3) / 1e12, 1),
+               "bwd_frac_of_burst_peak": round(alg / (ob * 1e-3) / 1e12 / pk["bf16_tflops"], 4),
+               "speedup_vs_two_pass": round(b_ms / ob, 4),
+               "what": "S and dP formed once (5 executed contractions), dQ partials added to an fp32 accumulator in key-tile order"}
     return {
+        "one_pass": one,
         "what": "hcms_attention_forward + hcms_attention_backward (scatter dO -> dK/dV pass + dQ pass -> gather dQ,dK,dV per chunk)",
         "steps": n, "fwd_ms": round(f_ms, 4), "bwd_ms": round(b_ms, 4), "fwd_bwd_ms": round(f_ms + b_ms, 4),
         "serial_fwd_bwd_ms": round(res["serial"][0] + res["serial"][1], 4),

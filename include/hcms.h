@@ -128,6 +128,14 @@ enum {
                                           compute side of the pipeline can be timed in the same stream arrangement
                                           without copies; the chunk buffers must hold an earlier call's data */
 
+#define HCMS_FLAG_BWD_ONE_PASS 0x40000u  /* D = 128, with HCMS_FLAG_TRAINING: hcms_attention_backward[_chunk] form S = QK^T
+                                          and dP = dO V^T once per (key tile, query tile) instead of once per pass
+                                          (5 executed contractions instead of 7): one kernel keeps dK_j, dV_j in tensor
+                                          memory and adds its dQ partials to an fp32 accumulator in a fixed key-tile
+                                          order (deterministic; gradients still independent of P and C).  Needs
+                                          P*h_max*(S rounded up to 64)*D*4 bytes of scratch, allocated on first use.
+                                          Ignored at D = 64 (the two-pass kernels run). */
+
 typedef struct hcms_plan hcms_plan_t;
 
 /* ---- introspection (host only, no GPU needed) ---------------------------------------- */

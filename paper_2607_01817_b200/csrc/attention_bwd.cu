@@ -480,6 +480,7 @@ cudaError_t launch(const AttnBwdArgs& a, cudaStream_t stream) {
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
   }
+  if (D == 128 && a.dq_acc && a.dq_turn) return launch_attention_bwd_1pass(a, stats, s_pad, stream);
   BwdParams prm;
   prm.S = static_cast<int>(a.S);
   prm.h_c = a.h_c;

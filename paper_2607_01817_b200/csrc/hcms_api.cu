@@ -72,6 +72,8 @@ void plan_free(hcms_plan_t* p) {
   if (p->train_ws) cudaFree(p->train_ws);
   if (p->lse) cudaFree(p->lse);
   if (p->stats) cudaFree(p->stats);
+  if (p->dq_acc) cudaFree(p->dq_acc);
+  if (p->dq_turn) cudaFree(p->dq_turn);
   for (auto& e : p->e_layer) if (e) cudaEventDestroy(e);
   delete p;
 }

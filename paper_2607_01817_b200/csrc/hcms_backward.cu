@@ -8,6 +8,13 @@ using namespace hcms;
 
 static int ensure_stats(hcms_plan_t* p) {
   if (!p->stats) HCMS_CUDA(cudaMalloc(&p->stats, attention_bwd_stats_bytes(p->sh.S, p->sh.H)));
+  if ((p->flags & HCMS_FLAG_BWD_ONE_PASS) && p->sh.D == 128 && !p->dq_acc) {
+    // two accumulators, each sized for the largest chunk: chunks alternate between the two compute streams, and the
+    // kernels of one stream run one after the other
+    const int heads = p->sh.P * p->chunks[0].h;      // Eq. 3: chunk 0 is a largest chunk
+    HCMS_CUDA(cudaMalloc(reinterpret_cast<void**>(&p->dq_acc), 2 * attention_bwd_1pass_acc_bytes(p->sh.S, heads)));
+    HCMS_CUDA(cudaMalloc(reinterpret_cast<void**>(&p->dq_turn), 2 * attention_bwd_1pass_turn_bytes(p->sh.S, heads)));
+  }
   return HCMS_OK;
 }
 
@@ -31,6 +38,11 @@ static int do_attention_bwd(hcms_plan_t* p, const void* qc, const void* kc, cons
   a.dk = dkc;
   a.dv = dvc;
   a.stats = stats_of_chunk(p, c);
+  if (p->dq_acc) {                                   // HCMS_FLAG_BWD_ONE_PASS: the buffer pair of this chunk's compute stream
+    const int heads = p->sh.P * p->chunks[0].h;
+    a.dq_acc = p->dq_acc + (c & 1) * (attention_bwd_1pass_acc_bytes(p->sh.S, heads) / sizeof(float));
+    a.dq_turn = p->dq_turn + (c & 1) * (attention_bwd_1pass_turn_bytes(p->sh.S, heads) / sizeof(int));
+  }
   a.S = p->sh.S;
   a.D = p->sh.D;
   a.P = p->sh.P;

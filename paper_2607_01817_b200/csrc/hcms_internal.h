@@ -114,6 +114,8 @@ struct AttnBwdArgs {
   void* dk;
   void* dv;
   void* stats;         // scratch, attention_bwd_stats_bytes(S, P*h_c) bytes
+  float* dq_acc = nullptr;   // single-pass kernel (D = 128): fp32 dQ accumulator, attention_bwd_1pass_acc_bytes(S, P*h_c)
+  int* dq_turn = nullptr;    // and its turn counters, attention_bwd_1pass_turn_bytes(S, P*h_c); both NULL = two passes
   int64_t S;
   int D, P, h_c;
   float scale;
@@ -122,6 +124,11 @@ struct AttnBwdArgs {
 cudaError_t launch_attention_bwd(const AttnBwdArgs& a, cudaStream_t stream);   // 3 launches
 cudaError_t attention_bwd_init();
 size_t attention_bwd_stats_bytes(int64_t S, int heads);
+// attention_bwd_1pass.cu: after the statistics kernel; a memset, the kernel and the dQ conversion on `stream`
+cudaError_t launch_attention_bwd_1pass(const AttnBwdArgs& a, const void* stats, int s_pad, cudaStream_t stream);
+cudaError_t attention_bwd_1pass_init();
+size_t attention_bwd_1pass_acc_bytes(int64_t S, int heads);
+size_t attention_bwd_1pass_turn_bytes(int64_t S, int heads);
 
 // ---- projection GEMMs (gemm_bf16.cu): C[M,N] = A[M,K] * B[N,K]^T, bf16 -> fp32 -> bf16 -------
 // chunk buffers of a plan, for the fused all-to-all modes of the projection GEMMs

@@ -35,6 +35,8 @@ struct hcms_plan {
   void* train_ws = nullptr;
   float* lse = nullptr;
   void* stats = nullptr;      // packed {lse*log2e, delta}: [H][s_pad] float2 (lazily allocated)
+  float* dq_acc = nullptr;    // HCMS_FLAG_BWD_ONE_PASS: fp32 dQ accumulator of the largest chunk, and its turn counters
+  int* dq_turn = nullptr;
   bool forward_done = false;
   float forward_scale = 0.f;  // the scale the saved lse belongs to
   // HCMS_FLAG_GRAPH: the captured chunk pipeline of the last (q, k, v, out, scale) and the stream it was captured on

@@ -167,3 +167,52 @@ def test_backward_errors():
             H.hcms_attention_backward(plan, t[0], t[1], t[1], t[3], 0.1)
         assert e.value.status == H.HCMS_ERR_ALIAS
         torch.cuda.synchronize()
+
+
+# ---------------------------------------------------------------------------------------------
+# HCMS_FLAG_BWD_ONE_PASS (D = 128): S and dP formed once, dQ reduced over the key tiles in a fixed order
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("S,P,h", [(333, 1, 3), (64, 2, 1), (1, 1, 1), (1100, 2, 1), (1365, 1, 2)])
+def test_backward_chunk_one_pass_vs_oracle(S, P, h):
+    """The single-pass kernel on oracle-made saved tensors: ragged S, one tile, one token, several key and query tiles."""
+    D, Hh = 128, P * h
+    q, k, v, do = seeded(S, Hh, D, 60 + S)
+    scale = float(np.float32(1.0 / np.sqrt(D)))
+    o_bits = bits(O.attention_full(q, k, v, scale))
+    qc, kc, vc, oc, doc = (O.scatter_chunk(t, P, 1, 0) for t in (q, k, v, o_bits, do))
+    lse = np.empty((Hh, S), np.float32)
+    for p in range(P):
+        for j in range(h):
+            lse[p * h + j] = B.log_sum_exp(qc[p, :, j, :], kc[p, :, j, :], scale)
+    ref = B.attention_backward(q, k, v, do, scale)
+    runs = []
+    with H.hcms_plan(S, Hh, D, P, 1, H.HCMS_DTYPE_BF16, H.HCMS_FLAG_BWD_ONE_PASS) as plan:
+        for _ in range(2):
+            dq, dk, dv = (dev_out(P, S, h, D) for _ in range(3))
+            H.hcms_attention_backward_chunk(plan, to_dev(qc), to_dev(kc), to_dev(vc), to_dev(oc), to_dev(doc), to_dev(lse),
+                                            dq, dk, dv, 0, scale)
+            torch.cuda.synchronize()
+            runs.append([to_host(g) for g in (dq, dk, dv)])
+    for name, g, r in zip(("dq", "dk", "dv"), runs[0], ref):
+        check_grad(g, O.scatter_chunk(r, P, 1, 0), f"one-pass {name} S={S}")
+    for a, b in zip(runs[0], runs[1]):
+        assert np.array_equal(a, b)                                # the ordered dQ reduction is deterministic
+
+
+def test_forward_backward_one_pass_invariance():
+    """Whole pipeline with the single-pass kernel: against the oracle, and bit for bit across P, C and the stream
+    arrangement (the dQ partials are added in key-tile order whatever the chunking)."""
+    S, Hh, D, P, C = 2730, 6, 128, 2, 2
+    q, k, v, do = seeded(S, Hh, D, 53, k_scale=0.5)
+    scale = float(np.float32(1.0 / np.sqrt(D)))
+    got = run_fwd_bwd(q, k, v, do, S, Hh, D, P, C, scale, H.HCMS_FLAG_BWD_ONE_PASS)
+    ref = B.attention_backward(q, k, v, do, scale)
+    for name, g, r in zip(("dq", "dk", "dv"), got[1:], ref):
+        check_grad(g, r, name)
+    two_pass = run_fwd_bwd(q, k, v, do, S, Hh, D, P, C, scale)
+    assert np.array_equal(got[0], two_pass[0])                      # the forward is untouched
+    for Pn, Cn, flags in [(1, 1, H.HCMS_FLAG_SERIAL), (3, 2, 0), (1, 6, 0), (6, 1, H.HCMS_FLAG_SINGLE_COMP)]:
+        other = run_fwd_bwd(q, k, v, do, S, Hh, D, Pn, Cn, scale, flags | H.HCMS_FLAG_BWD_ONE_PASS)
+        for a, b in zip(got, other):
+            assert np.array_equal(a, b), (Pn, Cn, flags)
