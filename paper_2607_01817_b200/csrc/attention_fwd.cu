@@ -595,7 +595,9 @@ cudaError_t make_maps(const AttnArgs& a, AttnMaps* m) {
 }
 
 // Of every 8 column pairs, kPolyPairs take their exponential on the FMA pipe (swept on B200 with this kernel, 40-step
-// sustained runs at cfg 3: 0 / 1 / 2 / 3 / 4 -> 16.79 / 16.75 / 16.52 / 16.91 / 17.36 ms; profiles/r2d_experiments.md)
+// sustained runs at cfg 3: 0 / 1 / 2 / 3 / 4 -> 16.79 / 16.75 / 16.52 / 16.91 / 17.36 ms; at D = 64, cfg 2: 2 / 3 / 4 / 5 / 6 ->
+// 0.294 / 0.294 / 0.306 / 0.334 / 0.362 ms: that shape is bound by the softmax warps' issue slots, not by MUFU;
+// profiles/r2d_experiments.md)
 constexpr int kPolyPairs = 2;
 
 cudaError_t set_attributes() {
