@@ -799,6 +799,24 @@ def run_hcms(args):
         g_res[name] = (ms_g, host_us)
         plan_g.close()
     result["pipeline"]["wall_over_max_compute_copy_graph"] = round(g_res["graph"][0] / max(attn_dual_ms, copy_ms), 4)
+    # ---- peak memory: two chunk buffer sets instead of C (HCMS_FLAG_RECYCLE_WS; the paper's Table 16 analogue) ----
+    if C > 2:
+        plan_r = H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, (base_flags & ~H.HCMS_FLAG_PROFILE) | H.HCMS_FLAG_RECYCLE_WS)
+        step_r = lambda: H.hcms_attention_forward(plan_r, qd, kd, vd, out, w.scale)
+        for _ in range(3):
+            step_r()
+        torch.cuda.synchronize()
+        ms_r = timed(plan_r, n_g, step_r) / n_g
+        ws_r = H.hcms_plan_workspace_bytes(plan_r)
+        plan_r.close()
+        plan_f = H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, 0)
+        ws_f = H.hcms_plan_workspace_bytes(plan_f)
+        plan_f.close()
+        result["recycle_ws"] = {"flag": "HCMS_FLAG_RECYCLE_WS", "ms_per_step": round(ms_r, 4),
+                                "ms_per_step_all_chunks_resident": round(g_res["enqueue"][0], 4),
+                                "workspace_bytes": ws_r, "workspace_bytes_all_chunks_resident": ws_f,
+                                "workspace_ratio": round(ws_r / ws_f, 4), "steps": n_g,
+                                "what": "chunk c reuses the buffers of chunk c - 2; A_{c-2}^out precedes A_c^in on the comm stream; same bits"}
     result["graph"] = {"enqueue_ms": round(g_res["enqueue"][0], 4), "graph_ms": round(g_res["graph"][0], 4),
                        "speedup": round(g_res["enqueue"][0] / g_res["graph"][0], 4), "steps": n_g,
                        "what": "hcms_attention_forward without profile events: %d launches + events enqueued per call vs one "

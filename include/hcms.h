@@ -136,6 +136,14 @@ enum {
                                           P*h_max*(S rounded up to 64)*D*4 bytes of scratch, allocated on first use.
                                           Ignored at D = 64 (the two-pass kernels run). */
 
+#define HCMS_FLAG_RECYCLE_WS 0x80000u    /* chunk c shares its buffers Q'_c, K'_c, V'_c, O'_c with chunk c - 2: the workspace is 2 buffer
+                                          sets sized for a largest chunk instead of one set per chunk (2/C of it for even
+                                          chunks; the paper reports 8.7 % lower peak memory for HCMS, Table 16),
+                                          and the communication stream runs A_{c-2}^out before A_c^in instead of all
+                                          inputs first (same Eq. 6-7 waits).  Same bits.  No effect for C <= 2.  Excludes
+                                          TRAINING, FUSE_A2A, SPLIT_COMM, DEBUG_ATTN_ONLY.  hcms_chunk_layout reports the
+                                          shared offsets. */
+
 typedef struct hcms_plan hcms_plan_t;
 
 /* ---- introspection (host only, no GPU needed) ---------------------------------------- */

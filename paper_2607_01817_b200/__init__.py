@@ -49,6 +49,7 @@ HCMS_FLAG_HOST_STAGED = 0x8000
 HCMS_FLAG_GEMM_1CTA = 0x10000
 HCMS_FLAG_DEBUG_ATTN_ONLY = 0x20000
 HCMS_FLAG_BWD_ONE_PASS = 0x40000
+HCMS_FLAG_RECYCLE_WS = 0x80000
 
 # every symbol include/hcms.h declares: name -> (restype, argtypes)
 _SIGNATURES = {

@@ -144,6 +144,8 @@ int do_attention(hcms_plan_t* p, const void* qc, const void* kc, const void* vc,
 // ------------------------------------------------------------------------------------------
 // the dual-stream chunk scheduler (Algorithm 1 lines 5-25), written once
 // ------------------------------------------------------------------------------------------
+constexpr int kRing = 2;     // HCMS_FLAG_RECYCLE_WS: double buffering of the chunk buffer sets
+
 int run_pipeline(hcms_plan_t* plan, cudaStream_t caller, const PipelineSteps& steps) {
   const int C = plan->sh.C;
   const bool serial = plan->flags & HCMS_FLAG_SERIAL;
@@ -174,33 +176,53 @@ int run_pipeline(hcms_plan_t* plan, cudaStream_t caller, const PipelineSteps& st
         if (s) cuda(cudaStreamWaitEvent(s, plan->e_main, 0), "wait E_main");
     }
   }
-  // Phase 1 -- input all-to-all of every chunk on S_comm (lines 8-11)
-  for (int c = 0; c < C && st == HCMS_OK && steps.comm_in; ++c) {
-    if (!cuda(mark(0, c, 0, s_in), "profile event")) break;
+  // A_c^in on S_comm (lines 8-11), then E_c^comm
+  auto do_in = [&](int c) {
+    if (!steps.comm_in || st != HCMS_OK) return;
+    if (!cuda(mark(0, c, 0, s_in), "profile event")) return;
     const int r = steps.comm_in(c, s_in);
-    if (r != HCMS_OK) { st = r; break; }
-    if (!cuda(mark(0, c, 1, s_in), "profile event")) break;
-    if (!serial) cuda(cudaEventRecord(plan->e_comm[c], s_in), "record E_c^comm");   // E_c^comm
-  }
-  // Phase 2 -- the per-chunk computation on S_comp (lines 14-18); Attn_c <- wait(E_c^comm)  (Eq. 6)
-  for (int c = 0; c < C && st == HCMS_OK && steps.compute; ++c) {
+    if (r != HCMS_OK) { st = r; return; }
+    if (!cuda(mark(0, c, 1, s_in), "profile event")) return;
+    if (!serial) cuda(cudaEventRecord(plan->e_comm[c], s_in), "record E_c^comm");
+  };
+  // Attn_c on S_comp (lines 14-18) after wait(E_c^comm) (Eq. 6), then E_c^comp
+  auto do_compute = [&](int c) {
+    if (!steps.compute || st != HCMS_OK) return;
     cudaStream_t s = comp_stream(c);
     if (!serial && steps.comm_in && !(plan->flags & HCMS_FLAG_DEBUG_NO_COMM_WAIT))
-      if (!cuda(cudaStreamWaitEvent(s, plan->e_comm[c], 0), "wait E_c^comm")) break;
-    if (!cuda(mark(1, c, 0, s), "profile event")) break;
+      if (!cuda(cudaStreamWaitEvent(s, plan->e_comm[c], 0), "wait E_c^comm")) return;
+    if (!cuda(mark(1, c, 0, s), "profile event")) return;
     const int r = steps.compute(c, s);
-    if (r != HCMS_OK) { st = r; break; }
-    if (!cuda(mark(1, c, 1, s), "profile event")) break;
-    if (!serial) cuda(cudaEventRecord(plan->e_comp[c], s), "record E_c^comp");       // E_c^comp
-  }
-  // Phase 3 -- output all-to-all per chunk on S_comm (lines 20-23); A_c^out <- wait(E_c^comp)  (Eq. 7)
-  for (int c = 0; c < C && st == HCMS_OK && steps.comm_out; ++c) {
+    if (r != HCMS_OK) { st = r; return; }
+    if (!cuda(mark(1, c, 1, s), "profile event")) return;
+    if (!serial) cuda(cudaEventRecord(plan->e_comp[c], s), "record E_c^comp");
+  };
+  // A_c^out on S_comm (lines 20-23) after wait(E_c^comp) (Eq. 7)
+  auto do_out = [&](int c) {
+    if (!steps.comm_out || st != HCMS_OK) return;
     if (!serial && steps.compute)
-      if (!cuda(cudaStreamWaitEvent(s_out, plan->e_comp[c], 0), "wait E_c^comp")) break;
-    if (!cuda(mark(2, c, 0, s_out), "profile event")) break;
+      if (!cuda(cudaStreamWaitEvent(s_out, plan->e_comp[c], 0), "wait E_c^comp")) return;
+    if (!cuda(mark(2, c, 0, s_out), "profile event")) return;
     const int r = steps.comm_out(c, s_out);
-    if (r != HCMS_OK) { st = r; break; }
+    if (r != HCMS_OK) { st = r; return; }
     cuda(mark(2, c, 1, s_out), "profile event");
+  };
+  if (steps.ring <= 0) {
+    // Alg. 1's order: the three phases one after the other (every chunk has its own buffers)
+    for (int c = 0; c < C; ++c) do_in(c);
+    for (int c = 0; c < C; ++c) do_compute(c);
+    for (int c = 0; c < C; ++c) do_out(c);
+  } else {
+    // HCMS_FLAG_RECYCLE_WS: chunk c lives in buffer set c % ring, so A_c^in may only run once A_{c-ring}^out has
+    // emptied that set.  S_comm's own order expresses it: ... A_{c-ring}^out, A_c^in ... (A^out waits for E^comp of a
+    // computation that was enqueued in an earlier iteration, so every event is recorded before it is waited on).
+    for (int c = 0; c < C + steps.ring; ++c) {
+      if (c >= steps.ring) do_out(c - steps.ring);
+      if (c < C) {
+        do_in(c);
+        do_compute(c);
+      }
+    }
   }
   if (steps.profile && st == HCMS_OK) plan->prof_calls += 1;
   // line 25: Synchronize(S_comm, S_comp) -- expressed as stream waits, the host is not blocked.  Also on the error
@@ -303,6 +325,9 @@ int hcms_plan(hcms_plan_t** out, int64_t S, int H, int D, int P, int C, int dtyp
     return fail(HCMS_ERR_INVALID_ARG, "HCMS_FLAG_GRAPH and HCMS_FLAG_PROFILE exclude each other (timing events cannot be read from a graph)");
   if ((flags & HCMS_FLAG_TRAINING) && dtype != HCMS_DTYPE_BF16)
     return fail(HCMS_ERR_UNSUPPORTED_DTYPE, "HCMS_FLAG_TRAINING needs a bf16 plan");
+  if ((flags & HCMS_FLAG_RECYCLE_WS) && (flags & (HCMS_FLAG_TRAINING | HCMS_FLAG_FUSE_A2A | HCMS_FLAG_SPLIT_COMM | HCMS_FLAG_DEBUG_ATTN_ONLY)))
+    return fail(HCMS_ERR_INVALID_ARG, "HCMS_FLAG_RECYCLE_WS excludes TRAINING (the backward reads every chunk's saved buffers), "
+                "FUSE_A2A (the projection writes all chunks at once), SPLIT_COMM and DEBUG_ATTN_ONLY");
 
   int dev = 0, sms = 0;
   int st = device_sms(&sms);          // also: a CUDA device exists and is sm_100
@@ -320,17 +345,21 @@ int hcms_plan(hcms_plan_t** out, int64_t S, int H, int D, int P, int C, int dtyp
   std::vector<int> o(C), h(C);
   chunk_table(Hl, C, o.data(), h.data());
   size_t off = 0;
+  // HCMS_FLAG_RECYCLE_WS: kRing buffer sets, each sized for a largest chunk (Eq. 3: chunk 0); chunk c uses set c % kRing
+  p->ring = (flags & HCMS_FLAG_RECYCLE_WS) && C > kRing ? kRing : 0;
+  const size_t set_stride = 4 * align_up(static_cast<size_t>(P) * S * h[0] * D * es, 1024);
   for (int c = 0; c < C; ++c) {
     Chunk& ck = p->chunks[c];
     ck.o = o[c];
     ck.h = h[c];
     ck.bytes = static_cast<size_t>(P) * S * h[c] * D * es;
+    if (p->ring) off = static_cast<size_t>(c % p->ring) * set_stride;
     for (int t = 0; t < 4; ++t) {
       ck.off[t] = off;
       off += align_up(ck.bytes, 1024);
     }
   }
-  p->ws_bytes = off;
+  p->ws_bytes = p->ring ? p->ring * set_stride : off;
 
   auto bail = [&](int status) {
     plan_free(p);
@@ -517,6 +546,7 @@ static int enqueue_forward(hcms_plan_t* plan, const void* q, const void* k, cons
   PipelineSteps steps;
   steps.split_out = plan->flags & HCMS_FLAG_SPLIT_COMM;
   steps.profile = plan->flags & HCMS_FLAG_PROFILE;
+  steps.ring = plan->ring;
   steps.comm_in = [&](int c, cudaStream_t s) -> int {           // line 8: AllToAll(Q_c, K_c, V_c), one launch
     if (attn_only) return HCMS_OK;
     const Chunk& ck = plan->chunks[c];
@@ -644,7 +674,8 @@ int hcms_attention_forward_host(hcms_plan_t* plan, const void* q, const void* k,
     const void* host_in[3] = {q, k, v};
     plan->last_launches = 0;
     PipelineSteps steps;
-    steps.split_out = true;
+    steps.split_out = plan->ring == 0;   // HCMS_FLAG_RECYCLE_WS: D2H of chunk c - ring before H2D of chunk c, on ONE stream
+    steps.ring = plan->ring;
     steps.profile = plan->flags & HCMS_FLAG_PROFILE;   // same event ring as the device path: 0 = H2D, 1 = attention, 2 = D2H
     steps.comm_in = [&](int c, cudaStream_t s) -> int {
       const Chunk& ck = plan->chunks[c];

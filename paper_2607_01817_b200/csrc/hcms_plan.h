@@ -16,6 +16,7 @@ struct hcms_plan {
   size_t ws_bytes = 0;
   void* ws = nullptr;          // chunk workspace; plan-owned memory is allocated on first use
   bool ws_owned = false;
+  int ring = 0;               // HCMS_FLAG_RECYCLE_WS: number of chunk buffer sets (0 = one per chunk)
   cudaStream_t s_comm = nullptr, s_comm_out = nullptr, s_comp = nullptr, s_comp2 = nullptr;
   cudaEvent_t e_main = nullptr, e_fin[4] = {nullptr, nullptr, nullptr, nullptr};
   std::vector<cudaEvent_t> e_comm, e_comp;
@@ -78,6 +79,7 @@ struct PipelineSteps {
   std::function<int(int c, cudaStream_t s)> comm_out;   // line 21  A_c^out  (S_comm), after wait(E_c^comp)  (Eq. 7)
   bool split_out = false;    // output all-to-all on the second communication stream (Eq. 8; HCMS_FLAG_SPLIT_COMM)
   bool profile = false;      // record the HCMS_FLAG_PROFILE event ring around every step
+  int ring = 0;              // > 0: chunk c shares its buffers with chunk c - ring (HCMS_FLAG_RECYCLE_WS): A_c^in follows A_{c-ring}^out
 };
 
 // Algorithm 1 lines 5-25: record E_main on `caller`, fork S_comm / S_comp (/ their second streams), enqueue the three

@@ -62,14 +62,16 @@ def test_projections_cfg3_sampled_rows():
         assert not bool((t == 0x7FC0).any())
 
 
-def test_forward_backward_cfg3_sampled():
+@pytest.mark.parametrize("bwd_flag", [0, H.HCMS_FLAG_BWD_ONE_PASS], ids=["two_pass", "one_pass"])
+def test_forward_backward_cfg3_sampled(bwd_flag):
+    """Full cfg 3 through the chunk pipeline, both backward kernels (the launch configuration bench.py times)."""
     w = W3
     S, Hh, D, P, C = w.S, w.H, w.D, w.P, w.C
     q, k, v = I.make_qkv(w)
     do = I.f32_to_bf16_bits(I.normal_f32(w.seed, 6, S * Hh * D).reshape(S, Hh, D))
     qd, kd, vd, dod = (to_dev(t) for t in (q, k, v, do))
     out, dq, dk, dv = (dev_out(S, Hh, D) for _ in range(4))
-    with H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, H.HCMS_FLAG_TRAINING) as plan:
+    with H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, H.HCMS_FLAG_TRAINING | bwd_flag) as plan:
         H.hcms_attention_forward(plan, qd, kd, vd, out, w.scale)
         H.hcms_attention_backward(plan, dod, dq, dk, dv, w.scale)
         torch.cuda.synchronize()

@@ -318,3 +318,51 @@ def test_backward_rejects_another_scale_and_a_replaced_workspace():
             H.hcms_attention_backward(plan, g[0], g[1], g[2], g[3], scale)
         assert ei.value.status == H.HCMS_ERR_INVALID_ARG
         torch.cuda.synchronize()
+
+
+# ---------------------------------------------------------------------------------------------
+# HCMS_FLAG_RECYCLE_WS: two chunk buffer sets instead of C (peak memory, Table 16)
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("S,Hh,D,P,C", [(1500, 12, 64, 2, 3), (2100, 20, 128, 2, 5), (1024, 12, 128, 1, 12), (1024, 8, 64, 2, 2)])
+def test_recycled_workspace_same_bits_and_smaller(S, Hh, D, P, C):
+    """Chunk c reuses the buffers of chunk c - 2 (A_{c-2}^out before A_c^in on the comm stream): same bits as the plain
+    plan from a NaN-poisoned workspace, three calls in a row, also serial, as a graph and through the host entry; the
+    workspace shrinks to two sets of the largest chunk."""
+    qkv, scale = _inputs(S, Hh, D, seed=21)
+    ref = _forward(qkv, S, Hh, D, P, C, scale)
+    R = H.HCMS_FLAG_RECYCLE_WS
+    with H.hcms_plan(S, Hh, D, P, C) as plain, H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, R) as ring:
+        full, small = H.hcms_plan_workspace_bytes(plain), H.hcms_plan_workspace_bytes(ring)
+        _, h = H.hcms_chunk_table(ring)
+        if C > 2:
+            assert small < full and small <= 2 * 4 * (P * S * h[0] * D * 2 + 1024)
+            l0, l2 = H.hcms_chunk_layout(ring, 0), H.hcms_chunk_layout(ring, 2)
+            assert l0["q_off"] == l2["q_off"] and l0["o_off"] >= l2["o_off"]          # chunk 2 lives in chunk 0's set
+        else:
+            assert small == full
+    for extra in (0, H.HCMS_FLAG_SERIAL, H.HCMS_FLAG_SINGLE_COMP, H.HCMS_FLAG_GRAPH, H.HCMS_FLAG_LAYOUT_TMA):
+        q, k, v = qkv
+        out = nan_fill_(torch.empty_like(q))
+        with H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, R | extra) as plan:
+            n = H.hcms_plan_workspace_bytes(plan)
+            ws = nan_fill_(torch.empty((n + 1) // 2, dtype=torch.int16, device=DEV))
+            H.hcms_plan_set_workspace(plan, ws, n)
+            for _ in range(3):
+                nan_fill_(out)
+                H.hcms_attention_forward(plan, q, k, v, out, scale)
+            torch.cuda.synchronize()
+            assert H.hcms_plan_last_launch_count(plan) == 3 * C or (extra & H.HCMS_FLAG_GRAPH)
+        assert np.array_equal(to_host(out), ref), hex(extra)
+    hq, hk, hv = (to_host(t) for t in qkv)
+    hout = np.full_like(hq, 0x7FC0)
+    with H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, R) as plan:
+        H.hcms_attention_forward_host(plan, hq, hk, hv, hout, scale)
+    assert np.array_equal(hout, ref)
+
+
+def test_recycled_workspace_flag_errors():
+    for bad in (H.HCMS_FLAG_TRAINING, H.HCMS_FLAG_FUSE_A2A, H.HCMS_FLAG_SPLIT_COMM):
+        with pytest.raises(H.HcmsError) as e:
+            H.hcms_plan(1024, 8, 64, 2, 4, H.HCMS_DTYPE_BF16, H.HCMS_FLAG_RECYCLE_WS | bad)
+        assert e.value.status == H.HCMS_ERR_INVALID_ARG
