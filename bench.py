@@ -62,6 +62,8 @@ def parse_args(argv=None):
     ap.add_argument("--attn-pair", action="store_true", help="HCMS_FLAG_ATTN_PAIR: attention forward on CTA pairs (D = 128)")
     ap.add_argument("--replicas", action="store_true", help="N > 1: independent replicas per rank instead of the sequence-sharded "
                                                             "hcms_dist path")
+    ap.add_argument("--dist-fuse-out", action="store_true", help="N > 1: HCMS_FLAG_DIST_FUSE_OUT, the output all-to-all as TMA stores "
+                                                                 "into peer memory from the attention epilogue (no pull-gather kernel)")
     ap.add_argument("--share-gpu", action="store_true", help="N > 1 on ONE GPU (tests): every rank uses cuda:0, rendezvous over gloo")
     ap.add_argument("--quick", action="store_true", help="only the contract measurement of the hot path (no layer, backward, e2e, "
                                                          "graph, value-independence, cpu baseline blocks)")
@@ -411,7 +413,7 @@ def run_dist(args, torch, H, rank, local, world, nccl):
     def agreed(ok: bool) -> bool:
         return max_over_ranks(0.0 if ok else 1.0, world, nccl) == 0.0
     try:
-        plan = H.hcms_dist_plan(S, Hh, D, P, C, rank)
+        plan = H.hcms_dist_plan(S, Hh, D, P, C, rank, H.HCMS_DTYPE_BF16, H.HCMS_FLAG_DIST_FUSE_OUT if args.dist_fuse_out else 0)
     except Exception as e:  # noqa: BLE001
         why = f"hcms_dist_plan: {e}"
     ok = agreed(plan is not None)
@@ -482,6 +484,7 @@ def run_dist(args, torch, H, rank, local, world, nccl):
                    "S": S, "H": Hh, "D": D, "P": P, "C": C,
                    "multi_gpu": "sequence-sharded, P = N: hcms_dist (push scatter / pull gather over CUDA-IPC peer memory, "
                                 "epoch flags awaited by streams; no NCCL on the data path)" +
+                                (" + HCMS_FLAG_DIST_FUSE_OUT (output all-to-all = TMA stores from the attention epilogue)" if args.dist_fuse_out else "") +
                                 (" -- ranks SHARE cuda:0 (test mode)" if args.share_gpu else ""),
                    "l2": "inputs larger than L2" if 3 * shard_bytes >= 2 * L2_BYTES else "per-rank shards fit in L2 (not flushed)",
                    "inputs": "hcms_inputs counter-based N(0,1) -> bf16 (seed %d), rank r holds rows [r*S/P, (r+1)*S/P)" % w.seed},

@@ -144,6 +144,13 @@ enum {
                                           TRAINING, FUSE_A2A, SPLIT_COMM, DEBUG_ATTN_ONLY.  hcms_chunk_layout reports the
                                           shared offsets. */
 
+#define HCMS_FLAG_DIST_FUSE_OUT 0x100000u /* hcms_dist_plan only: the output all-to-all (Alg. 1 line 21) happens in the attention
+                                          kernel's epilogue -- every 128-row output tile is TMA-stored straight into the
+                                          destination rank's sequence-sharded output inside that rank's exchange block
+                                          (peer memory), instead of O'_c followed by a pull-gather kernel: one kernel does
+                                          the compute and its collective.  The exchange block grows by S/P*H*D*2 bytes; the
+                                          call ends with one local copy into `out`.  Same bits. */
+
 typedef struct hcms_plan hcms_plan_t;
 
 /* ---- introspection (host only, no GPU needed) ---------------------------------------- */

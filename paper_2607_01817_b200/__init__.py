@@ -50,6 +50,7 @@ HCMS_FLAG_GEMM_1CTA = 0x10000
 HCMS_FLAG_DEBUG_ATTN_ONLY = 0x20000
 HCMS_FLAG_BWD_ONE_PASS = 0x40000
 HCMS_FLAG_RECYCLE_WS = 0x80000
+HCMS_FLAG_DIST_FUSE_OUT = 0x100000
 
 # every symbol include/hcms.h declares: name -> (restype, argtypes)
 _SIGNATURES = {

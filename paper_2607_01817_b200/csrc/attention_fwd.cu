@@ -96,6 +96,8 @@ __host__ __device__ constexpr uint32_t make_idesc(int M, int N, bool b_mn_major)
 struct alignas(64) AttnMaps {
   CUtensorMap q, k, v, o;   // rank-4 {D, h_c, S, P}, box {64, 1, 128, 1}, SWIZZLE_128B
   CUtensorMap kh;           // K with box {64, 1, 64, 1}: the half tile a CTA of a pair loads
+  CUtensorMap op[kMaxPeers];   // fused output all-to-all: rank r's [push_rows][push_heads][D] output, rank-3 {D, heads, rows},
+                               // box {64, 1, 128} (copies of o when unused)
 };
 
 struct AttnParams {
@@ -104,6 +106,9 @@ struct AttnParams {
   int h_c;
   float scale_log2;  // scale * log2(e)
   float* lse;        // optional [P*h_c][S]: log sum_k exp(scale q.k) per query row (natural log), for the backward
+  int n_push;        // > 0: output tiles go to the n_push ranks' sequence-sharded outputs (AttnMaps::op), not to o
+  int push_rows;     // tokens per rank
+  int push_head0;    // global head of this launch's head 0
 };
 
 // ---- packed fp32x2 arithmetic (FFMA2 / FADD2 on sm_100) and helpers ----------------------------------
@@ -553,9 +558,23 @@ attention_fwd_kernel(const __grid_constant__ AttnMaps maps, const AttnParams prm
     if ((warp & 3) == 0 && lane == 0) {
       const int row0 = q_row0 + t * kBM;
       if (row0 < prm.S) {
+        if (prm.n_push > 0) {
+          // Output all-to-all in the epilogue (Alg. 1 line 21 between real ranks): the tile's rows belong to
+          // one or two destination ranks.  Every destination has kBM pad rows in front of its row 0 (a TMA store with a
+          // negative start coordinate faults on sm_100: measured), so the second rank of a straddling tile receives the
+          // tile's leading rows in its pad; rows past a rank's end (and rows >= S) are clipped by the tensor map.
+          const int r_lo = row0 / prm.push_rows;
+          int r_hi = (row0 + kBM - 1) / prm.push_rows;
+          r_hi = r_hi < prm.n_push ? r_hi : prm.n_push - 1;
+          for (int r = r_lo; r <= r_hi; ++r)
 #pragma unroll
-        for (int pn = 0; pn < C::kPanels; ++pn)
-          tma_store_4d(&maps.o, o_smem + pn * kPanelBytes, pn * 64, hj, row0, rank);
+            for (int pn = 0; pn < C::kPanels; ++pn)
+              tma_store_3d(&maps.op[r], o_smem + pn * kPanelBytes, pn * 64, prm.push_head0 + hj, row0 - r * prm.push_rows + kBM);
+        } else {
+#pragma unroll
+          for (int pn = 0; pn < C::kPanels; ++pn)
+            tma_store_4d(&maps.o, o_smem + pn * kPanelBytes, pn * 64, hj, row0, rank);
+        }
         bulk_commit();
         bulk_wait<0>();
       }
@@ -584,6 +603,19 @@ cudaError_t make_maps(const AttnArgs& a, AttnMaps* m) {
     cudaError_t e = encode_tensor_map(a.cache, outs[i], CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, ptrs[i], dims, strides, box,
                                       CU_TENSOR_MAP_SWIZZLE_128B);
     if (e != cudaSuccess) return e;
+  }
+  for (int r = 0; r < kMaxPeers; ++r) m->op[r] = m->o;
+  if (a.o_push) {
+    if (a.P != 1 || a.n_push < 1 || a.n_push > kMaxPeers || a.push_rows < 1) return cudaErrorInvalidValue;
+    const uint64_t pdims[3] = {static_cast<uint64_t>(a.D), static_cast<uint64_t>(a.push_heads),
+                               static_cast<uint64_t>(a.push_rows) + kBM};     // o_push[r] points at kBM pad rows before row 0
+    const uint64_t pstrides[2] = {static_cast<uint64_t>(a.D) * 2, static_cast<uint64_t>(a.push_heads) * a.D * 2};
+    const uint32_t pbox[3] = {64, 1, 128};
+    for (int r = 0; r < a.n_push; ++r) {
+      cudaError_t e = encode_tensor_map(a.cache, &m->op[r], CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, a.o_push[r], pdims, pstrides, pbox,
+                                        CU_TENSOR_MAP_SWIZZLE_128B);
+      if (e != cudaSuccess) return e;
+    }
   }
   if (!a.pair) {        // only the CTA-pair kernel reads the half-tile map
     m->kh = m->k;
@@ -632,6 +664,9 @@ cudaError_t launch_attention(const AttnArgs& a0, cudaStream_t stream) {
   // masked tail keys while exp2(s*1e-30) is exactly 1 in fp32.
   prm.scale_log2 = fmaxf(a.scale * 1.4426950408889634f, 1e-30f);
   prm.lse = a.lse;
+  prm.n_push = a.o_push ? a.n_push : 0;
+  prm.push_rows = static_cast<int>(a.push_rows);
+  prm.push_head0 = a.push_head0;
   dim3 grid(static_cast<unsigned>((a.S + kQTiles * kBM - 1) / (kQTiles * kBM)), static_cast<unsigned>(a.P * a.h_c));
   if (a.pair) {
     // CTA pairs: a cluster of 2 consecutive CTAs (512 query rows) per launch unit; an odd block count is padded by

@@ -75,6 +75,9 @@ struct hcms_dist_plan {
   int device = 0;
   int64_t Sl = 0;                // tokens per rank
   std::vector<Chunk> chunks;     // bytes / off: this rank's buffers [S][h_c][D] inside the exchange block
+  size_t out_off = 0;            // HCMS_FLAG_DIST_FUSE_OUT: this rank's output [Sl][H][D], written by every rank's attention epilogue
+  size_t out_bytes = 0;
+  size_t out_pad = 0;            // pad rows in front of it
   size_t flag_off = 0;           // arrived[C][P] then ready[C][P], uint32
   size_t block_bytes = 0;
   char* block = nullptr;         // this rank's exchange block (cudaMalloc, exported through CUDA IPC)
@@ -116,8 +119,8 @@ int hcms_dist_plan(hcms_dist_plan_t** out, int64_t S, int H, int D, int P, int C
     return fail(HCMS_ERR_INVALID_ARG, "S=%lld H=%d D=%d P=%d C=%d must all be positive", static_cast<long long>(S), H, D, P, C);
   if (rank < 0 || rank >= P) return fail(HCMS_ERR_INVALID_ARG, "rank=%d outside [0,%d)", rank, P);
   if (dtype != HCMS_DTYPE_BF16) return fail(HCMS_ERR_UNSUPPORTED_DTYPE, "the distributed path is bf16 only");
-  if (flags & ~static_cast<uint32_t>(HCMS_FLAG_ATTN_PAIR))
-    return fail(HCMS_ERR_INVALID_ARG, "hcms_dist_plan accepts HCMS_FLAG_ATTN_PAIR only (flags=0x%x)", flags);
+  if (flags & ~static_cast<uint32_t>(HCMS_FLAG_ATTN_PAIR | HCMS_FLAG_DIST_FUSE_OUT))
+    return fail(HCMS_ERR_INVALID_ARG, "hcms_dist_plan accepts HCMS_FLAG_ATTN_PAIR and HCMS_FLAG_DIST_FUSE_OUT only (flags=0x%x)", flags);
   if (S % P) return fail(HCMS_ERR_UNSUPPORTED_SHAPE, "S=%lld is not divisible by P=%d", static_cast<long long>(S), P);
   if (H % P) return fail(HCMS_ERR_UNSUPPORTED_SHAPE, "H=%d is not divisible by P=%d", H, P);
   if (D != 64 && D != 128) return fail(HCMS_ERR_UNSUPPORTED_SHAPE, "D=%d: only head dimensions 64 and 128 are built", D);
@@ -150,6 +153,12 @@ int hcms_dist_plan(hcms_dist_plan_t** out, int64_t S, int H, int D, int P, int C
       ck.off[t] = off;
       off += (ck.bytes + 1023) / 1024 * 1024;
     }
+  }
+  if (flags & HCMS_FLAG_DIST_FUSE_OUT) {
+    p->out_pad = static_cast<size_t>(kAttnPushPadRows) * H * D * 2;      // spill rows of tiles that straddle two ranks
+    p->out_off = off;
+    p->out_bytes = static_cast<size_t>(S / P) * H * D * 2;
+    off += (p->out_pad + p->out_bytes + 1023) / 1024 * 1024;
   }
   p->flag_off = off;
   p->block_bytes = off + (static_cast<size_t>(2) * C * P * sizeof(uint32_t) + 1023) / 1024 * 1024;
@@ -373,6 +382,15 @@ int enqueue_phase(const RankCall& rc, int phase, float scale) {
                  sh.S, sh.D, 1, ck.h, scale};
       a.pair = (plan->flags & HCMS_FLAG_ATTN_PAIR) != 0;
       a.cache = &plan->tmaps;
+      void* push[kMaxPeers];
+      if (plan->out_bytes) {          // output all-to-all in the attention epilogue: TMA stores into every rank's output
+        for (int p = 0; p < P; ++p) push[p] = plan->peer[p] + plan->out_off;
+        a.o_push = push;
+        a.n_push = P;
+        a.push_rows = plan->Sl;
+        a.push_heads = sh.H;
+        a.push_head0 = r * sh.Hl + ck.o;
+      }
       plan->last_launches += 1;
       if (cuda(launch_attention(a, plan->s_comp), "attention launch")) signal(1, c, plan->s_comp);   // E_c^comp as a flag
     }
@@ -380,9 +398,13 @@ int enqueue_phase(const RankCall& rc, int phase, float scale) {
     // lines 20-23, 26: output all-to-all = loads of this rank's rows from every peer's O'_c (Eq. 7), written into `out`
     for (int c = 0; c < C && status == HCMS_OK; ++c) {
       if (!wait_all(1, c, plan->s_comm)) break;
+      if (plan->out_bytes) continue;        // fused: the peers' attention kernels have already delivered chunk c's heads
       const void* dst[1] = {rc.out};
       layout(c, true, 1, dst, plan->s_comm);
     }
+    if (plan->out_bytes && status == HCMS_OK)       // Concat (line 26): the assembled output leaves the exchange block
+      cuda(cudaMemcpyAsync(rc.out, plan->block + plan->out_off + plan->out_pad, plan->out_bytes, cudaMemcpyDeviceToDevice, plan->s_comm),
+           "copy of the assembled output");
     // line 25, on every path
     cudaStream_t forked[2] = {plan->s_comm, plan->s_comp};
     const int keep = status;

@@ -87,6 +87,7 @@ cudaError_t launch_layout_vec(const LayoutArgs& a, cudaStream_t stream);
 cudaError_t launch_layout_tma(const LayoutArgs& a, cudaStream_t stream, int num_sms);
 
 // ---- attention kernel (attention_fwd.cu) ------------------------------------------------
+constexpr int kAttnPushPadRows = 128;
 struct AttnArgs {
   const void* q;     // [P][S][h_c][D] bf16
   const void* k;
@@ -98,6 +99,14 @@ struct AttnArgs {
   float* lse = nullptr;   // optional [P*h_c][S] fp32: log sum_k exp(scale q.k) per row (saved for the backward)
   bool pair = false;      // CTA-pair kernel (HCMS_FLAG_ATTN_PAIR; D = 128 only, ignored otherwise)
   TmapCache* cache = nullptr;
+  // Output all-to-all fused into the epilogue (hcms_dist, HCMS_FLAG_DIST_FUSE_OUT; needs P == 1): instead of o, the 128-row
+  // output tiles are TMA-stored straight into the sequence-sharded [push_rows][push_heads][D] tensors of n_push ranks --
+  // row s of local head j goes to o_push[s / push_rows] at row s % push_rows, head push_head0 + j.  o_push[r] must point at
+  // kAttnPushPadRows pad rows in FRONT of rank r's row 0 (tiles that straddle two ranks spill there).  NULL = plain o.
+  void* const* o_push = nullptr;
+  int n_push = 0;
+  int64_t push_rows = 0;
+  int push_heads = 0, push_head0 = 0;
 };
 cudaError_t launch_attention(const AttnArgs& a, cudaStream_t stream);
 cudaError_t attention_init();  // sets kernel attributes once per device

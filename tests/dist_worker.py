@@ -35,7 +35,7 @@ def worker(rank, world, port, a):
     Sl = S // P
     dev = [torch.from_numpy(t[rank * Sl:(rank + 1) * Sl].view(np.int16).copy()).to("cuda:0") for t in (q, k, v)]
     out = torch.empty_like(dev[0])
-    plan = H.hcms_dist_plan(S, Hh, D, P, C, rank)
+    plan = H.hcms_dist_plan(S, Hh, D, P, C, rank, H.HCMS_DTYPE_BF16, a.flags)
     H.hcms_dist_exchange_handles(plan)                       # all_gather of 128 bytes per rank over gloo, then attach
     gathered = None
     for rep in range(3):
@@ -87,7 +87,7 @@ def local(a):
     shards = [[t[r * Sl:(r + 1) * Sl].contiguous() for t in (qd, kd, vd)] for r in range(P)]
     outs = [torch.empty_like(shards[r][0]) for r in range(P)]
     streams = [torch.cuda.Stream() for _ in range(P)]
-    plans = [H.hcms_dist_plan(S, Hh, D, P, C, r) for r in range(P)]
+    plans = [H.hcms_dist_plan(S, Hh, D, P, C, r, H.HCMS_DTYPE_BF16, a.flags) for r in range(P)]
     for pl in plans:
         H.hcms_dist_attach_local(pl, plans)
     for rep in range(3):
@@ -100,7 +100,8 @@ def local(a):
             s.synchronize()
         got = torch.cat(outs, dim=0).cpu().numpy().view(np.uint16)
         assert np.array_equal(got, want), f"call {rep}: ranks differ from the emulation"
-    assert H.hcms_dist_last_launch_count(plans[0]) == 5 * C
+    # push + signal + attention + signal (+ pull) per chunk; the fused form has no pull kernel
+    assert H.hcms_dist_last_launch_count(plans[0]) == (4 if a.flags & H.HCMS_FLAG_DIST_FUSE_OUT else 5) * C
     torch.cuda.synchronize()
     for pl in plans:
         pl.close()
@@ -113,6 +114,7 @@ def main():
     ap.add_argument("--local", type=int, default=0)
     for name in ("S", "H", "D", "C"):
         ap.add_argument("--" + name, type=int, required=True)
+    ap.add_argument("--flags", type=int, default=0, help="hcms_dist_plan flags (HCMS_FLAG_DIST_FUSE_OUT, HCMS_FLAG_ATTN_PAIR)")
     a = ap.parse_args()
     if a.local:
         local(a)

@@ -36,9 +36,9 @@ def _emulation(q, k, v, S, Hh, D, P, C, scale):
     return to_host(out)
 
 
-def _run_worker(mode, P, S, Hh, D, C, env=None):
+def _run_worker(mode, P, S, Hh, D, C, env=None, flags=0):
     cmd = [sys.executable, os.path.join(ROOT, "tests", "dist_worker.py"), mode, str(P), "--S", str(S), "--H", str(Hh),
-           "--D", str(D), "--C", str(C)]
+           "--D", str(D), "--C", str(C), "--flags", str(flags)]
     r = subprocess.run(cmd, capture_output=True, text=True, timeout=240, cwd=ROOT, env=dict(os.environ, **(env or {})))
     assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-3000:]
     assert "DIST_OK" in r.stdout, r.stdout[-2000:]
@@ -101,3 +101,24 @@ def test_ranks_as_processes_over_cuda_ipc(P, C):
     """One process per rank on cuda:0, CUDA-IPC handles exchanged over gloo, three forward calls; rank 0 compares the
     all-gathered outputs with the single-device emulation bit for bit.  Every worker carries a 120 s watchdog."""
     _run_worker("--spawn", P, 1024, 8, 128, C)
+
+
+# ---------------------------------------------------------------------------------------------
+# HCMS_FLAG_DIST_FUSE_OUT: the output all-to-all in the attention kernel's epilogue (TMA stores into peer memory)
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("S,Hh,D,P,C", [(1024, 4, 64, 2, 2), (2040, 12, 128, 4, 3), (768, 6, 128, 3, 2), (516, 8, 64, 1, 3),
+                                        (900, 6, 128, 3, 1)])
+def test_fused_output_push_in_one_process_bit_equal(S, Hh, D, P, C):
+    """Same check as above with the pull-gather kernel replaced by epilogue stores into every rank's output: tiles that
+    straddle two ranks (S/P = 510, 256, 300 are not multiples of 128) are stored twice with clipping."""
+    _run_worker("--local", P, S, Hh, D, C, flags=H.HCMS_FLAG_DIST_FUSE_OUT)
+
+
+def test_fused_output_push_with_pairs_in_one_process():
+    _run_worker("--local", 2, 2048, 8, 128, 2, flags=H.HCMS_FLAG_DIST_FUSE_OUT | H.HCMS_FLAG_ATTN_PAIR)
+
+
+@pytest.mark.parametrize("P,C", [(2, 2), (4, 1)])
+def test_fused_output_push_as_processes_over_cuda_ipc(P, C):
+    _run_worker("--spawn", P, 1024, 8, 128, C, flags=H.HCMS_FLAG_DIST_FUSE_OUT)
