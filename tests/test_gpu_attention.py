@@ -197,13 +197,19 @@ def test_attention_chunk_alone_matches_oracle_on_sharded_buffers():
 # ---------------------------------------------------------------------------------------------
 
 @pytest.mark.parametrize("cfg", [3, 4, 5])
-def test_full_size_configs_sampled_rows(cfg):
+def test_full_size_configs_sampled_rows(cfg, full_oracle):
     w = I.workload(cfg)
     q, k, v = I.make_qkv(w, threads=16)
     got = run_forward(q, k, v, w.S, w.H, w.D, w.P, w.C, w.scale, poison=True)
     rows = O.sample_rows(w.S, w.P, n_random=24 if cfg == 5 else 48, seed=cfg)
     ref = O.attention_sampled(q, k, v, w.scale, rows)
     mx, mean, rel = check(got[rows], ref, f"cfg{cfg}")
+    if full_oracle:           # --full-oracle: every query row of the first and the last head (two different ranks and chunks)
+        heads = [0, w.H - 1]
+        sub = lambda t: np.ascontiguousarray(t[:, heads, :])
+        ref_all = O.attention_full(sub(q), sub(k), sub(v), w.scale)
+        fm, fmean, frel = check(sub(got), ref_all, f"cfg{cfg} all rows of heads {heads}")
+        print(f"cfg{cfg} --full-oracle: rows={w.S} heads={heads} max_abs={fm:.3e} mean_abs={fmean:.3e} rel_l2={frel:.3e}")
     print(f"cfg{cfg}: rows={len(rows)} max_abs={mx:.3e} mean_abs={mean:.3e} rel_l2={rel:.3e}")
     # a property of every element, at any size: each output coordinate lies in [min_s V, max_s V]
     vf = I.bf16_bits_to_f32(v)
