@@ -454,7 +454,7 @@ void* hcms_plan_lse(const hcms_plan_t* plan);
  * the concatenated outputs of the P ranks are BIT-EQUAL to hcms_attention_forward on the concatenated inputs.
  *
  * hcms_dist_plan: collective in spirit (every rank creates its own with the same S, H, D, P, C); allocates the
- * exchange block (4*S*(H/P)*D*2 bytes + flags) on the current device.  flags: 0 or HCMS_FLAG_ATTN_PAIR.  bf16 only.
+ * exchange block (4*S*(H/P)*D*2 bytes + flags) on the current device.  flags: 0 or any of HCMS_FLAG_ATTN_PAIR, HCMS_FLAG_DIST_FUSE_OUT (the exchange block then also holds this rank's output and 128 pad rows).  bf16 only.
  * hcms_dist_export: writes HCMS_DIST_HANDLE_BYTES opaque bytes that another PROCESS passes to hcms_dist_attach.
  * hcms_dist_attach: `handles` = P consecutive handles in rank order (this rank's own entry is checked, not opened);
  * the caller moves the bytes between processes with any host channel (torch.distributed, files).
