@@ -470,6 +470,14 @@ void* hcms_plan_lse(const hcms_plan_t* plan);
  * deadlocks).  hcms_dist_attention_forward therefore rejects locally attached plans (INVALID_ARG); one process per
  * rank -- the deployment the paper describes -- has no such constraint.  Switches to each plan's device for its part.
  * All ranks must have finished (a host barrier after synchronising the streams) before any plan is destroyed.
+ * hcms_dist_layer_forward[_group]: the whole layer (Alg. 1 lines 2-27) between the ranks with BOTH all-to-alls inside
+ * compute kernels; the plan must carry HCMS_FLAG_DIST_FUSE_OUT.  x = this rank's tokens [S/P, Dm] bf16, w_qkv [3*H*D, Dm]
+ * and w_o [Dm, H*D] as in hcms_layer_forward (every rank holds the whole weights), rope_cos / rope_sin = this rank's
+ * rows [S/P, D/2] fp32 or both NULL, y = [S/P, Dm].  The QKV projection's epilogue (RoPE, one rounding to bf16) TMA-stores
+ * each 128 x 64 panel of q, k, v into the chunk buffer of the rank that owns its head (input all-to-all, peer memory); the
+ * attention epilogue stores into the destination ranks' outputs (output all-to-all); the output projection reads the
+ * assembled [S/P, H*D] output in place.  C + 2 kernels and 2C signals per rank.  The concatenated y of the P ranks is
+ * BIT-EQUAL to hcms_layer_forward on the concatenated x.  Needs 3*C*P <= 48, H/P <= 64, Dm and H*D multiples of 128.
  * Errors: INVALID_ARG, UNSUPPORTED_SHAPE (also P > 16), UNSUPPORTED_DTYPE, UNSUPPORTED_DEVICE, PLAN_MISMATCH (handle of
  * another shape / rank order, wrong device), MISALIGNED, ALIAS, CUDA.
  */
@@ -484,6 +492,11 @@ int hcms_dist_attention_forward(hcms_dist_plan_t* plan, const void* q, const voi
                                 float scale, void* stream);
 int hcms_dist_attention_forward_group(hcms_dist_plan_t* const* plans, int n, const void* const* q, const void* const* k,
                                       const void* const* v, void* const* out, float scale, void* const* streams);
+int hcms_dist_layer_forward(hcms_dist_plan_t* plan, const void* x, const void* w_qkv, const void* w_o, const void* rope_cos,
+                            const void* rope_sin, void* y, int Dm, float scale, void* stream);
+int hcms_dist_layer_forward_group(hcms_dist_plan_t* const* plans, int n, const void* const* x, const void* w_qkv,
+                                  const void* w_o, const void* const* rope_cos, const void* const* rope_sin, void* const* y,
+                                  int Dm, float scale, void* const* streams);
 /* Bytes of the rank's exchange block; kernels + signal launches of the last forward (C pushes + C attention + C pulls
  * + 2C signals).  0 for a NULL plan. */
 size_t hcms_dist_block_bytes(const hcms_dist_plan_t* plan);

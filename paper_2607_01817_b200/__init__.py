@@ -100,6 +100,9 @@ _SIGNATURES = {
     "hcms_dist_attach_local": (c_int, [c_void_p, POINTER(c_void_p), c_int]),
     "hcms_dist_attention_forward": (c_int, [c_void_p] * 5 + [c_float, c_void_p]),
     "hcms_dist_attention_forward_group": (c_int, [POINTER(c_void_p), c_int] + [POINTER(c_void_p)] * 4 + [c_float, POINTER(c_void_p)]),
+    "hcms_dist_layer_forward": (c_int, [c_void_p] * 7 + [c_int, c_float, c_void_p]),
+    "hcms_dist_layer_forward_group": (c_int, [POINTER(c_void_p), c_int, POINTER(c_void_p), c_void_p, c_void_p, POINTER(c_void_p),
+                                              POINTER(c_void_p), POINTER(c_void_p), c_int, c_float, POINTER(c_void_p)]),
     "hcms_dist_block_bytes": (c_size_t, [c_void_p]),
     "hcms_dist_last_launch_count": (c_int, [c_void_p]),
     "hcms_autotune_chunks_host": (c_int, [c_int64, c_int, c_int, c_int, c_uint32] + [c_void_p] * 4 +
@@ -499,6 +502,22 @@ def hcms_dist_attention_forward_group(plans, qs, ks, vs, outs, scale: float, str
     st = (c_void_p * n)(*[_stream(s) for s in streams])
     _check(lib.hcms_dist_attention_forward_group(pl, n, arr(qs), arr(ks), arr(vs), arr(outs), scale, st),
            "hcms_dist_attention_forward_group")
+
+
+def hcms_dist_layer_forward(plan: DistPlan, x, w_qkv, w_o, rope_cos, rope_sin, y, Dm: int, scale: float, stream=None) -> None:
+    """Alg. 1 lines 2-27 between real ranks (plan made with HCMS_FLAG_DIST_FUSE_OUT); this rank's [S/P, Dm] tokens."""
+    _check(lib.hcms_dist_layer_forward(plan.handle, _ptr(x), _ptr(w_qkv), _ptr(w_o), _ptr(rope_cos), _ptr(rope_sin), _ptr(y),
+                                       Dm, scale, _stream(stream)), "hcms_dist_layer_forward")
+
+
+def hcms_dist_layer_forward_group(plans, xs, w_qkv, w_o, coss, sins, ys, Dm: int, scale: float, streams) -> None:
+    """All P ranks of one process in one call (plans attached with hcms_dist_attach_local), distinct caller streams."""
+    n = len(plans)
+    arr = lambda v: (c_void_p * n)(*[_ptr(t) for t in v]) if v is not None else None
+    pl = (c_void_p * n)(*[p.handle.value for p in plans])
+    st = (c_void_p * n)(*[_stream(s) for s in streams])
+    _check(lib.hcms_dist_layer_forward_group(pl, n, arr(xs), _ptr(w_qkv), _ptr(w_o), arr(coss), arr(sins), arr(ys), Dm, scale, st),
+           "hcms_dist_layer_forward_group")
 
 
 def hcms_dist_block_bytes(plan: DistPlan) -> int:

@@ -73,6 +73,9 @@ struct GemmParams {
   const float* sin;
   int m_tiles, n_tiles;
   int group_m;          // m-tiles per band of the tile walk
+  // kFusedOut between real ranks (hcms_dist): one map per (tensor, chunk, destination rank) instead of one per (tensor,
+  // chunk) with the rank as its 4th coordinate: map index = (t * C + c) * peer_n + rank * peer_on
+  int peer_n, peer_on;  // (P, 1) with peer maps, (1, 0) without
 };
 
 __device__ __forceinline__ void tile_coords(int tile, const GemmParams& p, int& m0, int& n0) {
@@ -273,7 +276,8 @@ gemm_bf16_nt_kernel(const __grid_constant__ GemmMaps maps, const __grid_constant
           if (kMode == kFusedOut) {
             const int within = col0 + ch * 64;
             const int head = within >> prm.d_shift, rank = head / prm.Hl, lh = head - rank * prm.Hl;
-            tma_store_4d(&cmaps.m[t_out * prm.C + prm.chunk_of[lh]], buf, within & prm.d_mask, prm.j_of[lh], m0, rank);
+            tma_store_4d(&cmaps.m[(t_out * prm.C + prm.chunk_of[lh]) * prm.peer_n + rank * prm.peer_on], buf, within & prm.d_mask, prm.j_of[lh], m0,
+                         prm.peer_on ? 0 : rank);
           } else {
             tma_store_2d(&maps.out[t_out], buf, col0 + ch * 64, m0);
           }
@@ -492,7 +496,8 @@ gemm_bf16_nt_2cta_kernel(const __grid_constant__ GemmMaps maps, const __grid_con
           if (kMode == kFusedOut) {
             const int within = col0 + ch * 64;
             const int head = within >> prm.d_shift, hr = head / prm.Hl, lh = head - hr * prm.Hl;
-            tma_store_4d(&cmaps.m[t_out * prm.C + prm.chunk_of[lh]], buf, within & prm.d_mask, prm.j_of[lh], m0, hr);
+            tma_store_4d(&cmaps.m[(t_out * prm.C + prm.chunk_of[lh]) * prm.peer_n + hr * prm.peer_on], buf, within & prm.d_mask, prm.j_of[lh], m0,
+                         prm.peer_on ? 0 : hr);
           } else {
             tma_store_2d_hint(&maps.out[t_out], buf, col0 + ch * 64, m0, pol_out);
           }
@@ -561,7 +566,22 @@ cudaError_t launch(const GemmArgs& a, cudaStream_t stream) {
       if (kMode == kFusedOut || t > 0) maps.out[t] = kMode == kFusedOut ? maps.a : maps.out[0];
     const int n_tensors = kMode == kFusedOut ? n_out : 1;
     for (auto& m : cmaps.m) m = maps.b;
-    for (int t = 0; t < n_tensors; ++t)
+    if (ck.peer) {
+      // hcms_dist: tensor t, chunk c, destination rank p -> that rank's [rows][h_c][D] slice for THIS rank's tokens
+      // (ck.peer[(t * C + c) * P + p], a.M rows: rows past the shard are clipped by the map)
+      if (kMode != kFusedOut || n_tensors * ck.C * ck.P > 3 * kMaxChunks) return cudaErrorInvalidValue;
+      for (int i = 0; i < n_tensors * ck.C * ck.P; ++i) {
+        const int c = (i / ck.P) % ck.C;
+        const uint64_t dims[4] = {static_cast<uint64_t>(a.D), static_cast<uint64_t>(ck.h[c]), static_cast<uint64_t>(a.M), 1};
+        const uint64_t strides[3] = {static_cast<uint64_t>(a.D) * 2, static_cast<uint64_t>(ck.h[c]) * a.D * 2,
+                                     static_cast<uint64_t>(a.M) * ck.h[c] * a.D * 2};
+        const uint32_t box[4] = {64, 1, kBM, 1};
+        e = encode_tensor_map(a.cache, &cmaps.m[i], CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, ck.peer[i], dims, strides, box,
+                              CU_TENSOR_MAP_SWIZZLE_128B);
+        if (e != cudaSuccess) return e;
+      }
+    }
+    for (int t = 0; t < n_tensors && !ck.peer; ++t)
       for (int c = 0; c < ck.C; ++c) {
         const uint64_t dims[4] = {static_cast<uint64_t>(a.D), static_cast<uint64_t>(ck.h[c]), static_cast<uint64_t>(a.M),
                                   static_cast<uint64_t>(ck.P)};
@@ -574,6 +594,8 @@ cudaError_t launch(const GemmArgs& a, cudaStream_t stream) {
       }
     p.Hl = ck.Hl;
     p.C = ck.C;
+    p.peer_n = ck.peer ? ck.P : 1;
+    p.peer_on = ck.peer ? 1 : 0;
     for (int c = 0; c < ck.C; ++c)
       for (int j = 0; j < ck.h[c]; ++j) {
         p.chunk_of[ck.o[c] + j] = static_cast<uint8_t>(c);

@@ -90,6 +90,7 @@ struct hcms_dist_plan {
   cudaEvent_t e_main = nullptr, e_fin[2] = {nullptr, nullptr};
   TmapCache tmaps;
   int last_launches = 0;
+  int num_sms = 0;
 };
 
 static void dist_free(hcms_dist_plan_t* p) {
@@ -139,6 +140,7 @@ int hcms_dist_plan(hcms_dist_plan_t** out, int64_t S, int H, int D, int P, int C
   p->rank = rank;
   p->flags = flags;
   p->device = dev;
+  p->num_sms = sms;
   p->Sl = S / P;
   p->chunks.resize(C);
   std::vector<int> o(C), h(C);
@@ -290,6 +292,11 @@ struct RankCall {           // one rank's arguments of a forward call
   void* out;
   cudaStream_t caller;
   uint32_t epoch;
+  // hcms_dist_layer_forward: the input all-to-all is the QKV projection's epilogue, the output projection reads the
+  // assembled output from the exchange block (q, k, v, out above are unused)
+  const void *x = nullptr, *w_qkv = nullptr, *w_o = nullptr, *rope_cos = nullptr, *rope_sin = nullptr;
+  void* y = nullptr;
+  int Dm = 0;
 };
 
 int check_call(const RankCall& rc, float scale) {
@@ -369,9 +376,46 @@ int enqueue_phase(const RankCall& rc, int phase, float scale) {
     cuda(cudaStreamWaitEvent(plan->s_comm, plan->e_main, 0), "wait E_main");
     cuda(cudaStreamWaitEvent(plan->s_comp, plan->e_main, 0), "wait E_main");
     // lines 8-11: input all-to-all of every chunk = stores into the peers' chunk buffers, then E_c^comm as a flag
-    for (int c = 0; c < C && status == HCMS_OK; ++c) {
-      const void* src[3] = {rc.q, rc.k, rc.v};
-      if (layout(c, false, 3, src, plan->s_comm)) signal(0, c, plan->s_comm);
+    if (rc.x) {
+      // Alg. 1 lines 2-3 and 8 in ONE kernel: the projection GEMM's epilogue (RoPE, bf16) TMA-stores every 128 x 64 panel
+      // of q, k, v into the chunk buffer of the rank that owns its head -- peer memory; then E_c^comm for every chunk
+      std::vector<void*> peers(static_cast<size_t>(3) * C * P);
+      GemmChunks ck{};
+      ck.C = C;
+      ck.Hl = sh.Hl;
+      ck.P = P;
+      for (int c = 0; c < C; ++c) {
+        ck.o[c] = plan->chunks[c].o;
+        ck.h[c] = plan->chunks[c].h;
+        for (int t = 0; t < 3; ++t)
+          for (int p = 0; p < P; ++p)
+            peers[(static_cast<size_t>(t) * C + c) * P + p] =
+                plan->peer[p] + plan->chunks[c].off[t] + static_cast<size_t>(r) * plan->Sl * ck.h[c] * sh.D * sh.es;
+      }
+      ck.peer = peers.data();
+      GemmArgs g{};
+      g.a = rc.x;
+      g.b = rc.w_qkv;
+      g.M = plan->Sl;
+      g.N = 3 * sh.H * sh.D;
+      g.K = rc.Dm;
+      g.n_per_out = sh.H * sh.D;
+      g.rope_outs = rc.rope_cos ? 2 : 0;
+      g.D = sh.D;
+      g.cos = static_cast<const float*>(rc.rope_cos);
+      g.sin = static_cast<const float*>(rc.rope_sin);
+      g.num_sms = plan->num_sms;
+      g.fuse = 1;
+      g.chunks = &ck;
+      g.cache = &plan->tmaps;
+      plan->last_launches += 1;
+      if (cuda(launch_gemm(g, plan->s_comm), "QKV projection with the fused push"))
+        for (int c = 0; c < C && status == HCMS_OK; ++c) signal(0, c, plan->s_comm);
+    } else {
+      for (int c = 0; c < C && status == HCMS_OK; ++c) {
+        const void* src[3] = {rc.q, rc.k, rc.v};
+        if (layout(c, false, 3, src, plan->s_comm)) signal(0, c, plan->s_comm);
+      }
     }
   } else if (phase == 1) {
     // lines 14-18: attention of this rank's heads of chunk c once every rank's slice has arrived (Eq. 6)
@@ -402,9 +446,24 @@ int enqueue_phase(const RankCall& rc, int phase, float scale) {
       const void* dst[1] = {rc.out};
       layout(c, true, 1, dst, plan->s_comm);
     }
-    if (plan->out_bytes && status == HCMS_OK)       // Concat (line 26): the assembled output leaves the exchange block
+    if (plan->out_bytes && status == HCMS_OK && !rc.x)   // Concat (line 26): the assembled output leaves the exchange block
       cuda(cudaMemcpyAsync(rc.out, plan->block + plan->out_off + plan->out_pad, plan->out_bytes, cudaMemcpyDeviceToDevice, plan->s_comm),
            "copy of the assembled output");
+    if (rc.x && status == HCMS_OK) {                     // line 27: y = o W_o^T on the assembled [Sl, H*D] output, in place
+      GemmArgs g{};
+      g.a = plan->block + plan->out_off + plan->out_pad;
+      g.b = rc.w_o;
+      g.out[0] = rc.y;
+      g.M = plan->Sl;
+      g.N = rc.Dm;
+      g.K = sh.H * sh.D;
+      g.n_per_out = rc.Dm;
+      g.D = sh.D;
+      g.num_sms = plan->num_sms;
+      g.cache = &plan->tmaps;
+      plan->last_launches += 1;
+      cuda(launch_gemm(g, plan->s_comm), "output projection");
+    }
     // line 25, on every path
     cudaStream_t forked[2] = {plan->s_comm, plan->s_comp};
     const int keep = status;
@@ -462,6 +521,76 @@ int hcms_dist_attention_forward_group(hcms_dist_plan_t* const* plans, int n, con
   for (int phase = 0; phase < 3; ++phase)
     for (int r = 0; r < n; ++r) {
       if (st != HCMS_OK && phase < 2) continue;      // after a failure only the joins still run
+      cudaSetDevice(plans[r]->device);
+      const int s = enqueue_phase(rc[r], phase, scale);
+      if (s != HCMS_OK && st == HCMS_OK) st = s;
+    }
+  if (prev >= 0) cudaSetDevice(prev);
+  return st;
+}
+
+// ---- the whole layer between real ranks: both all-to-alls inside compute kernels -------------------------------
+static int check_layer_call(const RankCall& rc, float scale) {
+  hcms_dist_plan_t* plan = rc.plan;
+  if (!plan || !rc.x || !rc.w_qkv || !rc.w_o || !rc.y) return fail(HCMS_ERR_INVALID_ARG, "NULL argument");
+  if (!plan->attached) return fail(HCMS_ERR_INVALID_ARG, "the plan has not been attached to its peers");
+  if (!plan->out_bytes) return fail(HCMS_ERR_INVALID_ARG, "hcms_dist_layer_forward needs a plan made with HCMS_FLAG_DIST_FUSE_OUT");
+  if ((rc.rope_cos == nullptr) != (rc.rope_sin == nullptr)) return fail(HCMS_ERR_INVALID_ARG, "pass both RoPE tables or neither");
+  int st = check_scale(scale);
+  if (st) return st;
+  const Shape& sh = plan->sh;
+  if (rc.Dm <= 0 || rc.Dm % 128 || (sh.H * sh.D) % 128)
+    return fail(HCMS_ERR_UNSUPPORTED_SHAPE, "Dm=%d and H*D=%d must be multiples of 128", rc.Dm, sh.H * sh.D);
+  if (3 * sh.C * sh.P > 48 || sh.Hl > 64)
+    return fail(HCMS_ERR_UNSUPPORTED_SHAPE, "the fused push holds 48 tensor maps: 3*C*P = %d (C=%d, P=%d); H/P=%d must be <= 64",
+                3 * sh.C * sh.P, sh.C, sh.P, sh.Hl);
+  for (const void* ptr : {rc.x, rc.w_qkv, rc.w_o, rc.rope_cos, rc.rope_sin, static_cast<const void*>(rc.y)})
+    if (!aligned16(ptr)) return fail(HCMS_ERR_MISALIGNED, "every pointer must be 16-byte aligned");
+  return HCMS_OK;
+}
+
+int hcms_dist_layer_forward(hcms_dist_plan_t* plan, const void* x, const void* w_qkv, const void* w_o, const void* rope_cos,
+                            const void* rope_sin, void* y, int Dm, float scale, void* stream) {
+  RankCall rc{plan, nullptr, nullptr, nullptr, nullptr, static_cast<cudaStream_t>(stream), 0};
+  rc.x = x; rc.w_qkv = w_qkv; rc.w_o = w_o; rc.rope_cos = rope_cos; rc.rope_sin = rope_sin; rc.y = y; rc.Dm = Dm;
+  int st = check_layer_call(rc, scale);
+  if (st) return st;
+  if (plan->local)
+    return fail(HCMS_ERR_INVALID_ARG, "ranks attached with hcms_dist_attach_local are driven by hcms_dist_layer_forward_group");
+  rc.epoch = ++plan->epoch;
+  for (int phase = 0; phase < 3; ++phase) {
+    const int s = enqueue_phase(rc, phase, scale);
+    if (s != HCMS_OK && st == HCMS_OK) st = s;
+    if (s != HCMS_OK && phase < 2) phase = 1;      // skip to the join
+  }
+  return st;
+}
+
+int hcms_dist_layer_forward_group(hcms_dist_plan_t* const* plans, int n, const void* const* x, const void* w_qkv, const void* w_o,
+                                  const void* const* rope_cos, const void* const* rope_sin, void* const* y, int Dm, float scale,
+                                  void* const* streams) {
+  if (!plans || !x || !y || !streams) return fail(HCMS_ERR_INVALID_ARG, "NULL argument");
+  if (n < 1 || n > kMaxPeers) return fail(HCMS_ERR_INVALID_ARG, "n=%d outside [1,%d]", n, kMaxPeers);
+  RankCall rc[kMaxPeers];
+  for (int r = 0; r < n; ++r) {
+    rc[r] = RankCall{plans[r], nullptr, nullptr, nullptr, nullptr, static_cast<cudaStream_t>(streams[r]), 0};
+    rc[r].x = x[r]; rc[r].w_qkv = w_qkv; rc[r].w_o = w_o; rc[r].y = y[r]; rc[r].Dm = Dm;
+    rc[r].rope_cos = rope_cos ? rope_cos[r] : nullptr;
+    rc[r].rope_sin = rope_sin ? rope_sin[r] : nullptr;
+    int st = check_layer_call(rc[r], scale);
+    if (st) return st;
+    if (plans[r]->sh.P != n || plans[r]->rank != r)
+      return fail(HCMS_ERR_PLAN_MISMATCH, "plans[%d] is rank %d of %d: pass all P plans in rank order", r, plans[r]->rank, plans[r]->sh.P);
+    for (int o = 0; o < r; ++o)
+      if (rc[o].caller == rc[r].caller) return fail(HCMS_ERR_INVALID_ARG, "ranks %d and %d share a caller stream", o, r);
+  }
+  int prev = -1;
+  cudaGetDevice(&prev);
+  for (int r = 0; r < n; ++r) rc[r].epoch = ++plans[r]->epoch;
+  int st = HCMS_OK;
+  for (int phase = 0; phase < 3; ++phase)
+    for (int r = 0; r < n; ++r) {
+      if (st != HCMS_OK && phase < 2) continue;
       cudaSetDevice(plans[r]->device);
       const int s = enqueue_phase(rc[r], phase, scale);
       if (s != HCMS_OK && st == HCMS_OK) st = s;

@@ -36,9 +36,9 @@ def _emulation(q, k, v, S, Hh, D, P, C, scale):
     return to_host(out)
 
 
-def _run_worker(mode, P, S, Hh, D, C, env=None, flags=0):
+def _run_worker(mode, P, S, Hh, D, C, env=None, flags=0, layer=0):
     cmd = [sys.executable, os.path.join(ROOT, "tests", "dist_worker.py"), mode, str(P), "--S", str(S), "--H", str(Hh),
-           "--D", str(D), "--C", str(C), "--flags", str(flags)]
+           "--D", str(D), "--C", str(C), "--flags", str(flags), "--layer", str(layer)]
     r = subprocess.run(cmd, capture_output=True, text=True, timeout=240, cwd=ROOT, env=dict(os.environ, **(env or {})))
     assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-3000:]
     assert "DIST_OK" in r.stdout, r.stdout[-2000:]
@@ -122,3 +122,19 @@ def test_fused_output_push_with_pairs_in_one_process():
 @pytest.mark.parametrize("P,C", [(2, 2), (4, 1)])
 def test_fused_output_push_as_processes_over_cuda_ipc(P, C):
     _run_worker("--spawn", P, 1024, 8, 128, C, flags=H.HCMS_FLAG_DIST_FUSE_OUT)
+
+
+# ---------------------------------------------------------------------------------------------
+# hcms_dist_layer_forward: QKV projection -> (push in its epilogue) -> attention -> (push in its epilogue) -> output projection
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("S,Hh,D,P,C", [(1024, 4, 64, 2, 2), (2040, 12, 128, 4, 3), (768, 6, 128, 3, 2), (640, 8, 64, 1, 2)])
+def test_layer_between_ranks_in_one_process_bit_equal(S, Hh, D, P, C):
+    """Both all-to-alls inside compute kernels: the concatenated y of the ranks equals hcms_layer_forward bit for bit
+    (shards whose length is not a multiple of the 128-row GEMM tile included: 510, 256, 640 tokens per rank)."""
+    _run_worker("--local", P, S, Hh, D, C, layer=1)
+
+
+@pytest.mark.parametrize("P,C", [(2, 2), (4, 1)])
+def test_layer_between_processes_over_cuda_ipc(P, C):
+    _run_worker("--spawn", P, 1024, 8, 128, C, layer=1)
