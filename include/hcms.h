@@ -477,7 +477,7 @@ void* hcms_plan_lse(const hcms_plan_t* plan);
  * each 128 x 64 panel of q, k, v into the chunk buffer of the rank that owns its head (input all-to-all, peer memory); the
  * attention epilogue stores into the destination ranks' outputs (output all-to-all); the output projection reads the
  * assembled [S/P, H*D] output in place.  C + 2 kernels and 2C signals per rank.  The concatenated y of the P ranks is
- * BIT-EQUAL to hcms_layer_forward on the concatenated x.  Needs 3*C*P <= 48, H/P <= 64, Dm and H*D multiples of 128.
+ * BIT-EQUAL to hcms_layer_forward on the concatenated x.  Needs 3*C*P <= 96, H/P <= 64, Dm and H*D multiples of 128.
  * Errors: INVALID_ARG, UNSUPPORTED_SHAPE (also P > 16), UNSUPPORTED_DTYPE, UNSUPPORTED_DEVICE, PLAN_MISMATCH (handle of
  * another shape / rank order, wrong device), MISALIGNED, ALIAS, CUDA.
  */

@@ -54,9 +54,10 @@ struct alignas(64) GemmMaps {
 // Fused all-to-all (SURVEY 8(f3) "scatter fused into the QKV epilogue"): one rank-4 map {D, h_c, S, P}, box
 // {64, 1, 128, 1}, per (tensor, head chunk) over the head-sharded chunk buffers [P][S][h_c][D] of the plan.
 constexpr int kMaxChunks = 16;
+constexpr int kMaxFusedMaps = 96;   // 3 tensors x 16 chunks on one device, or 3 x C x P <= 96 between real ranks (12 KB of kernel parameters)
 constexpr int kMaxLocalHeads = 64;
 struct alignas(64) ChunkMaps {
-  CUtensorMap m[3 * kMaxChunks];   // [tensor * C + chunk]
+  CUtensorMap m[kMaxFusedMaps];   // [tensor * C + chunk], or [(tensor * C + chunk) * P + destination rank] between real ranks
 };
 enum { kPlain = 0, kFusedOut = 1, kFusedA = 2 };
 
@@ -569,7 +570,7 @@ cudaError_t launch(const GemmArgs& a, cudaStream_t stream) {
     if (ck.peer) {
       // hcms_dist: tensor t, chunk c, destination rank p -> that rank's [rows][h_c][D] slice for THIS rank's tokens
       // (ck.peer[(t * C + c) * P + p], a.M rows: rows past the shard are clipped by the map)
-      if (kMode != kFusedOut || n_tensors * ck.C * ck.P > 3 * kMaxChunks) return cudaErrorInvalidValue;
+      if (kMode != kFusedOut || n_tensors * ck.C * ck.P > kMaxFusedMaps) return cudaErrorInvalidValue;
       for (int i = 0; i < n_tensors * ck.C * ck.P; ++i) {
         const int c = (i / ck.P) % ck.C;
         const uint64_t dims[4] = {static_cast<uint64_t>(a.D), static_cast<uint64_t>(ck.h[c]), static_cast<uint64_t>(a.M), 1};

@@ -541,8 +541,8 @@ static int check_layer_call(const RankCall& rc, float scale) {
   const Shape& sh = plan->sh;
   if (rc.Dm <= 0 || rc.Dm % 128 || (sh.H * sh.D) % 128)
     return fail(HCMS_ERR_UNSUPPORTED_SHAPE, "Dm=%d and H*D=%d must be multiples of 128", rc.Dm, sh.H * sh.D);
-  if (3 * sh.C * sh.P > 48 || sh.Hl > 64)
-    return fail(HCMS_ERR_UNSUPPORTED_SHAPE, "the fused push holds 48 tensor maps: 3*C*P = %d (C=%d, P=%d); H/P=%d must be <= 64",
+  if (3 * sh.C * sh.P > 96 || sh.Hl > 64)
+    return fail(HCMS_ERR_UNSUPPORTED_SHAPE, "the fused push holds 96 tensor maps: 3*C*P = %d (C=%d, P=%d); H/P=%d must be <= 64",
                 3 * sh.C * sh.P, sh.C, sh.P, sh.Hl);
   for (const void* ptr : {rc.x, rc.w_qkv, rc.w_o, rc.rope_cos, rc.rope_sin, static_cast<const void*>(rc.y)})
     if (!aligned16(ptr)) return fail(HCMS_ERR_MISALIGNED, "every pointer must be 16-byte aligned");

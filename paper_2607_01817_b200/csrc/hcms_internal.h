@@ -146,7 +146,7 @@ struct GemmChunks {
   int o[16], h[16];        // Eq. 3 chunk table
   void* base[3][16];       // [tensor][chunk] -> [P][S][h_c][D] bf16 (fuse = 1: Q'_c, K'_c, V'_c; fuse = 2: base[0] = O'_c)
   void* const* peer = nullptr;   // fuse = 1 between real ranks: [(t * C + c) * P + p] -> rank p's [M][h_c][D] rows for this rank's tokens
-                                 // (3 * C * P <= 48 pointers); base is then unused
+                                 // (3 * C * P <= 96 pointers); base is then unused
 };
 struct GemmArgs {
   const void* a;       // [M, K] bf16, row-major

@@ -128,7 +128,8 @@ def test_fused_output_push_as_processes_over_cuda_ipc(P, C):
 # hcms_dist_layer_forward: QKV projection -> (push in its epilogue) -> attention -> (push in its epilogue) -> output projection
 # ---------------------------------------------------------------------------------------------
 
-@pytest.mark.parametrize("S,Hh,D,P,C", [(1024, 4, 64, 2, 2), (2040, 12, 128, 4, 3), (768, 6, 128, 3, 2), (640, 8, 64, 1, 2)])
+@pytest.mark.parametrize("S,Hh,D,P,C", [(1024, 4, 64, 2, 2), (2040, 12, 128, 4, 3), (768, 6, 128, 3, 2), (640, 8, 64, 1, 2),
+                                        (1024, 40, 128, 8, 4)])   # the last: cfg 3's heads on 8 ranks, 3*C*P = 96 maps
 def test_layer_between_ranks_in_one_process_bit_equal(S, Hh, D, P, C):
     """Both all-to-alls inside compute kernels: the concatenated y of the ranks equals hcms_layer_forward bit for bit
     (shards whose length is not a multiple of the 128-row GEMM tile included: 510, 256, 640 tokens per rank)."""
