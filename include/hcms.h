@@ -40,7 +40,7 @@
 extern "C" {
 #endif
 
-#define HCMS_VERSION 400 /* major*10000 + minor*100 + patch */
+#define HCMS_VERSION 500 /* major*10000 + minor*100 + patch */
 
 /* ---- status codes ------------------------------------------------------------------- */
 enum {
