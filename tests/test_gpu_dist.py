@@ -139,3 +139,35 @@ def test_layer_between_ranks_in_one_process_bit_equal(S, Hh, D, P, C):
 @pytest.mark.parametrize("P,C", [(2, 2), (4, 1)])
 def test_layer_between_processes_over_cuda_ipc(P, C):
     _run_worker("--spawn", P, 1024, 8, 128, C, layer=1)
+
+
+def test_dist_layer_argument_errors():
+    S, Hh, D, P, C = 512, 4, 64, 2, 2
+    Dm, Sl = Hh * D, S // P
+    def status(fn):
+        with pytest.raises(H.HcmsError) as ei:
+            fn()
+        return ei.value.status
+    plain = [H.hcms_dist_plan(S, Hh, D, P, C, r) for r in range(P)]
+    fused = [H.hcms_dist_plan(S, Hh, D, P, C, r, H.HCMS_DTYPE_BF16, H.HCMS_FLAG_DIST_FUSE_OUT) for r in range(P)]
+    x = torch.zeros((Sl, Dm), dtype=torch.int16, device=DEV)
+    wq = torch.zeros((3 * Dm, Dm), dtype=torch.int16, device=DEV)
+    wo = torch.zeros((Dm, Dm), dtype=torch.int16, device=DEV)
+    y = torch.zeros_like(x)
+    try:
+        assert status(lambda: H.hcms_dist_layer_forward(fused[0], x, wq, wo, None, None, y, Dm, 0.1)) == H.HCMS_ERR_INVALID_ARG   # not attached
+        for group in (plain, fused):
+            for pl in group:
+                H.hcms_dist_attach_local(pl, group)
+        streams = [torch.cuda.Stream() for _ in range(P)]
+        call = lambda plans, dm=Dm, cos=None: H.hcms_dist_layer_forward_group(plans, [x] * P, wq, wo, cos, None, [y, torch.zeros_like(y)], dm,
+                                                                            0.1, streams)
+        assert status(lambda: call(plain)) == H.HCMS_ERR_INVALID_ARG                 # plan without HCMS_FLAG_DIST_FUSE_OUT
+        assert status(lambda: call(fused, dm=Dm - 64)) == H.HCMS_ERR_UNSUPPORTED_SHAPE
+        assert status(lambda: call(fused, cos=[x, x])) == H.HCMS_ERR_INVALID_ARG     # cos without sin
+        assert status(lambda: H.hcms_dist_layer_forward(fused[0], x, wq, wo, None, None, y, Dm, 0.1)) == H.HCMS_ERR_INVALID_ARG  # local plans: group call
+        call(fused)                                                                   # and the valid call goes through
+        torch.cuda.synchronize()
+    finally:
+        for pl in plain + fused:
+            pl.close()

@@ -341,7 +341,8 @@ def test_recycled_workspace_same_bits_and_smaller(S, Hh, D, P, C):
             assert l0["q_off"] == l2["q_off"] and l0["o_off"] >= l2["o_off"]          # chunk 2 lives in chunk 0's set
         else:
             assert small == full
-    for extra in (0, H.HCMS_FLAG_SERIAL, H.HCMS_FLAG_SINGLE_COMP, H.HCMS_FLAG_GRAPH, H.HCMS_FLAG_LAYOUT_TMA):
+    for extra in (0, H.HCMS_FLAG_SERIAL, H.HCMS_FLAG_SINGLE_COMP, H.HCMS_FLAG_GRAPH, H.HCMS_FLAG_LAYOUT_TMA, H.HCMS_FLAG_PROFILE,
+                  H.HCMS_FLAG_HOST_ROUTE_Q | H.HCMS_FLAG_HOST_ROUTE_O):
         q, k, v = qkv
         out = nan_fill_(torch.empty_like(q))
         with H.hcms_plan(S, Hh, D, P, C, H.HCMS_DTYPE_BF16, R | extra) as plan:
@@ -352,7 +353,7 @@ def test_recycled_workspace_same_bits_and_smaller(S, Hh, D, P, C):
                 nan_fill_(out)
                 H.hcms_attention_forward(plan, q, k, v, out, scale)
             torch.cuda.synchronize()
-            assert H.hcms_plan_last_launch_count(plan) == 3 * C or (extra & H.HCMS_FLAG_GRAPH)
+            assert H.hcms_plan_last_launch_count(plan) == 3 * C or (extra & (H.HCMS_FLAG_GRAPH | H.HCMS_FLAG_HOST_ROUTE_Q))
         assert np.array_equal(to_host(out), ref), hex(extra)
     hq, hk, hv = (to_host(t) for t in qkv)
     hout = np.full_like(hq, 0x7FC0)
