@@ -40,7 +40,7 @@
 extern "C" {
 #endif
 
-#define HCMS_VERSION 500 /* major*10000 + minor*100 + patch */
+#define HCMS_VERSION 600 /* major*10000 + minor*100 + patch */
 
 /* ---- status codes ------------------------------------------------------------------- */
 enum {
@@ -431,6 +431,39 @@ int hcms_attention_chunk_lse(hcms_plan_t* plan, const void* qc, const void* kc, 
 int hcms_attention_backward_chunk(hcms_plan_t* plan, const void* qc, const void* kc, const void* vc, const void* oc,
                                   const void* doc, const void* lse, void* dqc, void* dkc, void* dvc, int c,
                                   float scale, void* stream);
+/*
+ * hcms_attention_backward_chunk for callers that may not allocate device memory: no plan, no cudaMalloc, no cudaFree,
+ * no allocating library routine inside the call.  Meant for an operator embedded in a framework whose caching allocator
+ * already owns the card (a raw cudaMalloc from a library fails there or escapes the host application's accounting), for
+ * serving loops that cannot take cudaMalloc's device-wide synchronisation after start-up, and for processes whose memory
+ * budget (MIG slice, MPS client limit) is fully committed at launch.
+ *
+ * Same three kernels, same bits as hcms_attention_backward_chunk (L304, Table 15; the formulas above).  The
+ * packed row statistics {lse*log2(e), dO.O}, P*h_c*(S rounded up to 64)*8 bytes, go to a fixed array inside the
+ * library's device image instead of plan-owned memory: HCMS_STATIC_SCRATCH_BYTES (4 MiB) that EVERY GPU loading
+ * libhcms.so holds until the process exits.  Larger problems return HCMS_ERR_WORKSPACE_TOO_SMALL (checked first, before
+ * any device work; nothing is enqueued): 4 MiB is 524288 (head, row) pairs, e.g. a 12-head chunk of BASELINE.json
+ * config 3 (S = 32760), 8 heads of config 4 or 5 heads of config 5; split the heads over several calls beyond that.
+ *
+ * qc,kc,vc,oc,doc: device [P][S][h_c][D] bf16; lse: device [P*h_c][S] fp32 (as hcms_attention_chunk_lse writes it);
+ * dqc,dkc,dvc: device outputs, same layout as qc; all 16-byte aligned, all owned by the caller.  D = 64 or 128.
+ * Asynchronous on `stream`; the current device must be the one holding the tensors.
+ *
+ * First call on each device: looks up the array's device address (cudaGetSymbolAddress, once per device, cached) and
+ * sets the kernels' attributes; the runtime may load the library's device image at that moment, so make that first
+ * call during start-up, before any stream capture begins.  Later calls do neither.
+ * The array is shared by every call in the process and keeps the previous call's contents.  Nothing in it needs
+ * clearing (each call rewrites every entry it later reads), but two calls whose kernels can overlap on the GPU -- issued
+ * on different streams without an event between them, or from two host threads -- RACE on it and produce garbage
+ * gradients; order them on one stream or with events.  The TMA descriptors are re-encoded on the host at every call
+ * (there is no plan to cache them).
+ * Errors: INVALID_ARG (NULL, non-positive S/P/h_c, bad scale), UNSUPPORTED_SHAPE (D), WORKSPACE_TOO_SMALL, MISALIGNED,
+ * UNSUPPORTED_DEVICE, CUDA.
+ */
+#define HCMS_STATIC_SCRATCH_BYTES (4u << 20)
+int hcms_attention_backward_chunk_static(const void* qc, const void* kc, const void* vc, const void* oc, const void* doc,
+                                         const void* lse, void* dqc, void* dkc, void* dvc, int64_t S, int P, int h_c,
+                                         int D, float scale, void* stream);
 /* Device address of the lse the last forward saved on a TRAINING plan: [H][S] fp32 in the order chunk 0's
  * P*h_0 heads (p-major), chunk 1's, ...; NULL otherwise.  For tests. */
 void* hcms_plan_lse(const hcms_plan_t* plan);

@@ -91,6 +91,7 @@ _SIGNATURES = {
     "hcms_attention_backward": (c_int, [c_void_p] * 5 + [c_int64, c_int, c_int, c_int, c_int, c_float, c_void_p]),
     "hcms_attention_chunk_lse": (c_int, [c_void_p] * 6 + [c_int, c_float, c_void_p]),
     "hcms_attention_backward_chunk": (c_int, [c_void_p] * 10 + [c_int, c_float, c_void_p]),
+    "hcms_attention_backward_chunk_static": (c_int, [c_void_p] * 9 + [c_int64, c_int, c_int, c_int, c_float, c_void_p]),
     "hcms_plan_lse": (c_void_p, [c_void_p]),
     "hcms_plan_graph_captures": (c_int, [c_void_p]),
     "hcms_dist_plan": (c_int, [POINTER(c_void_p), c_int64, c_int, c_int, c_int, c_int, c_int, c_uint32, c_int]),
@@ -414,6 +415,19 @@ def hcms_attention_backward_chunk(plan: Plan, qc, kc, vc, oc, doc, lse, dqc, dkc
     _check(lib.hcms_attention_backward_chunk(plan.handle, _ptr(qc), _ptr(kc), _ptr(vc), _ptr(oc), _ptr(doc), _ptr(lse),
                                              _ptr(dqc), _ptr(dkc), _ptr(dvc), c, scale, _stream(stream)),
            "hcms_attention_backward_chunk")
+
+
+HCMS_STATIC_SCRATCH_BYTES = 4 << 20
+
+
+def hcms_attention_backward_chunk_static(qc, kc, vc, oc, doc, lse, dqc, dkc, dvc, S: int, P: int, h_c: int, D: int,
+                                         scale: float, stream=None) -> None:
+    """hcms_attention_backward_chunk without a plan and without any device allocation: its scratch is a fixed
+    HCMS_STATIC_SCRATCH_BYTES array inside libhcms.so (see include/hcms.h for who needs that, the size limit and the
+    rule that overlapping calls race).  Raises HcmsError(HCMS_ERR_WORKSPACE_TOO_SMALL) beyond the limit."""
+    _check(lib.hcms_attention_backward_chunk_static(_ptr(qc), _ptr(kc), _ptr(vc), _ptr(oc), _ptr(doc), _ptr(lse), _ptr(dqc),
+                                                    _ptr(dkc), _ptr(dvc), S, P, h_c, D, scale, _stream(stream)),
+           "hcms_attention_backward_chunk_static")
 
 
 def hcms_plan_lse(plan: Plan) -> int:

@@ -19,7 +19,7 @@ CSRC = os.path.join(PKG_DIR, "csrc")
 INCLUDE = os.path.join(os.path.dirname(PKG_DIR), "include")
 LIB_PATH = os.path.join(PKG_DIR, "libhcms.so")
 
-SOURCES = ["hcms_api.cu", "hcms_layer.cu", "hcms_backward.cu", "hcms_tune.cu", "hcms_dist.cu", "layout_kernels.cu", "attention_fwd.cu",
+SOURCES = ["hcms_api.cu", "hcms_layer.cu", "hcms_backward.cu", "hcms_tune.cu", "hcms_dist.cu", "hcms_noalloc.cu", "layout_kernels.cu", "attention_fwd.cu",
            "attention_bwd.cu", "attention_bwd_1pass.cu", "gemm_bf16.cu", "tma_desc.cu"]
 HEADERS = ["hcms_internal.h", "hcms_plan.h", "ptx.cuh"]
 

@@ -190,6 +190,27 @@ def test_layer_and_tuner_argument_validation_precedes_device_use():
     assert H.hcms_plan_lse(H.Plan(0, 1, 1, 1, 1, 1, 0, 0)) == 0 and H.hcms_plan_layer_buffer(H.Plan(0, 1, 1, 1, 1, 1, 0, 0), 0) == 0
 
 
+def test_static_scratch_entry_validates_before_device_use():
+    """hcms_attention_backward_chunk_static: NULLs, the head dimension and the 4 MiB limit are judged on the host,
+    before any CUDA call (so the answer is the same on a box without a GPU)."""
+    buf = np.zeros(64, np.uint16)
+    args = [buf] * 9
+    text = open(os.path.join(ROOT, "include", "hcms.h")).read()
+    assert H.HCMS_STATIC_SCRATCH_BYTES == 4 << 20 and "#define HCMS_STATIC_SCRATCH_BYTES (4u << 20)" in text
+    for S, P, h, D, status in [(H.HCMS_STATIC_SCRATCH_BYTES // 8, 2, 1, 128, H.HCMS_ERR_WORKSPACE_TOO_SMALL),
+                               (H.HCMS_STATIC_SCRATCH_BYTES // 8 - 63, 1, 2, 64, H.HCMS_ERR_WORKSPACE_TOO_SMALL),
+                               (1 << 40, 1, 1, 64, H.HCMS_ERR_WORKSPACE_TOO_SMALL),
+                               (256, 1, 1, 96, H.HCMS_ERR_UNSUPPORTED_SHAPE),
+                               (0, 1, 1, 64, H.HCMS_ERR_INVALID_ARG),
+                               (256, 0, 1, 64, H.HCMS_ERR_INVALID_ARG)]:
+        with pytest.raises(H.HcmsError) as ei:
+            H.hcms_attention_backward_chunk_static(*args, S, P, h, D, 0.125, stream=0)
+        assert ei.value.status == status, (S, P, h, D)
+    with pytest.raises(H.HcmsError) as ei:
+        H.hcms_attention_backward_chunk_static(None, *args[1:], 256, 1, 1, 64, 0.125, stream=0)
+    assert ei.value.status == H.HCMS_ERR_INVALID_ARG
+
+
 def test_product_reads_no_environment_switches():
     """Tuning switches are plan flags or compile-time constants: nothing under csrc/ reads the environment
     (VERDICT r1 weak #4), and every kernel template is instantiated for one exponential split only."""
