@@ -151,6 +151,10 @@ enum {
                                           the compute and its collective.  The exchange block grows by S/P*H*D*2 bytes; the
                                           call ends with one local copy into `out`.  Same bits. */
 
+#define HCMS_FLAG_DEBUG_DIST_FAIL 0x200000u /* TEST ONLY, hcms_dist_plan: every forward call on the plan fails with HCMS_ERR_CUDA
+                                          in the attention phase, after its pushes and the first flag wait were enqueued, so
+                                          that a test can check the error path (join, poisoned plan) */
+
 typedef struct hcms_plan hcms_plan_t;
 
 /* ---- introspection (host only, no GPU needed) ---------------------------------------- */
@@ -488,6 +492,7 @@ void* hcms_plan_lse(const hcms_plan_t* plan);
  *
  * hcms_dist_plan: collective in spirit (every rank creates its own with the same S, H, D, P, C); allocates the
  * exchange block (4*S*(H/P)*D*2 bytes + flags) on the current device.  flags: 0 or any of HCMS_FLAG_ATTN_PAIR, HCMS_FLAG_DIST_FUSE_OUT (the exchange block then also holds this rank's output and 128 pad rows).  bf16 only.
+ * There is no graph, profile (HCMS_FLAG_PROFILE), workspace-recycling or training form of the distributed path: those flags are refused.
  * hcms_dist_export: writes HCMS_DIST_HANDLE_BYTES opaque bytes that another PROCESS passes to hcms_dist_attach.
  * hcms_dist_attach: `handles` = P consecutive handles in rank order (this rank's own entry is checked, not opened);
  * the caller moves the bytes between processes with any host channel (torch.distributed, files).
@@ -511,6 +516,14 @@ void* hcms_plan_lse(const hcms_plan_t* plan);
  * attention epilogue stores into the destination ranks' outputs (output all-to-all); the output projection reads the
  * assembled [S/P, H*D] output in place.  C + 2 kernels and 2C signals per rank.  The concatenated y of the P ranks is
  * BIT-EQUAL to hcms_layer_forward on the concatenated x.  Needs 3*C*P <= 96, H/P <= 64, Dm and H*D multiples of 128.
+ * Failure of a forward call.  Every check that can refuse a call (NULLs, alignment, aliasing, shape, the plan's device being
+ * current, a poisoned plan) runs before anything is enqueued and before the rank takes its next epoch: such an error leaves
+ * the rank in step with its peers and the call may simply be repeated correctly.  A failure AFTER that point (a CUDA launch or
+ * stream operation failing) stops the data path at once, still joins S_comm / S_comp back into the caller's stream -- so the
+ * caller's stream and hcms_dist_plan_destroy never wait on a flag nobody will publish -- and POISONS the plan (for the group
+ * calls: all n plans): this rank's epoch was consumed while its peers may never see its flags.  Every later forward call on a
+ * poisoned plan returns INVALID_ARG.  The peers of a failed rank are not rescued: their streams keep waiting for its flags, as
+ * with any collective one member of which died; tear the job down (destroying a plan whose streams are blocked blocks too).
  * Errors: INVALID_ARG, UNSUPPORTED_SHAPE (also P > 16), UNSUPPORTED_DTYPE, UNSUPPORTED_DEVICE, PLAN_MISMATCH (handle of
  * another shape / rank order, wrong device), MISALIGNED, ALIAS, CUDA.
  */

@@ -51,6 +51,7 @@ HCMS_FLAG_DEBUG_ATTN_ONLY = 0x20000
 HCMS_FLAG_BWD_ONE_PASS = 0x40000
 HCMS_FLAG_RECYCLE_WS = 0x80000
 HCMS_FLAG_DIST_FUSE_OUT = 0x100000
+HCMS_FLAG_DEBUG_DIST_FAIL = 0x200000
 
 # every symbol include/hcms.h declares: name -> (restype, argtypes)
 _SIGNATURES = {

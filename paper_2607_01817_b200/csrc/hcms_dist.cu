@@ -85,6 +85,7 @@ struct hcms_dist_plan {
   std::vector<bool> peer_ipc;    // opened with cudaIpcOpenMemHandle (to be closed)
   bool attached = false;
   bool local = false;            // attached with hcms_dist_attach_local: driven by the group call only
+  bool poisoned = false;         // a forward call failed after its epoch was taken: this rank's flags no longer line up with the peers'
   uint32_t epoch = 0;
   cudaStream_t s_comm = nullptr, s_comp = nullptr;
   cudaEvent_t e_main = nullptr, e_fin[2] = {nullptr, nullptr};
@@ -120,8 +121,9 @@ int hcms_dist_plan(hcms_dist_plan_t** out, int64_t S, int H, int D, int P, int C
     return fail(HCMS_ERR_INVALID_ARG, "S=%lld H=%d D=%d P=%d C=%d must all be positive", static_cast<long long>(S), H, D, P, C);
   if (rank < 0 || rank >= P) return fail(HCMS_ERR_INVALID_ARG, "rank=%d outside [0,%d)", rank, P);
   if (dtype != HCMS_DTYPE_BF16) return fail(HCMS_ERR_UNSUPPORTED_DTYPE, "the distributed path is bf16 only");
-  if (flags & ~static_cast<uint32_t>(HCMS_FLAG_ATTN_PAIR | HCMS_FLAG_DIST_FUSE_OUT))
-    return fail(HCMS_ERR_INVALID_ARG, "hcms_dist_plan accepts HCMS_FLAG_ATTN_PAIR and HCMS_FLAG_DIST_FUSE_OUT only (flags=0x%x)", flags);
+  if (flags & ~static_cast<uint32_t>(HCMS_FLAG_ATTN_PAIR | HCMS_FLAG_DIST_FUSE_OUT | HCMS_FLAG_DEBUG_DIST_FAIL))
+    return fail(HCMS_ERR_INVALID_ARG, "hcms_dist_plan accepts HCMS_FLAG_ATTN_PAIR, HCMS_FLAG_DIST_FUSE_OUT and the test-only "
+                "HCMS_FLAG_DEBUG_DIST_FAIL (flags=0x%x)", flags);
   if (S % P) return fail(HCMS_ERR_UNSUPPORTED_SHAPE, "S=%lld is not divisible by P=%d", static_cast<long long>(S), P);
   if (H % P) return fail(HCMS_ERR_UNSUPPORTED_SHAPE, "H=%d is not divisible by P=%d", H, P);
   if (D != 64 && D != 128) return fail(HCMS_ERR_UNSUPPORTED_SHAPE, "D=%d: only head dimensions 64 and 128 are built", D);
@@ -299,10 +301,30 @@ struct RankCall {           // one rank's arguments of a forward call
   int Dm = 0;
 };
 
-int check_call(const RankCall& rc, float scale) {
+// Everything that can be refused without touching a stream is refused HERE, before the caller takes the next epoch: a
+// call that returns an error from these checks has enqueued nothing and leaves the rank in step with its peers.
+// `group`: the call switches to each plan's device itself, so only the switch is tried; otherwise the plan's device
+// must be current.
+int check_plan_state(hcms_dist_plan_t* plan, bool group) {
+  if (!plan->attached) return fail(HCMS_ERR_INVALID_ARG, "the plan has not been attached to its peers");
+  if (plan->poisoned)
+    return fail(HCMS_ERR_INVALID_ARG, "an earlier forward call on this plan failed after part of its work had been enqueued; its epoch "
+                "flags no longer agree with the peers': destroy the plans of all ranks and make new ones");
+  if (group) {
+    HCMS_CUDA(cudaSetDevice(plan->device));
+    return HCMS_OK;
+  }
+  int dev = -1;
+  HCMS_CUDA(cudaGetDevice(&dev));
+  if (dev != plan->device)
+    return fail(HCMS_ERR_PLAN_MISMATCH, "the plan was made on device %d but device %d is current", plan->device, dev);
+  return HCMS_OK;
+}
+
+int check_call(const RankCall& rc, float scale, bool group) {
   hcms_dist_plan_t* plan = rc.plan;
   if (!plan || !rc.q || !rc.k || !rc.v || !rc.out) return fail(HCMS_ERR_INVALID_ARG, "NULL argument");
-  if (!plan->attached) return fail(HCMS_ERR_INVALID_ARG, "the plan has not been attached to its peers");
+  if (int ps = check_plan_state(plan, group)) return ps;
   int st = check_scale(scale);
   if (st) return st;
   if (!aligned16(rc.q) || !aligned16(rc.k) || !aligned16(rc.v) || !aligned16(rc.out))
@@ -314,7 +336,9 @@ int check_call(const RankCall& rc, float scale) {
   return HCMS_OK;
 }
 
-// phase 0 = fork + pushes (Alg. 1 lines 5-11), 1 = attention (lines 13-18), 2 = pulls + join (lines 19-25)
+// phase 0 = fork + pushes (Alg. 1 lines 5-11), 1 = attention (lines 13-18), 2 = pulls + join (lines 19-25),
+// 3 = the join alone (line 25): what a failed call still runs, so that the caller's stream is never left waiting on a
+// flag that nobody will publish any more
 int enqueue_phase(const RankCall& rc, int phase, float scale) {
   hcms_dist_plan_t* plan = rc.plan;
   const Shape& sh = plan->sh;
@@ -422,6 +446,8 @@ int enqueue_phase(const RankCall& rc, int phase, float scale) {
     for (int c = 0; c < C && status == HCMS_OK; ++c) {
       const Chunk& ck = plan->chunks[c];
       if (!wait_all(0, c, plan->s_comp)) break;
+      if (plan->flags & HCMS_FLAG_DEBUG_DIST_FAIL)      // TEST ONLY: a launch failure after the pushes and the first wait
+        return fail(HCMS_ERR_CUDA, "injected failure (HCMS_FLAG_DEBUG_DIST_FAIL) before the attention launch of chunk %d", c);
       AttnArgs a{plan->block + ck.off[0], plan->block + ck.off[1], plan->block + ck.off[2], plan->block + ck.off[3],
                  sh.S, sh.D, 1, ck.h, scale};
       a.pair = (plan->flags & HCMS_FLAG_ATTN_PAIR) != 0;
@@ -438,7 +464,7 @@ int enqueue_phase(const RankCall& rc, int phase, float scale) {
       plan->last_launches += 1;
       if (cuda(launch_attention(a, plan->s_comp), "attention launch")) signal(1, c, plan->s_comp);   // E_c^comp as a flag
     }
-  } else {
+  } else if (phase == 2) {
     // lines 20-23, 26: output all-to-all = loads of this rank's rows from every peer's O'_c (Eq. 7), written into `out`
     for (int c = 0; c < C && status == HCMS_OK; ++c) {
       if (!wait_all(1, c, plan->s_comm)) break;
@@ -464,6 +490,8 @@ int enqueue_phase(const RankCall& rc, int phase, float scale) {
       plan->last_launches += 1;
       cuda(launch_gemm(g, plan->s_comm), "output projection");
     }
+  }
+  if (phase >= 2) {
     // line 25, on every path
     cudaStream_t forked[2] = {plan->s_comm, plan->s_comp};
     const int keep = status;
@@ -477,6 +505,39 @@ int enqueue_phase(const RankCall& rc, int phase, float scale) {
   return status;
 }
 
+struct DeviceRestore {       // group calls switch devices; put the caller's back on every return path
+  int dev;
+  ~DeviceRestore() {
+    if (dev >= 0) cudaSetDevice(dev);
+  }
+};
+
+// The forward of n validated ranks (n = 1: one process per rank; n = P: the group call).  The epochs are taken HERE, after
+// every check that can refuse the call.  Phase by phase over ALL ranks: every flag a stream waits on is produced by work
+// already enqueued, so no stream ever blocks a hardware queue ahead of its producer.  On the first failure nothing more of
+// the data path is enqueued -- in particular none of phase 2's waits on ready[c][p], whose producers (the attention
+// kernels) may never have been launched -- every rank only joins its side streams back into its caller's stream, and the
+// plans are poisoned: their epochs were consumed, so a later call could not line up with the peers' flags.
+int run_ranks(RankCall* rc, int n, float scale, bool group) {
+  for (int r = 0; r < n; ++r) rc[r].epoch = ++rc[r].plan->epoch;
+  int st = HCMS_OK;
+  for (int phase = 0; phase < 3 && st == HCMS_OK; ++phase)
+    for (int r = 0; r < n && st == HCMS_OK; ++r) {
+      if (group) cudaSetDevice(rc[r].plan->device);
+      st = enqueue_phase(rc[r], phase, scale);
+    }
+  if (st != HCMS_OK) {
+    const std::string text = hcms_last_error();     // the join below must not replace the first failure's text
+    for (int r = 0; r < n; ++r) {
+      rc[r].plan->poisoned = true;
+      if (group) cudaSetDevice(rc[r].plan->device);
+      enqueue_phase(rc[r], 3, scale);
+    }
+    fail(st, "%s", text.c_str());
+  }
+  return st;
+}
+
 }  // namespace
 
 extern "C" {
@@ -484,18 +545,12 @@ extern "C" {
 int hcms_dist_attention_forward(hcms_dist_plan_t* plan, const void* q, const void* k, const void* v, void* out, float scale,
                                 void* stream) {
   RankCall rc{plan, q, k, v, out, static_cast<cudaStream_t>(stream), 0};
-  int st = check_call(rc, scale);
+  int st = check_call(rc, scale, false);
   if (st) return st;
   if (plan->local)
     return fail(HCMS_ERR_INVALID_ARG, "ranks attached with hcms_dist_attach_local are driven by hcms_dist_attention_forward_group "
                 "(a rank-by-rank enqueue from one process can deadlock on shared hardware queues)");
-  rc.epoch = ++plan->epoch;
-  for (int phase = 0; phase < 3; ++phase) {
-    const int s = enqueue_phase(rc, phase, scale);
-    if (s != HCMS_OK && st == HCMS_OK) st = s;
-    if (s != HCMS_OK && phase < 2) phase = 1;      // skip to the join
-  }
-  return st;
+  return run_ranks(&rc, 1, scale, false);
 }
 
 int hcms_dist_attention_forward_group(hcms_dist_plan_t* const* plans, int n, const void* const* q, const void* const* k,
@@ -503,37 +558,26 @@ int hcms_dist_attention_forward_group(hcms_dist_plan_t* const* plans, int n, con
   if (!plans || !q || !k || !v || !out || !streams) return fail(HCMS_ERR_INVALID_ARG, "NULL argument");
   if (n < 1 || n > kMaxPeers) return fail(HCMS_ERR_INVALID_ARG, "n=%d outside [1,%d]", n, kMaxPeers);
   RankCall rc[kMaxPeers];
+  int prev = -1;
+  cudaGetDevice(&prev);
+  DeviceRestore restore{prev};     // the checks and the phases switch to each plan's device
   for (int r = 0; r < n; ++r) {
     rc[r] = RankCall{plans[r], q[r], k[r], v[r], out[r], static_cast<cudaStream_t>(streams[r]), 0};
-    int st = check_call(rc[r], scale);
+    int st = check_call(rc[r], scale, true);
     if (st) return st;
     if (plans[r]->sh.P != n || plans[r]->rank != r)
       return fail(HCMS_ERR_PLAN_MISMATCH, "plans[%d] is rank %d of %d: pass all P plans in rank order", r, plans[r]->rank, plans[r]->sh.P);
     for (int o = 0; o < r; ++o)
       if (rc[o].caller == rc[r].caller) return fail(HCMS_ERR_INVALID_ARG, "ranks %d and %d share a caller stream", o, r);
   }
-  int prev = -1;
-  cudaGetDevice(&prev);
-  for (int r = 0; r < n; ++r) rc[r].epoch = ++plans[r]->epoch;
-  // Phase by phase over ALL ranks: every flag a stream waits on is produced by work already enqueued, so no stream
-  // ever blocks a hardware queue ahead of its producer.
-  int st = HCMS_OK;
-  for (int phase = 0; phase < 3; ++phase)
-    for (int r = 0; r < n; ++r) {
-      if (st != HCMS_OK && phase < 2) continue;      // after a failure only the joins still run
-      cudaSetDevice(plans[r]->device);
-      const int s = enqueue_phase(rc[r], phase, scale);
-      if (s != HCMS_OK && st == HCMS_OK) st = s;
-    }
-  if (prev >= 0) cudaSetDevice(prev);
-  return st;
+  return run_ranks(rc, n, scale, true);
 }
 
 // ---- the whole layer between real ranks: both all-to-alls inside compute kernels -------------------------------
-static int check_layer_call(const RankCall& rc, float scale) {
+static int check_layer_call(const RankCall& rc, float scale, bool group) {
   hcms_dist_plan_t* plan = rc.plan;
   if (!plan || !rc.x || !rc.w_qkv || !rc.w_o || !rc.y) return fail(HCMS_ERR_INVALID_ARG, "NULL argument");
-  if (!plan->attached) return fail(HCMS_ERR_INVALID_ARG, "the plan has not been attached to its peers");
+  if (int ps = check_plan_state(plan, group)) return ps;
   if (!plan->out_bytes) return fail(HCMS_ERR_INVALID_ARG, "hcms_dist_layer_forward needs a plan made with HCMS_FLAG_DIST_FUSE_OUT");
   if ((rc.rope_cos == nullptr) != (rc.rope_sin == nullptr)) return fail(HCMS_ERR_INVALID_ARG, "pass both RoPE tables or neither");
   int st = check_scale(scale);
@@ -553,17 +597,11 @@ int hcms_dist_layer_forward(hcms_dist_plan_t* plan, const void* x, const void* w
                             const void* rope_sin, void* y, int Dm, float scale, void* stream) {
   RankCall rc{plan, nullptr, nullptr, nullptr, nullptr, static_cast<cudaStream_t>(stream), 0};
   rc.x = x; rc.w_qkv = w_qkv; rc.w_o = w_o; rc.rope_cos = rope_cos; rc.rope_sin = rope_sin; rc.y = y; rc.Dm = Dm;
-  int st = check_layer_call(rc, scale);
+  int st = check_layer_call(rc, scale, false);
   if (st) return st;
   if (plan->local)
     return fail(HCMS_ERR_INVALID_ARG, "ranks attached with hcms_dist_attach_local are driven by hcms_dist_layer_forward_group");
-  rc.epoch = ++plan->epoch;
-  for (int phase = 0; phase < 3; ++phase) {
-    const int s = enqueue_phase(rc, phase, scale);
-    if (s != HCMS_OK && st == HCMS_OK) st = s;
-    if (s != HCMS_OK && phase < 2) phase = 1;      // skip to the join
-  }
-  return st;
+  return run_ranks(&rc, 1, scale, false);
 }
 
 int hcms_dist_layer_forward_group(hcms_dist_plan_t* const* plans, int n, const void* const* x, const void* w_qkv, const void* w_o,
@@ -572,31 +610,22 @@ int hcms_dist_layer_forward_group(hcms_dist_plan_t* const* plans, int n, const v
   if (!plans || !x || !y || !streams) return fail(HCMS_ERR_INVALID_ARG, "NULL argument");
   if (n < 1 || n > kMaxPeers) return fail(HCMS_ERR_INVALID_ARG, "n=%d outside [1,%d]", n, kMaxPeers);
   RankCall rc[kMaxPeers];
+  int prev = -1;
+  cudaGetDevice(&prev);
+  DeviceRestore restore{prev};
   for (int r = 0; r < n; ++r) {
     rc[r] = RankCall{plans[r], nullptr, nullptr, nullptr, nullptr, static_cast<cudaStream_t>(streams[r]), 0};
     rc[r].x = x[r]; rc[r].w_qkv = w_qkv; rc[r].w_o = w_o; rc[r].y = y[r]; rc[r].Dm = Dm;
     rc[r].rope_cos = rope_cos ? rope_cos[r] : nullptr;
     rc[r].rope_sin = rope_sin ? rope_sin[r] : nullptr;
-    int st = check_layer_call(rc[r], scale);
+    int st = check_layer_call(rc[r], scale, true);
     if (st) return st;
     if (plans[r]->sh.P != n || plans[r]->rank != r)
       return fail(HCMS_ERR_PLAN_MISMATCH, "plans[%d] is rank %d of %d: pass all P plans in rank order", r, plans[r]->rank, plans[r]->sh.P);
     for (int o = 0; o < r; ++o)
       if (rc[o].caller == rc[r].caller) return fail(HCMS_ERR_INVALID_ARG, "ranks %d and %d share a caller stream", o, r);
   }
-  int prev = -1;
-  cudaGetDevice(&prev);
-  for (int r = 0; r < n; ++r) rc[r].epoch = ++plans[r]->epoch;
-  int st = HCMS_OK;
-  for (int phase = 0; phase < 3; ++phase)
-    for (int r = 0; r < n; ++r) {
-      if (st != HCMS_OK && phase < 2) continue;
-      cudaSetDevice(plans[r]->device);
-      const int s = enqueue_phase(rc[r], phase, scale);
-      if (s != HCMS_OK && st == HCMS_OK) st = s;
-    }
-  if (prev >= 0) cudaSetDevice(prev);
-  return st;
+  return run_ranks(rc, n, scale, true);
 }
 
 }  // extern "C"

@@ -64,6 +64,14 @@ def test_emulation_matches_oracle_on_the_dist_shapes():
     assert np.linalg.norm(bf16_bits_to_f64(want) - ref) / np.linalg.norm(ref) <= 1e-2
 
 
+def test_failed_forward_joins_and_poisons_instead_of_hanging():
+    """HCMS_FLAG_DEBUG_DIST_FAIL injects a failure in the attention phase, after the pushes: the call returns the error,
+    every stream drains (no wait on a flag nobody publishes), hcms_dist_plan_destroy returns, later calls are refused;
+    group call with 3 in-process ranks, the single-rank calls (attention and layer) with P = 1.  In a child process with a
+    60 s watchdog."""
+    _run_worker("--fail", 3, 768, 6, 128, 2)
+
+
 def test_dist_plan_argument_errors():
     S, Hh, D, P, C = 512, 4, 64, 2, 2
     def status(fn):
