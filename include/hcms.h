@@ -128,13 +128,18 @@ enum {
                                           compute side of the pipeline can be timed in the same stream arrangement
                                           without copies; the chunk buffers must hold an earlier call's data */
 
-#define HCMS_FLAG_BWD_ONE_PASS 0x40000u  /* D = 128, with HCMS_FLAG_TRAINING: hcms_attention_backward[_chunk] form S = QK^T
-                                          and dP = dO V^T once per (key tile, query tile) instead of once per pass
-                                          (5 executed contractions instead of 7): one kernel keeps dK_j, dV_j in tensor
-                                          memory and adds its dQ partials to an fp32 accumulator in a fixed key-tile
-                                          order (deterministic; gradients still independent of P and C).  Needs
-                                          P*h_max*(S rounded up to 64)*D*4 bytes of scratch, allocated on first use.
-                                          Ignored at D = 64 (the two-pass kernels run). */
+#define HCMS_FLAG_BWD_ONE_PASS 0x40000u  /* D = 128: hcms_attention_backward (HCMS_FLAG_TRAINING plans) and hcms_attention_backward_chunk
+                                          (any bf16 plan) form S = QK^T and dP = dO V^T once per (key tile, query tile) instead
+                                          of once per pass (5 executed contractions instead of 7): one kernel keeps dK_j, dV_j in
+                                          tensor memory and adds its dQ partials to an fp32 accumulator in a fixed key-tile
+                                          order (deterministic; gradients still independent of P and C).  Scratch, allocated on
+                                          first use: TWO accumulators (one per compute stream, chunks alternate) of
+                                          P*h_max*(S rounded up to 64)*D*4 bytes each, h_max = the largest chunk, plus
+                                          2*P*h_max*(S/64 + 1) 4-byte counters -- 2 x 201 MB at BASELINE.json config 3.
+                                          A CTA of this kernel waits for the CTAs of the lower key tiles of its head; each CTA
+                                          draws its key tile from a per-head ticket counter as it starts, so it only ever waits
+                                          for CTAs that are already running (no reliance on blockIdx dispatch order).
+                                          Measured slower than the two-pass default.  Ignored at D = 64. */
 
 #define HCMS_FLAG_RECYCLE_WS 0x80000u    /* chunk c shares its buffers Q'_c, K'_c, V'_c, O'_c with chunk c - 2: the workspace is 2 buffer
                                           sets sized for a largest chunk instead of one set per chunk (2/C of it for even

@@ -26,8 +26,14 @@
 //
 // Order of the dQ reduction: one counter per (head, query tile).  The CTA of key tile j waits until the counter equals
 // j, issues its 64 x 128 reds (tile 0: stores), and sets the counter to j + 1 one step later, after a fence (by then the
-// reds have been performed, so the fence costs its fixed latency only).  CTAs are dispatched in blockIdx order (key tile
-// fastest), so a CTA only ever waits for one that was dispatched before it.
+// reds have been performed, so the fence costs its fixed latency only).
+// Forward progress: a CTA spins on a counter that another CTA of the same launch advances, so that other CTA must already
+// be running.  CUDA does not promise that CTAs start in blockIdx order (another kernel may hold SMs, the two compute
+// streams may each have such a grid in flight, MPS, a debugger), so the key tile is NOT blockIdx.x: every CTA draws a
+// ticket from a per-head counter when it starts (atomicAdd, zeroed with the turn counters) and works on key tile
+// `ticket`.  The CTA of key tile j therefore waits only for CTAs that drew j-1, j-2, ... before it -- CTAs that are
+// resident and waiting on nobody newer -- whatever order the hardware starts them in.  The reduction order (ascending
+// key tile) and with it every bit of dQ is unchanged.
 //
 // MEASURED (cfg 3 backward, one B200, profiles/r2k_bwd_one_pass.md): two-pass kernels 59.2-60.0 ms; this kernel without
 // any dQ output 48.4 ms (the contraction pipeline alone: the 5-vs-7 saving is real), with unordered reds 60.9 ms, with the
@@ -76,6 +82,7 @@ struct Bwd1Params {
   const float2* stats;    // [P*h_c][s_pad]: {lse * log2(e), delta}; rows >= S hold {+inf, 0}
   float* dq_acc;          // [P*h_c][s_pad][D] fp32
   int* dq_turn;           // [P*h_c][n_iter], zero before the launch
+  int* dq_ticket;         // [P*h_c], zero before the launch: next key tile of the head to hand out
 };
 
 __device__ __forceinline__ void st_shared_v4(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
@@ -119,17 +126,19 @@ attention_bwd_1pass_kernel(const __grid_constant__ Bwd1Maps maps, const Bwd1Para
   const uint32_t bar_dq_free = bar_acc + 16;                 // drain -> MMA: dQ^T of step t is in registers
   const uint32_t bar_done = bar_dq_free + 8;                 // MMA -> all: every accumulation has completed
   const uint32_t tmem_slot = bar_done + 8;
+  const uint32_t ticket_slot = tmem_slot + 4;
 
   const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
   const int lane = threadIdx.x & 31;
   const int head = blockIdx.y;                 // p*h_c + j
   const int rank = head / prm.h_c;
   const int hj = head - rank * prm.h_c;
-  const int key_tile = blockIdx.x;
-  const int row0 = key_tile * kRows;
   const int n_iter = prm.n_iter;
 
   if (threadIdx.x == 0) {
+    // the key tile is the order in which this head's CTAs actually start (see "Forward progress" above)
+    const int ticket = atomicAdd(prm.dq_ticket + head, 1);
+    asm volatile("st.shared.u32 [%0], %1;" ::"r"(ticket_slot), "r"(ticket) : "memory");
     mbar_init(bar_r_full, 1);
     for (int b = 0; b < 2; ++b) {
       mbar_init(bar_t_full + 8 * b, 1);
@@ -155,6 +164,9 @@ attention_bwd_1pass_kernel(const __grid_constant__ Bwd1Maps maps, const Bwd1Para
   tc_fence_after();
   uint32_t tmem_base;
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+  int key_tile;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(key_tile) : "r"(ticket_slot));
+  const int row0 = key_tile * kRows;
 
   if (warp < 4) {
     setmaxnreg_dec<56>();
@@ -460,7 +472,7 @@ size_t attention_bwd_1pass_acc_bytes(int64_t S, int heads) {
 }
 size_t attention_bwd_1pass_turn_bytes(int64_t S, int heads) {
   const int64_t s_pad = (S + kQ - 1) / kQ * kQ;
-  return static_cast<size_t>(heads) * (s_pad / kQ) * sizeof(int);
+  return static_cast<size_t>(heads) * (s_pad / kQ + 1) * sizeof(int);     // turn counters, then one ticket counter per head
 }
 
 // After the statistics kernel: zero the turn counters, the single-pass kernel, the dQ conversion (3 stream operations).
@@ -486,6 +498,7 @@ cudaError_t launch_attention_bwd_1pass(const AttnBwdArgs& a, const void* stats, 
   prm.stats = static_cast<const float2*>(stats);
   prm.dq_acc = a.dq_acc;
   prm.dq_turn = a.dq_turn;
+  prm.dq_ticket = a.dq_turn + static_cast<size_t>(heads) * (s_pad / kQ);
   if ((e = cudaMemsetAsync(a.dq_turn, 0, attention_bwd_1pass_turn_bytes(a.S, heads), stream)) != cudaSuccess) return e;
   const dim3 grid(static_cast<unsigned>((a.S + kRows - 1) / kRows), static_cast<unsigned>(heads));
   attention_bwd_1pass_kernel<<<grid, kThreads, kSmemBytes, stream>>>(m, prm);
