@@ -1,5 +1,6 @@
-"""-m gpu: the SURVEY 8(f) rows at BASELINE.json's full cfg 3 size (S=32760, H=40, D=128, P=4, C=4; Dm = 5120), in
-the launch configuration bench.py times, checked on sampled outputs the oracle computes one by one:
+"""-m gpu: the SURVEY 8(f) rows at BASELINE.json's full sizes -- cfg 3 (S=32760, H=40, D=128, P=4, C=4; Dm = 5120), cfg 4
+(S=56160, H=40, P=8, C=2: 5 heads per rank split 3 + 2) and cfg 5 (S=98304, H=24, P=8, C=3: one head per chunk, 768 key
+tiles; Dm = 3072) -- in the launch configuration bench.py times, checked on sampled outputs the oracle computes one by one:
 
 * projections: sampled token rows (tile and shard boundaries + seeded rows) of q, k, v and y;
 * backward: dq on sampled query rows and dk, dv on sampled key rows of sampled heads (one per logical rank pair,
@@ -20,7 +21,7 @@ from gpu_util import DEV, bf16_bits_to_f64, nan_fill_, to_dev, to_host
 
 pytestmark = pytest.mark.gpu
 
-W3 = I.workload(3)
+FULL = pytest.mark.parametrize("cfg", [3, 4, 5], ids=["cfg3", "cfg4", "cfg5"])
 
 
 def dev_out(*shape):
@@ -40,8 +41,9 @@ def check_rounded(got_bits, ref, what):
     assert (err / bound).max() <= 1.0 and rel <= 3e-3, f"{what}: worst={(err / bound).max():.3f} rel_l2={rel:.3e}"
 
 
-def test_projections_cfg3_sampled_rows():
-    w = W3
+@FULL
+def test_projections_sampled_rows(cfg):
+    w = I.workload(cfg)
     S, Hh, D = w.S, w.H, w.D
     Dm = Hh * D
     x, w_qkv, w_o, cos, sin = I.make_layer_inputs(w)
@@ -55,17 +57,24 @@ def test_projections_cfg3_sampled_rows():
         torch.cuda.synchronize()
     ref = L.project_and_rotate(x[rows], w_qkv, cos[rows], sin[rows], Hh, D)
     for name, g, r in zip("qkv", (q, k, v), ref):
-        check_rounded(to_host(g[torch.from_numpy(rows).to(DEV)]), r, f"{name} rows of cfg 3")
-    check_rounded(to_host(y[torch.from_numpy(rows).to(DEV)]), L.output_projection(o_in[rows], w_o), "y rows of cfg 3")
+        check_rounded(to_host(g[torch.from_numpy(rows).to(DEV)]), r, f"{name} rows of cfg {cfg}")
+    check_rounded(to_host(y[torch.from_numpy(rows).to(DEV)]), L.output_projection(o_in[rows], w_o), f"y rows of cfg {cfg}")
     # every element was written (no tile skipped anywhere)
     for t in (q, k, v, y):
         assert not bool((t == 0x7FC0).any())
 
 
-@pytest.mark.parametrize("bwd_flag", [0, H.HCMS_FLAG_BWD_ONE_PASS], ids=["two_pass", "one_pass"])
-def test_forward_backward_cfg3_sampled(bwd_flag):
-    """Full cfg 3 through the chunk pipeline, both backward kernels (the launch configuration bench.py times)."""
-    w = W3
+# (cfg, backward kernel, sampled global heads).  The oracle walks all S queries for every sampled key row, S^2 work per
+# head: two heads at cfg 3 / 4, one at cfg 5.  cfg 4: head 2 = rank 0 chunk 0, head 39 = rank 7 chunk 1 (local head 4);
+# cfg 5: head 16 = rank 5 chunk 1.
+@pytest.mark.parametrize("cfg,bwd_flag,heads", [(3, 0, [2, 27]), (3, H.HCMS_FLAG_BWD_ONE_PASS, [2, 27]), (4, 0, [2, 39]),
+                                                (4, H.HCMS_FLAG_BWD_ONE_PASS, [39]), (5, 0, [16])],
+                         ids=["cfg3-two_pass", "cfg3-one_pass", "cfg4-two_pass", "cfg4-one_pass", "cfg5-two_pass"])
+def test_forward_backward_sampled(cfg, bwd_flag, heads):
+    """Full configs through the chunk pipeline, both backward kernels (the launch configuration bench.py times).  The
+    one-pass runs are also the stress case of its ordered reduction: 256 / 439 key tiles x 12 / 24 heads per launch, far
+    more CTAs than SMs, a grid in flight on each of the two compute streams."""
+    w = I.workload(cfg)
     S, Hh, D, P, C = w.S, w.H, w.D, w.P, w.C
     q, k, v = I.make_qkv(w)
     do = I.f32_to_bf16_bits(I.normal_f32(w.seed, 6, S * Hh * D).reshape(S, Hh, D))
@@ -77,7 +86,7 @@ def test_forward_backward_cfg3_sampled(bwd_flag):
         torch.cuda.synchronize()
     for t in (dq, dk, dv):
         assert not bool((t == 0x7FC0).any()), "a gradient element was never written (or is NaN)"
-    heads = [2, 27]                               # rank 0 chunk 0 (local head 2), rank 2 chunk 2 (local head 7)
+    # cfg 3: head 2 = rank 0 chunk 0 (local head 2), head 27 = rank 2 chunk 2 (local head 7)
     q_rows = rows_sample(S, P, 24, 11)
     k_rows = rows_sample(S, P, 8, 12)
     sub = lambda t: np.ascontiguousarray(t[:, heads, :])
@@ -95,9 +104,10 @@ def test_forward_backward_cfg3_sampled(bwd_flag):
             f"{name}: rel_l2={rel:.3e} max_err={err.max():.3e} max_ref={np.abs(ref).max():.3e}"
 
 
-def test_fused_layer_cfg3_equals_unfused_bitwise():
-    """HCMS_FLAG_FUSE_A2A at the full cfg 3 shape: 6 launches instead of 14, identical y."""
-    w = W3
+@FULL
+def test_fused_layer_equals_unfused_bitwise(cfg):
+    """HCMS_FLAG_FUSE_A2A at the full shapes (cfg 3: 6 launches instead of 14), identical y."""
+    w = I.workload(cfg)
     S, Hh, D = w.S, w.H, w.D
     Dm = Hh * D
     arrs = I.make_layer_inputs(w)
