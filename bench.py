@@ -257,16 +257,16 @@ def time_oracle_full_small(cfg: int) -> dict:
 
 
 def dram_traffic(kernel: str, cfg: int):
-    """DRAM bytes per step of `kernel` from the committed ncu pass (profiles/r2_dram_traffic.csv: config,kernel,
+    """DRAM bytes per step of `kernel` from the committed ncu pass (profiles/dram_traffic.csv: config,kernel,
     launches_per_step,dram_bytes_per_step,commit,source), or (None, None) when no row exists for this config."""
-    path = os.path.join(ROOT, "profiles", "r2_dram_traffic.csv")
+    path = os.path.join(ROOT, "profiles", "dram_traffic.csv")
     if not os.path.exists(path):
         return None, None
     with open(path) as f:
         for line in f:
             cells = [c.strip() for c in line.split(",")]
             if len(cells) >= 6 and cells[0] == str(cfg) and cells[1] == kernel:
-                return float(cells[3]), f"profiles/r2_dram_traffic.csv ({cells[5]}, commit {cells[4]})"
+                return float(cells[3]), f"profiles/dram_traffic.csv ({cells[5]}, commit {cells[4]})"
     return None, None
 
 
