@@ -490,11 +490,9 @@ def run_dist(args, torch, H, rank, local, world, nccl):
     ms_per_step = max_over_ranks(ms_total, world, nccl) / args.steps
     launches = H.hcms_dist_last_launch_count(plan) * args.steps
 
-    # end to end: this rank's shard from pinned host memory, forward, its output shard back
+    # end to end through the C ABI: this rank's shards from pinned host memory, forward, its output shard back
     def step_e():
-        a, b, c_ = (t.to(dev, non_blocking=True) for t in host)
-        H.hcms_dist_attention_forward(plan, a, b, c_, out, w.scale)
-        host_out.copy_(out, non_blocking=True)
+        H.hcms_dist_attention_forward_host(plan, host[0], host[1], host[2], host_out, w.scale)
     n_e = min(args.steps, 10)
     for _ in range(2):
         step_e()
@@ -524,7 +522,7 @@ def run_dist(args, torch, H, rank, local, world, nccl):
                      "nvlink_bytes_per_rank_per_step": 4 * shard_bytes * (P - 1) // P},
         "e2e": {"value": round(flop_step / (ms_e * 1e-3) / 1e12, 2), "unit": UNIT, "h2d_bytes_per_step": 3 * shard_bytes * world,
                 "d2h_bytes_per_step": shard_bytes * world, "ms_per_step": round(ms_e, 3), "steps": n_e,
-                "api": "per rank: pinned host shard -> device, hcms_dist_attention_forward, output shard -> pinned host"},
+                "api": "hcms_dist_attention_forward_host per rank (pinned host shards -> device staging, the distributed forward, output shard -> pinned host)"},
     }
     torch.cuda.synchronize()
     barrier(world, True)

@@ -541,6 +541,12 @@ int hcms_dist_attach(hcms_dist_plan_t* plan, const void* handles, int n);
 int hcms_dist_attach_local(hcms_dist_plan_t* plan, hcms_dist_plan_t* const* peers, int n);
 int hcms_dist_attention_forward(hcms_dist_plan_t* plan, const void* q, const void* k, const void* v, void* out,
                                 float scale, void* stream);
+/* The same call with HOST shards (q, k, v, out: host pointers, bf16 [S/P, H, D]; pinned memory makes the copies asynchronous):
+ * H2D copies of the three input shards into plan-owned device staging (4 * S/P*H*D*2 bytes, allocated on first use) on
+ * `stream`, hcms_dist_attention_forward on the staging, D2H copy of this rank's output shard, then SYNCHRONISES `stream`.
+ * Every rank must make the call like the device form.  Same bits.  Errors: those of hcms_dist_attention_forward. */
+int hcms_dist_attention_forward_host(hcms_dist_plan_t* plan, const void* q, const void* k, const void* v, void* out,
+                                     float scale, void* stream);
 int hcms_dist_attention_forward_group(hcms_dist_plan_t* const* plans, int n, const void* const* q, const void* const* k,
                                       const void* const* v, void* const* out, float scale, void* const* streams);
 int hcms_dist_layer_forward(hcms_dist_plan_t* plan, const void* x, const void* w_qkv, const void* w_o, const void* rope_cos,

@@ -101,6 +101,7 @@ _SIGNATURES = {
     "hcms_dist_attach": (c_int, [c_void_p, c_void_p, c_int]),
     "hcms_dist_attach_local": (c_int, [c_void_p, POINTER(c_void_p), c_int]),
     "hcms_dist_attention_forward": (c_int, [c_void_p] * 5 + [c_float, c_void_p]),
+    "hcms_dist_attention_forward_host": (c_int, [c_void_p] * 5 + [c_float, c_void_p]),
     "hcms_dist_attention_forward_group": (c_int, [POINTER(c_void_p), c_int] + [POINTER(c_void_p)] * 4 + [c_float, POINTER(c_void_p)]),
     "hcms_dist_layer_forward": (c_int, [c_void_p] * 7 + [c_int, c_float, c_void_p]),
     "hcms_dist_layer_forward_group": (c_int, [POINTER(c_void_p), c_int, POINTER(c_void_p), c_void_p, c_void_p, POINTER(c_void_p),
@@ -507,6 +508,12 @@ def hcms_dist_attach_local(plan: DistPlan, peers) -> None:
 def hcms_dist_attention_forward(plan: DistPlan, q, k, v, out, scale: float, stream=None) -> None:
     _check(lib.hcms_dist_attention_forward(plan.handle, _ptr(q), _ptr(k), _ptr(v), _ptr(out), scale, _stream(stream)),
            "hcms_dist_attention_forward")
+
+
+def hcms_dist_attention_forward_host(plan: DistPlan, q, k, v, out, scale: float, stream=None) -> None:
+    """hcms_dist_attention_forward on HOST shards (pinned for asynchronous copies); synchronises the stream."""
+    _check(lib.hcms_dist_attention_forward_host(plan.handle, _ptr(q), _ptr(k), _ptr(v), _ptr(out), scale, _stream(stream)),
+           "hcms_dist_attention_forward_host")
 
 
 def hcms_dist_attention_forward_group(plans, qs, ks, vs, outs, scale: float, streams) -> None:

@@ -92,6 +92,7 @@ struct hcms_dist_plan {
   TmapCache tmaps;
   int last_launches = 0;
   int num_sms = 0;
+  void* staging[4] = {nullptr, nullptr, nullptr, nullptr};   // hcms_dist_attention_forward_host: device copies of q, k, v, out shards
 };
 
 static void dist_free(hcms_dist_plan_t* p) {
@@ -105,6 +106,7 @@ static void dist_free(hcms_dist_plan_t* p) {
   if (p->s_comm) cudaStreamDestroy(p->s_comm);
   if (p->s_comp) cudaStreamDestroy(p->s_comp);
   if (p->block) cudaFree(p->block);
+  for (void* b : p->staging) if (b) cudaFree(b);
   delete p;
 }
 
@@ -551,6 +553,26 @@ int hcms_dist_attention_forward(hcms_dist_plan_t* plan, const void* q, const voi
     return fail(HCMS_ERR_INVALID_ARG, "ranks attached with hcms_dist_attach_local are driven by hcms_dist_attention_forward_group "
                 "(a rank-by-rank enqueue from one process can deadlock on shared hardware queues)");
   return run_ranks(&rc, 1, scale, false);
+}
+
+int hcms_dist_attention_forward_host(hcms_dist_plan_t* plan, const void* q, const void* k, const void* v, void* out, float scale,
+                                     void* stream) {
+  if (!plan || !q || !k || !v || !out) return fail(HCMS_ERR_INVALID_ARG, "NULL argument");
+  const Shape& sh = plan->sh;
+  const size_t bytes = static_cast<size_t>(plan->Sl) * sh.H * sh.D * sh.es;
+  for (const void* in : {q, k, v})
+    if (overlaps(out, bytes, in, bytes)) return fail(HCMS_ERR_ALIAS, "out overlaps an input tensor");
+  if (int ps = check_plan_state(plan, false)) return ps;      // before the staging is touched: attached, healthy, right device
+  for (void*& b : plan->staging)
+    if (!b) HCMS_CUDA(cudaMalloc(&b, bytes));
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const void* host_in[3] = {q, k, v};
+  for (int t = 0; t < 3; ++t) HCMS_CUDA(cudaMemcpyAsync(plan->staging[t], host_in[t], bytes, cudaMemcpyHostToDevice, st));
+  const int status = hcms_dist_attention_forward(plan, plan->staging[0], plan->staging[1], plan->staging[2], plan->staging[3], scale, stream);
+  if (status != HCMS_OK) return status;                       // the failed call has joined its streams; nothing to copy back
+  HCMS_CUDA(cudaMemcpyAsync(out, plan->staging[3], bytes, cudaMemcpyDeviceToHost, st));
+  HCMS_CUDA(cudaStreamSynchronize(st));
+  return HCMS_OK;
 }
 
 int hcms_dist_attention_forward_group(hcms_dist_plan_t* const* plans, int n, const void* const* q, const void* const* k,

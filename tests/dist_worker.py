@@ -72,6 +72,12 @@ def worker(rank, world, port, a):
             if rep == 2:
                 from oracle import hcms_oracle as O
                 check_against_oracle(gathered, O.attention_full(q, k, v, w.scale), f"{world} processes")
+    # the host-buffer entry point: pinned host shards in, this rank's output shard out, same bits as the device call
+    host_in = [t.cpu().pin_memory() for t in dev]
+    host_out = torch.full_like(host_in[0], 0x7FC0).pin_memory()
+    dist.barrier()
+    H.hcms_dist_attention_forward_host(plan, host_in[0], host_in[1], host_in[2], host_out, w.scale)
+    assert torch.equal(host_out, out.cpu()), "hcms_dist_attention_forward_host differs from the device call"
     torch.cuda.synchronize()
     dist.barrier()                                           # nobody unmaps while a peer may still read
     plan.close()
@@ -308,6 +314,12 @@ def local_fail(a):
         H.hcms_dist_attention_forward(pl, qd, kd, vd, out1, w.scale)
         torch.cuda.synchronize()
         assert torch.equal(out1, want)
+        host_in = [t.cpu().pin_memory() for t in (qd, kd, vd)]
+        host_out = torch.full_like(host_in[0], 0x7FC0).pin_memory()
+        H.hcms_dist_attention_forward_host(pl, host_in[0], host_in[1], host_in[2], host_out, w.scale)
+        assert torch.equal(host_out, want.cpu())
+        assert status_of(lambda: H.hcms_dist_attention_forward_host(pl, host_in[0], host_in[1], host_in[2], host_in[0], w.scale))[0] \
+            == H.HCMS_ERR_ALIAS
     print("DIST_OK", flush=True)
 
 
