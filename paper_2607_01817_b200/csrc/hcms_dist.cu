@@ -29,8 +29,22 @@ namespace {
 using WaitValueFn = CUresult (*)(CUstream, CUdeviceptr, cuuint32_t, unsigned int);
 WaitValueFn g_wait_value = nullptr;
 
+// cuStreamBatchMemOp: the P flag waits of one chunk as ONE stream operation (P = 8, C = 4: 8 operations per call on each
+// stream instead of 64).  Optional: without it the waits are enqueued one by one.
+using BatchMemOpFn = CUresult (*)(CUstream, unsigned int, CUstreamBatchMemOpParams*, unsigned int);
+BatchMemOpFn g_batch_mem_op = nullptr;
+
 int resolve_wait_value() {
   if (g_wait_value) return HCMS_OK;
+  {
+    void* bfn = nullptr;
+    cudaDriverEntryPointQueryResult bres;
+    if (cudaGetDriverEntryPoint("cuStreamBatchMemOp", &bfn, cudaEnableDefault, &bres) == cudaSuccess &&
+        bres == cudaDriverEntryPointSuccess && bfn)
+      g_batch_mem_op = reinterpret_cast<BatchMemOpFn>(bfn);
+    else
+      cudaGetLastError();
+  }
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qres;
   cudaError_t e = cudaGetDriverEntryPoint("cuStreamWaitValue32", &fn, cudaEnableDefault, &qres);
@@ -362,6 +376,19 @@ int enqueue_phase(const RankCall& rc, int phase, float scale) {
     return cuda(cudaGetLastError(), "signal launch");
   };
   auto wait_all = [&](int which, int c, cudaStream_t s) {        // until flag[which][c][p] >= epoch for every p (local memory)
+    if (g_batch_mem_op && P > 1) {
+      CUstreamBatchMemOpParams ops[kMaxPeers];
+      std::memset(ops, 0, sizeof(ops));
+      for (int p = 0; p < P; ++p) {
+        ops[p].waitValue.operation = CU_STREAM_MEM_OP_WAIT_VALUE_32;
+        ops[p].waitValue.address = reinterpret_cast<CUdeviceptr>(flag_ptr(plan, plan->block, which, c, p));
+        ops[p].waitValue.value = epoch;
+        ops[p].waitValue.flags = CU_STREAM_WAIT_VALUE_GEQ;
+      }
+      const CUresult cr = g_batch_mem_op(reinterpret_cast<CUstream>(s), static_cast<unsigned>(P), ops, 0);
+      if (cr != CUDA_SUCCESS) status = fail(HCMS_ERR_CUDA, "cuStreamBatchMemOp failed with CUresult %d", static_cast<int>(cr));
+      return status == HCMS_OK;
+    }
     for (int p = 0; p < P && status == HCMS_OK; ++p) {
       const CUresult cr = g_wait_value(reinterpret_cast<CUstream>(s),
                                        reinterpret_cast<CUdeviceptr>(flag_ptr(plan, plan->block, which, c, p)), epoch,
