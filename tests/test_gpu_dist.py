@@ -36,10 +36,10 @@ def _emulation(q, k, v, S, Hh, D, P, C, scale):
     return to_host(out)
 
 
-def _run_worker(mode, P, S, Hh, D, C, env=None, flags=0, layer=0):
+def _run_worker(mode, P, S, Hh, D, C, env=None, flags=0, layer=0, timeout=240):
     cmd = [sys.executable, os.path.join(ROOT, "tests", "dist_worker.py"), mode, str(P), "--S", str(S), "--H", str(Hh),
            "--D", str(D), "--C", str(C), "--flags", str(flags), "--layer", str(layer)]
-    r = subprocess.run(cmd, capture_output=True, text=True, timeout=240, cwd=ROOT, env=dict(os.environ, **(env or {})))
+    r = subprocess.run(cmd, capture_output=True, text=True, timeout=timeout, cwd=ROOT, env=dict(os.environ, **(env or {})))
     assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-3000:]
     assert "DIST_OK" in r.stdout, r.stdout[-2000:]
 
@@ -62,6 +62,19 @@ def test_emulation_matches_oracle_on_the_dist_shapes():
     err = np.abs(bf16_bits_to_f64(want) - ref)
     assert err.max() <= 2e-2 and err.mean() <= 2e-3
     assert np.linalg.norm(bf16_bits_to_f64(want) - ref) / np.linalg.norm(ref) <= 1e-2
+
+
+@pytest.mark.parametrize("cfg,P,flags,layer", [(3, 4, 0, 0), (3, 4, H.HCMS_FLAG_DIST_FUSE_OUT, 0), (3, 4, 0, 1),
+                                              (4, 8, 0, 0), (4, 8, H.HCMS_FLAG_DIST_FUSE_OUT, 0)],
+                         ids=["cfg3-4ranks-pull", "cfg3-4ranks-fused-out", "cfg3-4ranks-layer", "cfg4-8ranks-pull", "cfg4-8ranks-fused-out"])
+def test_full_size_ranks_in_one_process(cfg, P, flags, layer):
+    """BASELINE.json's full shapes between in-process ranks: cfg 3 as 4 ranks (shards of 8190 rows: output tiles straddle
+    two ranks' shards, GB-sized exchange blocks, more than one wave per launch) and cfg 4 as 8 ranks (shards of 7020 rows,
+    chunks 3 + 2); push scatter + pull gather, the fused output push, and the whole layer with both all-to-alls inside the
+    GEMM / attention epilogues (48 chunk maps).  Bit-equal to the emulation on all three calls; attention forms also
+    against the fp64 oracle on sampled rows (shard boundaries + seeded rows)."""
+    w = I.workload(cfg)
+    _run_worker("--local", P, w.S, w.H, w.D, w.C, flags=flags, layer=layer, timeout=500)
 
 
 def test_failed_forward_joins_and_poisons_instead_of_hanging():
